@@ -1,0 +1,208 @@
+"""B200-native spectral Ewald for the triply periodic Stokeslet sum (arXiv 2606.19059).
+
+Thin ctypes binding over the C-ABI in include/se.h (libse_b200.so, built in-tree by
+`python -m paper_2606_19059_b200.build`).  Argument marshalling only: every step of the
+path runs in the library's CUDA kernels.  PyTorch supplies device memory and streams.
+There is no CPU fallback: a missing library or a missing GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libse_b200.so"
+
+SE_FP64, SE_FP32 = 0, 1
+STAGES = ("sort", "p2p", "p2g", "fft", "scale", "ifft", "g2p", "sum")
+(SE_STAGE_SORT, SE_STAGE_P2P, SE_STAGE_P2G, SE_STAGE_FFT, SE_STAGE_SCALE, SE_STAGE_IFFT,
+ SE_STAGE_G2P, SE_STAGE_SUM) = range(8)
+SE_NSTAGES = 8
+(SE_BUF_UN, SE_BUF_UF, SE_BUF_GRID, SE_BUF_SPEC, SE_BUF_PERM_NEAR, SE_BUF_PERM_GRID,
+ SE_BUF_CELL_START, SE_BUF_BIN_START) = range(8)
+
+EXPORTS = ("se_plan_create", "se_eval", "se_eval_host", "se_plan_destroy", "se_strerror",
+           "se_plan_info", "se_eval_stage", "se_buffer_read", "se_buffer_write",
+           "se_set_profiling", "se_stage_ms", "se_last_launch_count")
+
+
+class SeInfo(C.Structure):
+    _fields_ = [("N", C.c_int64), ("M", C.c_int), ("P", C.c_int), ("precision", C.c_int),
+                ("L", C.c_double), ("xi", C.c_double), ("rc", C.c_double), ("h", C.c_double),
+                ("m", C.c_double), ("eta", C.c_double), ("a", C.c_double), ("cw", C.c_double),
+                ("ncell", C.c_int), ("nbin", C.c_int), ("nmodes", C.c_int64),
+                ("workspace_bytes", C.c_size_t)]
+
+
+class SeError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().se_strerror(status).decode() if status >= 0 else "?"
+        super().__init__(f"{where}: {msg} (se_status {status})")
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libse_b200.so; raises if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise ImportError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_2606_19059_b200.build` "
+                "(nvcc, sm_100a).  This package has no CPU or PyTorch fallback.")
+        L = C.CDLL(str(LIB_PATH))
+        vp, i64, dbl, i32 = C.c_void_p, C.c_int64, C.c_double, C.c_int
+        L.se_plan_create.argtypes = [C.POINTER(vp), i64, dbl, dbl, dbl, i32, i32, i32]
+        L.se_eval.argtypes = [vp, vp, vp, vp, vp]
+        L.se_eval_host.argtypes = [vp, vp, vp, vp, vp]
+        L.se_plan_destroy.argtypes = [vp]
+        L.se_strerror.argtypes = [i32]
+        L.se_strerror.restype = C.c_char_p
+        L.se_plan_info.argtypes = [vp, C.POINTER(SeInfo)]
+        L.se_eval_stage.argtypes = [vp, i32, vp, vp, vp, vp]
+        L.se_buffer_read.argtypes = [vp, i32, vp, C.c_size_t, C.POINTER(C.c_size_t), vp]
+        L.se_buffer_write.argtypes = [vp, i32, vp, C.c_size_t, vp]
+        L.se_set_profiling.argtypes = [vp, i32]
+        L.se_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
+        L.se_last_launch_count.argtypes = [vp, C.POINTER(i32)]
+        for name in EXPORTS:
+            if name != "se_strerror":
+                getattr(L, name).restype = i32
+        _lib = L
+    return _lib
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        raise SeError(status, where)
+
+
+def _stream_ptr(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+class Plan:
+    """se_plan_create / se_eval / se_plan_destroy with torch tensors for memory."""
+
+    def __init__(self, N, L, xi, rc, M, P, precision="fp64"):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_19059_b200 needs a CUDA device (no CPU fallback)")
+        self._h = C.c_void_p()
+        self.precision = precision
+        self.dtype = torch.float64 if precision == "fp64" else torch.float32
+        prec = {"fp64": SE_FP64, "fp32": SE_FP32}[precision]
+        _check(lib().se_plan_create(C.byref(self._h), int(N), float(L), float(xi), float(rc), int(M), int(P), prec),
+               "se_plan_create")
+        self.N, self.M, self.P = int(N), int(M), int(P)
+
+    # -- lifetime -----------------------------------------------------------------------
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().se_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.destroy()
+
+    # -- helpers --------------------------------------------------------------------------
+    def _dev(self, t, name):
+        if t is None:
+            return C.c_void_p()
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == self.dtype):
+            raise ValueError(f"{name}: need a contiguous CUDA tensor of dtype {self.dtype}")
+        if t.numel() != 3 * self.N:
+            raise ValueError(f"{name}: need N x 3 = {3 * self.N} elements, got {t.numel()}")
+        return C.c_void_p(t.data_ptr())
+
+    def info(self) -> SeInfo:
+        out = SeInfo()
+        _check(lib().se_plan_info(self._h, C.byref(out)), "se_plan_info")
+        return out
+
+    # -- evaluation -------------------------------------------------------------------------
+    def eval(self, x, f, u=None, stream=None):
+        import torch
+        if u is None:
+            u = torch.empty((self.N, 3), dtype=self.dtype, device=x.device)
+        _check(lib().se_eval(self._h, self._dev(x, "x"), self._dev(f, "f"), self._dev(u, "u"), _stream_ptr(stream)),
+               "se_eval")
+        return u
+
+    def eval_host(self, x_host, f_host, u_host, stream=None):
+        """x_host, f_host, u_host: CPU tensors (ideally pinned); async on the stream."""
+        for t in (x_host, f_host, u_host):
+            if t.is_cuda or not t.is_contiguous() or t.dtype != self.dtype or t.numel() != 3 * self.N:
+                raise ValueError("eval_host: need contiguous CPU tensors N x 3 of the plan's dtype")
+        _check(lib().se_eval_host(self._h, C.c_void_p(x_host.data_ptr()), C.c_void_p(f_host.data_ptr()),
+                                  C.c_void_p(u_host.data_ptr()), _stream_ptr(stream)), "se_eval_host")
+        return u_host
+
+    def stage(self, stage, x=None, f=None, u=None, stream=None):
+        if isinstance(stage, str):
+            stage = STAGES.index(stage)
+        _check(lib().se_eval_stage(self._h, int(stage), self._dev(x, "x"), self._dev(f, "f"), self._dev(u, "u"),
+                                   _stream_ptr(stream)), f"se_eval_stage({stage})")
+
+    # -- buffers ------------------------------------------------------------------------------
+    def _buf_shape(self, which):
+        import torch
+        N, M = self.N, self.M
+        i = self.info()
+        if which in (SE_BUF_UN, SE_BUF_UF):
+            return (N, 3), self.dtype
+        if which == SE_BUF_GRID:
+            return (3, M, M, M), self.dtype
+        if which == SE_BUF_SPEC:
+            return (3, M, M, M // 2 + 1, 2), self.dtype
+        if which in (SE_BUF_PERM_NEAR, SE_BUF_PERM_GRID):
+            return (N,), torch.int32
+        if which == SE_BUF_CELL_START:
+            return (i.ncell ** 3 + 1,), torch.int32
+        if which == SE_BUF_BIN_START:
+            return (i.nbin ** 3 + 1,), torch.int32
+        raise ValueError(which)
+
+    def read(self, which, stream=None):
+        import torch
+        shape, dt = self._buf_shape(which)
+        out = torch.empty(shape, dtype=dt, device="cuda")
+        nbytes = out.numel() * out.element_size()
+        _check(lib().se_buffer_read(self._h, which, C.c_void_p(out.data_ptr()), nbytes, None, _stream_ptr(stream)),
+               "se_buffer_read")
+        return out
+
+    def write(self, which, t, stream=None):
+        shape, dt = self._buf_shape(which)
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == dt):
+            raise ValueError("write: need a contiguous CUDA tensor of the buffer's dtype")
+        nbytes = t.numel() * t.element_size()
+        _check(lib().se_buffer_write(self._h, which, C.c_void_p(t.data_ptr()), nbytes, _stream_ptr(stream)),
+               "se_buffer_write")
+
+    # -- timing ---------------------------------------------------------------------------------
+    def set_profiling(self, on: bool):
+        _check(lib().se_set_profiling(self._h, int(bool(on))), "se_set_profiling")
+
+    def stage_ms(self):
+        arr = (C.c_float * SE_NSTAGES)()
+        _check(lib().se_stage_ms(self._h, arr), "se_stage_ms")
+        return dict(zip(STAGES, [float(v) for v in arr]))
+
+    def launch_count(self) -> int:
+        n = C.c_int()
+        _check(lib().se_last_launch_count(self._h, C.byref(n)), "se_last_launch_count")
+        return n.value

@@ -1,0 +1,320 @@
+// C-ABI of libse_b200.so (declared in include/se.h): plan management, cuFFT plumbing,
+// stage sequencing.  All arithmetic of the method lives in the kernels of se_sort.cu (K1, K6),
+// se_p2p.cu (K2), se_grid.cu (K3, K5), se_scale.cu (K4); the two FFT steps of Algorithm 2.1
+// are cuFFT R2C / C2R with batch 3.
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "se_common.cuh"
+
+namespace {
+
+struct Alloc {
+    se_plan *p;
+    bool ok = true;
+    template <typename T> void get(T **dst, size_t bytes)
+    {
+        *dst = nullptr;
+        if (!ok) return;
+        void *q = nullptr;
+        if (bytes == 0) bytes = 16;
+        if (cudaMalloc(&q, bytes) != cudaSuccess) { ok = false; cudaGetLastError(); return; }
+        p->workspace_bytes += bytes;
+        *dst = (T *)q;
+    }
+};
+
+void free_all(se_plan *p)
+{
+    if (!p) return;
+    void *ptrs[] = {p->cell_of, p->cell_start, p->cell_cursor, p->perm_near, p->inv_near, p->cell_sorted,
+                    p->xs_near, p->fs_near, p->uN, p->bin_of, p->bin_start, p->bin_cursor, p->perm_grid,
+                    p->inv_grid, p->anchor, p->wtab, p->fs_grid, p->uF, p->grid, p->spec, p->ktab,
+                    p->hx, p->hf, p->hu};
+    for (void *q : ptrs) if (q) cudaFree(q);
+    if (p->fft_ok & 1) cufftDestroy(p->fft_fwd);
+    if (p->fft_ok & 2) cufftDestroy(p->fft_inv);
+    if (p->ev_ok) for (int i = 0; i <= SE_NSTAGES; ++i) cudaEventDestroy(p->ev[i]);
+    delete p;
+}
+
+se_status run_fft(se_plan *p, bool forward, cudaStream_t s)
+{
+    cufftHandle h = forward ? p->fft_fwd : p->fft_inv;
+    if (cufftSetStream(h, s) != CUFFT_SUCCESS) return SE_ECUFFT;
+    cufftResult r;
+    if (p->precision == SE_FP64)
+        r = forward ? cufftExecD2Z(h, (cufftDoubleReal *)p->grid, (cufftDoubleComplex *)p->spec)
+                    : cufftExecZ2D(h, (cufftDoubleComplex *)p->spec, (cufftDoubleReal *)p->grid);
+    else
+        r = forward ? cufftExecR2C(h, (cufftReal *)p->grid, (cufftComplex *)p->spec)
+                    : cufftExecC2R(h, (cufftComplex *)p->spec, (cufftReal *)p->grid);
+    return r == CUFFT_SUCCESS ? SE_OK : SE_ECUFFT;
+}
+
+se_status run_stage(se_plan *p, int stage, const void *x, const void *f, void *u, cudaStream_t s)
+{
+    cudaError_t e = cudaSuccess;
+    switch (stage) {
+    case SE_STAGE_SORT:
+        if (!x || !f) return SE_EINVAL;
+        e = se_launch_sort(p, x, f, s);
+        break;
+    case SE_STAGE_P2P: e = se_launch_p2p(p, s); break;
+    case SE_STAGE_P2G: e = se_launch_p2g(p, s); break;
+    case SE_STAGE_FFT: return run_fft(p, true, s);
+    case SE_STAGE_SCALE: e = se_launch_scale(p, s); break;
+    case SE_STAGE_IFFT: return run_fft(p, false, s);
+    case SE_STAGE_G2P: e = se_launch_g2p(p, s); break;
+    case SE_STAGE_SUM:
+        if (!f || !u) return SE_EINVAL;
+        e = se_launch_sum(p, f, u, s);
+        break;
+    default: return SE_EINVAL;
+    }
+    return e == cudaSuccess ? SE_OK : SE_ECUDA;
+}
+
+size_t buffer_bytes(const se_plan *p, int which, void **ptr)
+{
+    const SeGeom &g = p->g;
+    size_t rb = p->real_bytes;
+    size_t M3 = (size_t)g.M * g.M * g.M, nm = (size_t)g.M * g.M * (g.M / 2 + 1);
+    switch (which) {
+    case SE_BUF_UN: *ptr = p->uN; return (size_t)g.N * 3 * rb;
+    case SE_BUF_UF: *ptr = p->uF; return (size_t)g.N * 3 * rb;
+    case SE_BUF_GRID: *ptr = p->grid; return 3 * M3 * rb;
+    case SE_BUF_SPEC: *ptr = p->spec; return 3 * nm * 2 * rb;
+    case SE_BUF_PERM_NEAR: *ptr = p->perm_near; return (size_t)g.N * sizeof(int);
+    case SE_BUF_PERM_GRID: *ptr = p->perm_grid; return (size_t)g.N * sizeof(int);
+    case SE_BUF_CELL_START: *ptr = p->cell_start; return ((size_t)g.ncell * g.ncell * g.ncell + 1) * sizeof(int);
+    case SE_BUF_BIN_START: *ptr = p->bin_start; return ((size_t)g.nbin * g.nbin * g.nbin + 1) * sizeof(int);
+    default: *ptr = nullptr; return 0;
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *se_strerror(se_status s)
+{
+    switch (s) {
+    case SE_OK: return "ok";
+    case SE_EINVAL: return "invalid argument";
+    case SE_ENOMEM: return "out of memory";
+    case SE_ECUDA: return "CUDA error";
+    case SE_ECUFFT: return "cuFFT error";
+    default: return "unknown status";
+    }
+}
+
+se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double rc, int M, int P,
+                         se_precision prec)
+{
+    if (!out) return SE_EINVAL;
+    *out = nullptr;
+    if (!(N >= 1) || N >= ((int64_t)1 << 31) || !(L > 0) || !(xi > 0) || !(rc > 0) || !std::isfinite(L) ||
+        !std::isfinite(xi) || !std::isfinite(rc))
+        return SE_EINVAL;
+    if (M < 2 || (M & 1) || M > 4096 || P < 2 || (P & 1) || P > SE_PMAX || P > M) return SE_EINVAL;
+    if (prec != SE_FP64 && prec != SE_FP32) return SE_EINVAL;
+    double ncd = std::floor(L / rc);
+    if (!(ncd >= 3)) return SE_EINVAL;
+    int ncell = ncd > 1024 ? 1024 : (int)ncd;          // more cells than this only wastes memory
+
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return SE_ECUDA; }
+
+    se_plan *p = new (std::nothrow) se_plan();
+    if (!p) return SE_ENOMEM;
+    std::memset(p, 0, sizeof(*p));
+    p->device = dev;
+    p->precision = (int)prec;
+    p->real_bytes = prec == SE_FP64 ? 8 : 4;
+    SeGeom &g = p->g;
+    g.N = N; g.M = M; g.P = P; g.L = L; g.xi = xi; g.rc = rc;
+    g.ncell = ncell;
+    g.nbin = (M + SE_BIN - 1) / SE_BIN;
+    g.rel_coords = prec == SE_FP32;
+    g.h = L / M;
+    g.wcell = L / ncell;
+    double m = 0.95 * std::sqrt(SE_PI * P);             // reading S4
+    g.eta = (P * g.h * xi / m) * (P * g.h * xi / m);
+    double a = 2.0 * xi * xi / g.eta;
+    g.beta = a * g.h * g.h;
+    g.cw = std::pow(a / SE_PI, 1.5);
+
+    size_t rb = p->real_bytes;
+    size_t nc3 = (size_t)ncell * ncell * ncell, nb3 = (size_t)g.nbin * g.nbin * g.nbin;
+    size_t M3 = (size_t)M * M * M, nm = (size_t)M * M * (M / 2 + 1);
+    size_t scan_tiles = (std::max(nc3, nb3) + 2047) / 2048 + 1;
+
+    Alloc A{p};
+    A.get(&p->cell_of, N * sizeof(int));
+    A.get(&p->cell_start, (nc3 + 1 + scan_tiles) * sizeof(int));
+    A.get(&p->cell_cursor, (nc3 + 1) * sizeof(int));
+    A.get(&p->perm_near, N * sizeof(int));
+    A.get(&p->inv_near, N * sizeof(int));
+    A.get(&p->cell_sorted, N * sizeof(int));
+    A.get(&p->xs_near, N * 3 * rb);
+    A.get(&p->fs_near, N * 3 * rb);
+    A.get(&p->uN, N * 3 * rb);
+    A.get(&p->bin_of, N * sizeof(int));
+    A.get(&p->bin_start, (nb3 + 1 + scan_tiles) * sizeof(int));
+    A.get(&p->bin_cursor, (nb3 + 1) * sizeof(int));
+    A.get(&p->perm_grid, N * sizeof(int));
+    A.get(&p->inv_grid, N * sizeof(int));
+    A.get(&p->anchor, N * sizeof(short4));
+    A.get(&p->wtab, (size_t)N * 3 * P * rb);
+    A.get(&p->fs_grid, N * 3 * rb);
+    A.get(&p->uF, std::max((size_t)N * 3 * rb, (size_t)N * sizeof(int)));
+    A.get(&p->grid, 3 * M3 * rb);
+    A.get(&p->spec, 3 * nm * 2 * rb);
+    A.get(&p->ktab, 2 * (size_t)M * rb);
+    if (!A.ok) { free_all(p); return SE_ENOMEM; }
+
+    // cuFFT: batch of 3 out-of-place 3-D transforms, contiguous, z fastest, halved axis last
+    int n[3] = {M, M, M};
+    cufftType tf = prec == SE_FP64 ? CUFFT_D2Z : CUFFT_R2C, ti = prec == SE_FP64 ? CUFFT_Z2D : CUFFT_C2R;
+    size_t wsz = 0;
+    cufftResult r = cufftPlanMany(&p->fft_fwd, 3, n, nullptr, 1, (int)0, nullptr, 1, (int)0, tf, 3);
+    if (r == CUFFT_SUCCESS) {
+        p->fft_ok |= 1;
+        if (cufftGetSize(p->fft_fwd, &wsz) == CUFFT_SUCCESS) p->fft_work_bytes += wsz;
+        r = cufftPlanMany(&p->fft_inv, 3, n, nullptr, 1, (int)0, nullptr, 1, (int)0, ti, 3);
+    }
+    if (r == CUFFT_SUCCESS) {
+        p->fft_ok |= 2;
+        if (cufftGetSize(p->fft_inv, &wsz) == CUFFT_SUCCESS) p->fft_work_bytes += wsz;
+    } else {
+        se_status st = (r == CUFFT_ALLOC_FAILED) ? SE_ENOMEM : SE_ECUFFT;
+        free_all(p);
+        return st;
+    }
+    p->workspace_bytes += p->fft_work_bytes;
+
+    if (se_build_ktab(p) != cudaSuccess) { cudaGetLastError(); free_all(p); return SE_ECUDA; }
+    for (int i = 0; i <= SE_NSTAGES; ++i)
+        if (cudaEventCreate(&p->ev[i]) != cudaSuccess) { free_all(p); return SE_ECUDA; }
+    p->ev_ok = 1;
+    *out = p;
+    return SE_OK;
+}
+
+se_status se_plan_destroy(se_plan *p)
+{
+    if (!p) return SE_OK;
+    cudaDeviceSynchronize();
+    free_all(p);
+    return SE_OK;
+}
+
+se_status se_plan_info(const se_plan *p, se_info *o)
+{
+    if (!p || !o) return SE_EINVAL;
+    const SeGeom &g = p->g;
+    o->N = g.N; o->M = g.M; o->P = g.P; o->precision = p->precision;
+    o->L = g.L; o->xi = g.xi; o->rc = g.rc; o->h = g.h;
+    o->m = 0.95 * std::sqrt(SE_PI * g.P);
+    o->eta = g.eta;
+    o->a = g.beta / (g.h * g.h);
+    o->cw = g.cw;
+    o->ncell = g.ncell; o->nbin = g.nbin;
+    o->nmodes = (int64_t)g.M * g.M * (g.M / 2 + 1);
+    o->workspace_bytes = p->workspace_bytes;
+    return SE_OK;
+}
+
+se_status se_eval(se_plan *p, const void *x, const void *f, void *u, void *stream)
+{
+    if (!p || !x || !f || !u) return SE_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    p->launches = 0;
+    p->ev_recorded = 0;
+    const bool prof = p->profiling != 0;
+    if (prof && cudaEventRecord(p->ev[0], s) != cudaSuccess) return SE_ECUDA;
+    for (int st = 0; st < SE_NSTAGES; ++st) {
+        se_status r = run_stage(p, st, x, f, u, s);
+        if (r != SE_OK) return r;
+        if (prof && cudaEventRecord(p->ev[st + 1], s) != cudaSuccess) return SE_ECUDA;
+    }
+    if (prof) p->ev_recorded = 1;
+    return SE_OK;
+}
+
+se_status se_eval_host(se_plan *p, const void *xh, const void *fh, void *uh, void *stream)
+{
+    if (!p || !xh || !fh || !uh) return SE_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    size_t bytes = (size_t)p->g.N * 3 * p->real_bytes;
+    if (!p->hx) {
+        Alloc A{p};
+        A.get(&p->hx, bytes); A.get(&p->hf, bytes); A.get(&p->hu, bytes);
+        if (!A.ok) return SE_ENOMEM;
+    }
+    if (cudaMemcpyAsync(p->hx, xh, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) return SE_ECUDA;
+    if (cudaMemcpyAsync(p->hf, fh, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) return SE_ECUDA;
+    se_status r = se_eval(p, p->hx, p->hf, p->hu, stream);
+    if (r != SE_OK) return r;
+    if (cudaMemcpyAsync(uh, p->hu, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) return SE_ECUDA;
+    return SE_OK;
+}
+
+se_status se_eval_stage(se_plan *p, int stage, const void *x, const void *f, void *u, void *stream)
+{
+    if (!p) return SE_EINVAL;
+    return run_stage(p, stage, x, f, u, (cudaStream_t)stream);
+}
+
+se_status se_buffer_read(se_plan *p, int which, void *dst, size_t bytes, size_t *size_out, void *stream)
+{
+    if (!p) return SE_EINVAL;
+    void *src = nullptr;
+    size_t n = buffer_bytes(p, which, &src);
+    if (!src) return SE_EINVAL;
+    if (size_out) *size_out = n;
+    if (!dst) return SE_OK;
+    if (bytes != n) return SE_EINVAL;
+    return cudaMemcpyAsync(dst, src, n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream) == cudaSuccess ? SE_OK
+                                                                                                         : SE_ECUDA;
+}
+
+se_status se_buffer_write(se_plan *p, int which, const void *srcv, size_t bytes, void *stream)
+{
+    if (!p || !srcv) return SE_EINVAL;
+    void *dst = nullptr;
+    size_t n = buffer_bytes(p, which, &dst);
+    if (!dst || bytes != n) return SE_EINVAL;
+    return cudaMemcpyAsync(dst, srcv, n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream) == cudaSuccess ? SE_OK
+                                                                                                          : SE_ECUDA;
+}
+
+se_status se_set_profiling(se_plan *p, int on)
+{
+    if (!p) return SE_EINVAL;
+    p->profiling = on != 0;
+    return SE_OK;
+}
+
+se_status se_stage_ms(se_plan *p, float ms[SE_NSTAGES])
+{
+    if (!p || !ms) return SE_EINVAL;
+    if (!p->ev_recorded) return SE_EINVAL;
+    if (cudaEventSynchronize(p->ev[SE_NSTAGES]) != cudaSuccess) return SE_ECUDA;
+    for (int st = 0; st < SE_NSTAGES; ++st)
+        if (cudaEventElapsedTime(&ms[st], p->ev[st], p->ev[st + 1]) != cudaSuccess) return SE_ECUDA;
+    return SE_OK;
+}
+
+se_status se_last_launch_count(const se_plan *p, int *count)
+{
+    if (!p || !count) return SE_EINVAL;
+    *count = p->launches;
+    return SE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,87 @@
+// Internal definitions shared by the kernels of libse_b200.so (sm_100a only).
+// Boundary and semantics: include/se.h.  Paper citations are PAPER.md line numbers.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+
+#include "../../include/se.h"
+
+#define SE_PI 3.14159265358979323846264338327950288
+
+// ---- geometry of the gridding kernels (K3 P2G / K5 G2P) ---------------------------------
+// Output tile owned by one block: TX x TY x TZ grid points; one thread per (x,y) column,
+// TZ accumulators x 3 components in registers.  Particles are sorted by bins of BIN^3
+// grid cells (z fastest) so that the candidates of a tile are a few contiguous runs.
+constexpr int SE_TX = 16;
+constexpr int SE_TY = 16;
+constexpr int SE_TZ = 8;
+constexpr int SE_BIN = 8;
+constexpr int SE_GRID_THREADS = SE_TX * SE_TY;      // 256
+constexpr int SE_ROUND = 128;                        // candidates examined per staging round
+constexpr int SE_PMAX = 32;                          // largest window support
+
+struct SeGeom {
+    int64_t N;
+    int M, P;
+    int ncell;          // near cells per dimension
+    int nbin;           // grid bins per dimension = ceil(M / SE_BIN)
+    int rel_coords;     // 1: near-sorted positions are cell-relative (fp32 path)
+    double L, xi, rc;
+    double h;           // L / M
+    double wcell;       // L / ncell
+    double beta;        // a h^2 : window = exp(-beta (l' - frac)^2) in grid units
+    double cw;          // (a/pi)^{3/2}
+    double eta;
+};
+
+struct se_plan {
+    SeGeom g;
+    int precision;
+    int device;
+    int profiling;
+    int launches;
+    size_t real_bytes;             // sizeof(Real)
+    // near field (K1a, K2)
+    int *cell_of;                  // [N]  near cell of user particle i
+    int *cell_start;               // [ncell^3 + 1]
+    int *cell_cursor;              // [ncell^3 + 1] scatter cursors
+    int *perm_near;                // [N] sorted pos -> user index
+    int *inv_near;                 // [N] user index -> sorted pos
+    int *cell_sorted;              // [N] near cell of sorted particle
+    void *xs_near;                 // [N][3] Real  (absolute fp64 / cell-relative fp32)
+    void *fs_near;                 // [N][3] Real
+    void *uN;                      // [N][3] Real, near-sorted order
+    // grid path (K1b, K3, K5)
+    int *bin_of;                   // [N]
+    int *bin_start;                // [nbin^3 + 1]
+    int *bin_cursor;               // [nbin^3 + 1]
+    int *perm_grid;                // [N]
+    int *inv_grid;                 // [N]
+    short4 *anchor;                // [N] (a_x, a_y, a_z, 0): anchor grid index in [0, M)
+    void *wtab;                    // [N][3][P] Real: 1-D window values of every particle
+    void *fs_grid;                 // [N][3] Real
+    void *uF;                      // [N][3] Real, grid-sorted order (unscaled sum)
+    // grids
+    void *grid;                    // [3][M][M][M] Real
+    void *spec;                    // [3][M][M][M/2+1] complex Real
+    void *ktab;                    // [2][M] Real : k value, exp factor per 1-D index
+    cufftHandle fft_fwd, fft_inv;
+    int fft_ok;
+    size_t fft_work_bytes;
+    // host-buffer entry point staging
+    void *hx, *hf, *hu;            // device staging [N][3] Real each
+    size_t workspace_bytes;
+    cudaEvent_t ev[SE_NSTAGES + 1];
+    int ev_ok, ev_recorded;
+};
+
+// ---- launchers implemented in the .cu files -------------------------------------------------
+cudaError_t se_launch_sort(se_plan *p, const void *x, const void *f, cudaStream_t s);
+cudaError_t se_launch_p2p(se_plan *p, cudaStream_t s);
+cudaError_t se_launch_p2g(se_plan *p, cudaStream_t s);
+cudaError_t se_launch_scale(se_plan *p, cudaStream_t s);
+cudaError_t se_launch_g2p(se_plan *p, cudaStream_t s);
+cudaError_t se_launch_sum(se_plan *p, const void *f, void *u, cudaStream_t s);
+cudaError_t se_build_ktab(se_plan *p);

@@ -1,0 +1,291 @@
+// K1: wrap + bin + counting sort, for both orderings the later stages need
+//   (a) near cells of width L/ncell >= rc  -> K2 P2P
+//   (b) grid bins of SE_BIN^3 Fourier-grid cells (the paper's C^F) -> K3 P2G, K5 G2P
+// Unlike the paper's padded cell lists (two passes + max-occupancy padding)
+// the lists are CSR (start offsets + a permutation), so clustered inputs cost no padding.
+// The grid ordering also stores, per particle, the anchor grid index and the
+// three 1-D Gaussian window tables of P values each, so that P2G and G2P never evaluate exp.
+#include "se_common.cuh"
+
+namespace {
+
+__device__ __forceinline__ double wrap1(double x, double L)
+{
+    double v = x - L * floor(x / L);
+    if (!(v >= 0.0 && v < L)) v = 0.0;      // also catches NaN/Inf: no out-of-range bins
+    return v;
+}
+
+__device__ __forceinline__ int near_cell1(double v, const SeGeom &g)
+{
+    int c = (int)floor(v / g.wcell);
+    return min(max(c, 0), g.ncell - 1);
+}
+
+// base grid index floor(x/h) and fractional offset in grid units
+__device__ __forceinline__ int grid_base1(double v, const SeGeom &g, double &frac)
+{
+    double q = v / g.h;
+    int i0 = (int)floor(q);
+    i0 = min(max(i0, 0), g.M - 1);
+    frac = q - (double)i0;
+    return i0;
+}
+
+template <typename Real>
+__global__ void k_bin(SeGeom g, const Real *__restrict__ x, int *__restrict__ cell_of,
+                      int *__restrict__ bin_of, int *__restrict__ cell_cnt, int *__restrict__ bin_cnt)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.N) return;
+    int c[3], b[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        double v = wrap1((double)x[3 * i + d], g.L);
+        c[d] = near_cell1(v, g);
+        double fr;
+        b[d] = grid_base1(v, g, fr) / SE_BIN;
+    }
+    int ci = (c[0] * g.ncell + c[1]) * g.ncell + c[2];
+    int bi = (b[0] * g.nbin + b[1]) * g.nbin + b[2];
+    cell_of[i] = ci;
+    bin_of[i] = bi;
+    atomicAdd(&cell_cnt[ci], 1);
+    atomicAdd(&bin_cnt[bi], 1);
+}
+
+// ---- exclusive scan of the two histograms: tile sums, then per-tile scan -----------------
+constexpr int SCAN_T = 256;            // threads
+constexpr int SCAN_E = 8;              // elements per thread
+constexpr int SCAN_TILE = SCAN_T * SCAN_E;
+
+__device__ __forceinline__ int block_sum(int v, int *sm)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    int t = 0;
+    for (int w = 0; w < SCAN_T / 32; ++w) t += sm[w];
+    __syncthreads();
+    return t;
+}
+
+// which = blockIdx.y (0: near cells, 1: grid bins)
+__global__ void __launch_bounds__(SCAN_T) k_tile_sums(const int *cntA, int nA, int *sumsA,
+                                                      const int *cntB, int nB, int *sumsB)
+{
+    __shared__ int sm[SCAN_T / 32];
+    const int *cnt = blockIdx.y ? cntB : cntA;
+    int n = blockIdx.y ? nB : nA;
+    int *sums = blockIdx.y ? sumsB : sumsA;
+    int base = blockIdx.x * SCAN_TILE;
+    if (base >= n) return;
+    int v = 0;
+#pragma unroll
+    for (int e = 0; e < SCAN_E; ++e) {
+        int i = base + e * SCAN_T + threadIdx.x;
+        if (i < n) v += cnt[i];
+    }
+    int t = block_sum(v, sm);
+    if (threadIdx.x == 0) sums[blockIdx.x] = t;
+}
+
+// cursor (in: counts) -> cursor = start (exclusive prefix), start[0..n] likewise
+__global__ void __launch_bounds__(SCAN_T) k_tile_scan(int *curA, int *startA, int nA, const int *sumsA,
+                                                      int *curB, int *startB, int nB, const int *sumsB)
+{
+    __shared__ int sm[SCAN_T / 32];
+    __shared__ int wsum[SCAN_T / 32];
+    int *cur = blockIdx.y ? curB : curA;
+    int *start = blockIdx.y ? startB : startA;
+    int n = blockIdx.y ? nB : nA;
+    const int *sums = blockIdx.y ? sumsB : sumsA;
+    int base = blockIdx.x * SCAN_TILE;
+    if (base >= n) return;
+    // offset of this tile = sum of the preceding tile sums
+    int pre = 0;
+    for (int b = threadIdx.x; b < (int)blockIdx.x; b += SCAN_T) pre += sums[b];
+    pre = block_sum(pre, sm);
+    // each thread owns SCAN_E consecutive elements
+    int i0 = base + threadIdx.x * SCAN_E;
+    int v[SCAN_E], tot = 0;
+#pragma unroll
+    for (int e = 0; e < SCAN_E; ++e) {
+        v[e] = (i0 + e < n) ? cur[i0 + e] : 0;
+        tot += v[e];
+    }
+    // inclusive warp scan of tot
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int inc = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += y;
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    int woff = 0;
+    for (int q = 0; q < w; ++q) woff += wsum[q];
+    int run = pre + woff + inc - tot;
+#pragma unroll
+    for (int e = 0; e < SCAN_E; ++e) {
+        if (i0 + e < n) { cur[i0 + e] = run; start[i0 + e] = run; }
+        run += v[e];
+        if (i0 + e == n - 1) start[n] = run;
+    }
+}
+
+__global__ void k_scatter(int64_t N, const int *__restrict__ cell_of, const int *__restrict__ bin_of,
+                          int *__restrict__ cell_cur, int *__restrict__ bin_cur,
+                          int *__restrict__ perm_near, int *__restrict__ inv_near,
+                          int *__restrict__ perm_grid, int *__restrict__ inv_grid)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int p = atomicAdd(&cell_cur[cell_of[i]], 1);
+    perm_near[p] = (int)i;
+    inv_near[i] = p;
+    int q = atomicAdd(&bin_cur[bin_of[i]], 1);
+    perm_grid[q] = (int)i;
+    inv_grid[i] = q;
+}
+
+// The slot a particle gets inside its cell depends on atomic arrival order.  Re-rank every
+// cell segment by user index so that the sorted order (hence every later floating-point
+// summation order) is a pure function of the input.  One thread per sorted slot, O(s) each.
+__global__ void k_rank_in_cell(int64_t N, const int *__restrict__ key_of, const int *__restrict__ start,
+                               const int *__restrict__ perm_in, int *__restrict__ perm_out,
+                               int *__restrict__ inv)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    int i = perm_in[p];
+    int c = key_of[i];
+    int s = start[c], e = start[c + 1];
+    int r = 0;
+    for (int q = s; q < e; ++q) r += (perm_in[q] < i);
+    perm_out[s + r] = i;
+    inv[i] = s + r;
+}
+
+template <typename Real>
+__global__ void k_gather_near(SeGeom g, const Real *__restrict__ x, const Real *__restrict__ f,
+                              const int *__restrict__ perm, const int *__restrict__ cell_of,
+                              Real *__restrict__ xs, Real *__restrict__ fs, int *__restrict__ cell_sorted)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= g.N) return;
+    int i = perm[p];
+    int ci = cell_of[i];
+    int c[3] = {ci / (g.ncell * g.ncell), (ci / g.ncell) % g.ncell, ci % g.ncell};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        double v = wrap1((double)x[3 * (int64_t)i + d], g.L);
+        if (g.rel_coords) v -= (double)c[d] * g.wcell;     // cell-relative (fp32 path), rounded once
+        xs[3 * p + d] = (Real)v;
+        fs[3 * p + d] = f[3 * (int64_t)i + d];
+    }
+    cell_sorted[p] = ci;
+}
+
+// one thread per (sorted particle, dim, l): window value exp(-beta (l - (P/2-1) - frac)^2)
+// = exp(-a t_l^2), t_l = (anchor + l) h - x  (reading S11).  Always evaluated in
+// double and rounded once to Real.
+template <typename Real>
+__global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *__restrict__ f,
+                              const int *__restrict__ perm, short4 *__restrict__ anchor,
+                              Real *__restrict__ wtab, Real *__restrict__ fs)
+{
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int P3 = 3 * g.P;
+    int64_t p = t / P3;
+    if (p >= g.N) return;
+    int e = (int)(t - p * P3);
+    int d = e / g.P, l = e - d * g.P;
+    int i = perm[p];
+    double frac;
+    int i0 = grid_base1(wrap1((double)x[3 * (int64_t)i + d], g.L), g, frac);
+    double u = (double)(l - (g.P / 2 - 1)) - frac;
+    wtab[t] = (Real)exp(-g.beta * u * u);
+    if (l == 0) {
+        int a = i0 - (g.P / 2 - 1);
+        if (a < 0) a += g.M;
+        short *ap = reinterpret_cast<short *>(&anchor[p]);
+        ap[d] = (short)a;
+        if (d == 0) ap[3] = 0;
+        fs[3 * p + d] = f[3 * (int64_t)i + d];
+    }
+}
+
+template <typename Real>
+__global__ void k_sum(int64_t N, const Real *__restrict__ uN, const Real *__restrict__ uF,
+                      const Real *__restrict__ f, const int *__restrict__ inv_near,
+                      const int *__restrict__ inv_grid, Real far_scale, Real cself, Real *__restrict__ u)
+{
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= 3 * N) return;
+    int64_t i = t / 3;
+    int c = (int)(t - 3 * i);
+    u[t] = uN[3 * (int64_t)inv_near[i] + c] + far_scale * uF[3 * (int64_t)inv_grid[i] + c] - cself * f[t];
+}
+
+template <typename Real>
+cudaError_t sort_impl(se_plan *p, const void *xv, const void *fv, cudaStream_t s)
+{
+    const SeGeom &g = p->g;
+    const Real *x = (const Real *)xv, *f = (const Real *)fv;
+    int nc3 = g.ncell * g.ncell * g.ncell, nb3 = g.nbin * g.nbin * g.nbin;
+    cudaMemsetAsync(p->cell_cursor, 0, sizeof(int) * (nc3 + 1), s);
+    cudaMemsetAsync(p->bin_cursor, 0, sizeof(int) * (nb3 + 1), s);
+    int T = 256;
+    unsigned nblk = (unsigned)((g.N + T - 1) / T);
+    k_bin<Real><<<nblk, T, 0, s>>>(g, x, p->cell_of, p->bin_of, p->cell_cursor, p->bin_cursor);
+    int tilesA = (nc3 + SCAN_TILE - 1) / SCAN_TILE, tilesB = (nb3 + SCAN_TILE - 1) / SCAN_TILE;
+    int tiles = tilesA > tilesB ? tilesA : tilesB;
+    // tile sums live behind the CSR arrays' scratch: reuse perm arrays (N >= 1) is unsafe for tiny N,
+    // so the plan allocates cell_start/bin_start with room for the tile sums after entry n.
+    int *sumsA = p->cell_start + (nc3 + 1), *sumsB = p->bin_start + (nb3 + 1);
+    k_tile_sums<<<dim3(tiles, 2), SCAN_T, 0, s>>>(p->cell_cursor, nc3, sumsA, p->bin_cursor, nb3, sumsB);
+    k_tile_scan<<<dim3(tiles, 2), SCAN_T, 0, s>>>(p->cell_cursor, p->cell_start, nc3, sumsA,
+                                                   p->bin_cursor, p->bin_start, nb3, sumsB);
+    // scatter into scratch permutations (cell_sorted / inv arrays double as scratch), then re-rank
+    int *tmp_near = p->cell_sorted, *tmp_grid = (int *)p->uF;     // both >= N ints, overwritten later
+    k_scatter<<<nblk, T, 0, s>>>(g.N, p->cell_of, p->bin_of, p->cell_cursor, p->bin_cursor,
+                                 tmp_near, p->inv_near, tmp_grid, p->inv_grid);
+    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, p->cell_of, p->cell_start, tmp_near, p->perm_near, p->inv_near);
+    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, p->bin_of, p->bin_start, tmp_grid, p->perm_grid, p->inv_grid);
+    k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, p->perm_near, p->cell_of, (Real *)p->xs_near,
+                                           (Real *)p->fs_near, p->cell_sorted);
+    int64_t nt = g.N * 3 * g.P;
+    k_gather_grid<Real><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(g, x, f, p->perm_grid, p->anchor,
+                                                                  (Real *)p->wtab, (Real *)p->fs_grid);
+    p->launches += 8;
+    return cudaGetLastError();
+}
+
+template <typename Real>
+cudaError_t sum_impl(se_plan *p, const void *f, void *u, cudaStream_t s)
+{
+    const SeGeom &g = p->g;
+    double far_scale = g.h * g.h * g.h * g.cw;                 // eq. (2.7) h^3 and the window's c_w
+    double cself = 4.0 * g.xi / sqrt(SE_PI);                   // self term, reading S3
+    int T = 256;
+    k_sum<Real><<<(unsigned)((3 * g.N + T - 1) / T), T, 0, s>>>(g.N, (const Real *)p->uN, (const Real *)p->uF,
+                                                               (const Real *)f, p->inv_near, p->inv_grid,
+                                                               (Real)far_scale, (Real)cself, (Real *)u);
+    p->launches += 1;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t se_launch_sort(se_plan *p, const void *x, const void *f, cudaStream_t s)
+{
+    return p->precision == SE_FP64 ? sort_impl<double>(p, x, f, s) : sort_impl<float>(p, x, f, s);
+}
+
+cudaError_t se_launch_sum(se_plan *p, const void *f, void *u, cudaStream_t s)
+{
+    return p->precision == SE_FP64 ? sum_impl<double>(p, f, u, s) : sum_impl<float>(p, f, u, s);
+}

@@ -1,0 +1,53 @@
+"""Helpers for the GPU parity tests (call the CUDA path through the C-ABI binding only)."""
+import numpy as np
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def run_stages(c, x, f):
+    """Run every stage through se_eval_stage and return the intermediates as numpy (user order)."""
+    import torch
+    import paper_2606_19059_b200 as se
+    dt = torch.float64 if c.precision == "fp64" else torch.float32
+    xd = torch.as_tensor(x, dtype=dt, device="cuda").contiguous()
+    fd = torch.as_tensor(f, dtype=dt, device="cuda").contiguous()
+    ud = torch.empty_like(xd)
+    out = {}
+    with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P, c.precision) as plan:
+        info = plan.info()
+        out["info"] = {k: getattr(info, k) for k, _ in info._fields_}
+        plan.stage("sort", x=xd, f=fd)
+        out["perm_near"] = plan.read(se.SE_BUF_PERM_NEAR).cpu().numpy()
+        out["perm_grid"] = plan.read(se.SE_BUF_PERM_GRID).cpu().numpy()
+        out["cell_start"] = plan.read(se.SE_BUF_CELL_START).cpu().numpy()
+        out["bin_start"] = plan.read(se.SE_BUF_BIN_START).cpu().numpy()
+        plan.stage("p2p")
+        uN = plan.read(se.SE_BUF_UN).cpu().numpy()
+        out["uN"] = np.empty_like(uN)
+        out["uN"][out["perm_near"]] = uN
+        plan.stage("p2g")
+        out["H"] = plan.read(se.SE_BUF_GRID).cpu().numpy()
+        plan.stage("fft")
+        plan.stage("scale")
+        sp = plan.read(se.SE_BUF_SPEC).cpu().numpy()
+        out["Hs"] = sp[..., 0] + 1j * sp[..., 1]
+        plan.stage("ifft")
+        out["Ht"] = plan.read(se.SE_BUF_GRID).cpu().numpy()
+        plan.stage("g2p")
+        uF = plan.read(se.SE_BUF_UF).cpu().numpy().astype(np.float64)
+        uF *= info.h ** 3 * info.cw
+        out["uF"] = np.empty_like(uF)
+        out["uF"][out["perm_grid"]] = uF
+        plan.stage("sum", f=fd, u=ud)
+        torch.cuda.synchronize()
+        out["u"] = ud.cpu().numpy()
+        # and the one-call path
+        u2 = plan.eval(xd, fd)
+        torch.cuda.synchronize()
+        out["u_eval"] = u2.cpu().numpy()
+        out["launches"] = plan.launch_count()
+    return out

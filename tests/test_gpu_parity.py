@@ -1,0 +1,235 @@
+"""GPU parity: CUDA path (through the C-ABI) vs the CPU oracle, stage by stage and end to end.
+
+Tolerances (relative L2 against the oracle's array of the same name):
+            fp64      fp32
+  u^N       1e-12     3e-6
+  H         1e-13     1e-6
+  H~hat,H~  1e-12     3e-6      (includes cuFFT vs pocketfft rounding)
+  u^F       1e-12     3e-6
+  u         1e-11     1e-5      (BASELINE.json north_star)
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_19059_b200 import workloads as W
+from gpu_util import rel, run_stages
+
+pytestmark = pytest.mark.gpu
+
+TOL = {
+    "fp64": dict(uN=1e-12, H=1e-13, Hs=1e-12, Ht=1e-12, uF=1e-12, u=1e-11),
+    "fp32": dict(uN=3e-6, H=1e-6, Hs=3e-6, Ht=3e-6, uF=3e-6, u=1e-5),
+}
+
+
+def check_all(c, x, f):
+    o = oracle.se_eval(x, f, c.L, c.xi, c.rc, c.M, c.P, keep=True)
+    g = run_stages(c, x, f)
+    tol = TOL[c.precision]
+    N = c.N
+    # K1: permutations are bijections, CSR offsets monotone and complete, particles in their cells
+    for key in ("perm_near", "perm_grid"):
+        assert np.array_equal(np.sort(g[key]), np.arange(N))
+    cs, bs = g["cell_start"], g["bin_start"]
+    assert cs[0] == 0 and cs[-1] == N and np.all(np.diff(cs) >= 0)
+    assert bs[0] == 0 and bs[-1] == N and np.all(np.diff(bs) >= 0)
+    nc = g["info"]["ncell"]
+    xw = o["xw"]
+    cid = np.minimum(np.floor(xw / (c.L / nc)).astype(np.int64), nc - 1)
+    lin = (cid[:, 0] * nc + cid[:, 1]) * nc + cid[:, 2]
+    pos_cell = np.searchsorted(cs, np.arange(N), side="right") - 1
+    assert np.array_equal(lin[g["perm_near"]], pos_cell)
+    nb = g["info"]["nbin"]
+    i0 = np.minimum(np.floor(xw / (c.L / c.M)).astype(np.int64), c.M - 1) // 8
+    linb = (i0[:, 0] * nb + i0[:, 1]) * nb + i0[:, 2]
+    pos_bin = np.searchsorted(bs, np.arange(N), side="right") - 1
+    assert np.array_equal(linb[g["perm_grid"]], pos_bin)
+    # deterministic order inside a cell: ascending user index
+    d = np.diff(g["perm_near"])
+    same = np.diff(pos_cell) == 0
+    assert np.all(d[same] > 0)
+    # stages
+    errs = dict(
+        uN=rel(g["uN"], o["uN"]),
+        H=rel(g["H"], o["H"]),
+        Hs=rel(g["Hs"], o["Hs"][..., : c.M // 2 + 1]),
+        Ht=rel(g["Ht"], o["Ht"]),
+        uF=rel(g["uF"], o["uF"]),
+        u=rel(g["u"], o["u"]),
+    )
+    print(c.label, {k: f"{v:.2e}" for k, v in errs.items()}, "launches", g["launches"])
+    for k, v in errs.items():
+        assert v <= tol[k], (k, v, tol[k])
+    assert rel(g["u_eval"], o["u"]) <= tol["u"]
+    assert g["launches"] > 0
+    return errs
+
+
+def test_cfg1_fp64_full():
+    c, x, f = W.make(1)
+    check_all(c, x, f)
+
+
+def test_cfg1_matches_direct_ewald():
+    """The GPU result itself meets BASELINE config 1's 1e-9 vs the exact sum."""
+    c, x, f = W.make(1)
+    g = run_stages(c, x, f)
+    ud = oracle.direct_ewald(x, f, c.L, c.xi)
+    assert rel(g["u_eval"], ud) < 1e-9
+
+
+@pytest.mark.parametrize("cfg,N", [(2, 6000), (3, 5000), (5, 7000)])
+def test_scaled_fp64(cfg, N):
+    """Configs 2/3/5 dimensionless parameters at a size that spans many tiles, cells and a ragged tail."""
+    c, x, f = W.scaled(cfg, N)
+    check_all(c, x, f)
+
+
+def test_scaled_fp32_cfg4():
+    c, x, f = W.scaled(4, 20000)
+    check_all(c, x, f)
+
+
+def test_cfg1_params_fp32():
+    c, x, f = W.make(1)
+    from dataclasses import replace
+    c = replace(c, precision="fp32")
+    x = x.astype(np.float32); f = f.astype(np.float32)
+    check_all(c, x, f)
+
+
+def test_cfg2_full_fp64():
+    c, x, f = W.make(2)
+    check_all(c, x, f)
+
+
+# ---- edge cases -------------------------------------------------------------------------------
+def test_single_particle_hasimoto():
+    from dataclasses import replace
+    c = replace(W.CONFIGS[1], N=1)
+    x = np.array([[0.3, 0.2, 0.9]]); f = np.array([[1.0, -2.0, 0.5]])
+    g = run_stages(c, x, f)
+    np.testing.assert_allclose(g["u_eval"], -(4 / 3) * 2.8372974795 * f, rtol=2e-9)
+
+
+def test_boundary_and_unwrapped_positions():
+    """x exactly 0, just below L, negative, > L, and many particles in one cell next to empty cells."""
+    from dataclasses import replace
+    rng = np.random.default_rng(77)
+    c = replace(W.CONFIGS[1], N=600)
+    x = rng.random((600, 3))
+    x[:50] = 0.5 + 0.01 * rng.random((50, 3))          # cluster in one cell
+    x[50] = [0.0, 0.0, 0.0]
+    x[51] = [np.nextafter(1.0, 0), 0.5, np.nextafter(1.0, 0)]
+    x[52] = [-0.25, 1.75, 3.5]
+    x[53] = [1.0, 1.0, 1.0]
+    x[54] = [-1e-17, 0.3, 0.6]
+    f = rng.standard_normal((600, 3))
+    check_all(c, x, f)
+
+
+def test_clustered_empty_cells():
+    from dataclasses import replace
+    rng = np.random.default_rng(78)
+    c, _, _ = W.scaled(5, 4000)
+    x = 0.3 + 0.05 * rng.standard_normal((4000, 3))
+    f = rng.standard_normal((4000, 3))
+    check_all(c, np.mod(x, 1.0), f)
+
+
+def test_minimum_cells_and_odd_grid_sizes():
+    """ncell = 3 (every cell is every other's colleague), M not a multiple of the tile (M=26, P=12)."""
+    from dataclasses import replace
+    rng = np.random.default_rng(79)
+    c = replace(W.CONFIGS[1], N=300, rc=0.33, xi=9.0, M=26, P=12)
+    x = rng.random((300, 3)); f = rng.standard_normal((300, 3))
+    check_all(c, x, f)
+    c = replace(W.CONFIGS[1], N=300, rc=0.3, xi=10.0, M=38, P=24)
+    check_all(c, x, f)
+    c = replace(W.CONFIGS[1], N=300, rc=0.3, xi=10.0, M=24, P=24)      # P == M
+    check_all(c, x, f)
+
+
+def test_coincident_particles_skipped():
+    from dataclasses import replace
+    rng = np.random.default_rng(80)
+    c = replace(W.CONFIGS[1], N=200)
+    x = rng.random((200, 3)); x[1] = x[0]; f = rng.standard_normal((200, 3))
+    check_all(c, x, f)
+
+
+def test_eval_is_repeatable_and_keeps_inputs():
+    import torch
+    import paper_2606_19059_b200 as se
+    c, x, f = W.scaled(2, 3000)
+    xd = torch.as_tensor(x, device="cuda"); fd = torch.as_tensor(f, device="cuda")
+    x0, f0 = xd.clone(), fd.clone()
+    with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P) as plan:
+        u1 = plan.eval(xd, fd).clone()
+        u2 = plan.eval(xd, fd).clone()
+        x2 = torch.as_tensor(np.mod(x + 0.37, 1.0), device="cuda")
+        u3 = plan.eval(x2, fd).clone()
+        u4 = plan.eval(xd, fd).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(xd, x0) and torch.equal(fd, f0)
+    assert torch.equal(u1, u2) and torch.equal(u1, u4)      # bit-reproducible
+    assert not torch.equal(u1, u3)
+
+
+def test_eval_host_matches_eval():
+    import torch
+    import paper_2606_19059_b200 as se
+    c, x, f = W.scaled(2, 3000)
+    xh = torch.as_tensor(x).pin_memory(); fh = torch.as_tensor(f).pin_memory()
+    uh = torch.empty_like(xh).pin_memory()
+    with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P) as plan:
+        u = plan.eval(xh.cuda(), fh.cuda())
+        plan.eval_host(xh, fh, uh)
+        torch.cuda.synchronize()
+        assert torch.equal(u.cpu(), uh)
+
+
+def test_standalone_scale_and_g2p_on_synthetic_buffers():
+    import torch
+    import paper_2606_19059_b200 as se
+    c, x, f = W.scaled(3, 2000)
+    M = c.M
+    spec = W.random_spectrum(5, M)
+    Y = W.smooth_grid(6, M)
+    xd = torch.as_tensor(x, device="cuda"); fd = torch.as_tensor(f, device="cuda")
+    with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P) as plan:
+        plan.stage("sort", x=xd, f=fd)
+        sp = torch.as_tensor(np.stack([spec.real, spec.imag], axis=-1).copy(), device="cuda")
+        plan.write(se.SE_BUF_SPEC, sp)
+        plan.stage("scale")
+        got = plan.read(se.SE_BUF_SPEC).cpu().numpy()
+        got = got[..., 0] + 1j * got[..., 1]
+        plan.write(se.SE_BUF_GRID, torch.as_tensor(Y, device="cuda"))
+        plan.stage("g2p")
+        info = plan.info()
+        uF = plan.read(se.SE_BUF_UF).cpu().numpy() * info.h ** 3 * info.cw
+        perm = plan.read(se.SE_BUF_PERM_GRID).cpu().numpy()
+    rng = np.random.default_rng(1)
+    idx = np.stack([rng.integers(0, M, 400), rng.integers(0, M, 400), rng.integers(0, M // 2 + 1, 400)], axis=1)
+    idx[:6] = [[0, 0, 0], [M // 2, 1, 1], [1, M // 2, 2], [3, 4, M // 2], [M - 1, M - 1, 1], [0, 0, 1]]
+    ref = oracle.scale_modes(idx, spec[:, idx[:, 0], idx[:, 1], idx[:, 2]].T.copy(), c.L, c.xi, M, c.P)
+    gv = got[:, idx[:, 0], idx[:, 1], idx[:, 2]].T
+    assert rel(gv, ref) < 1e-13
+    assert np.all(gv[:4] == 0)
+    u_user = np.empty_like(uF); u_user[perm] = uF
+    assert rel(u_user, oracle.g2p(oracle.wrap(x, c.L), Y, c.L, c.xi, M, c.P)) < 1e-13
+
+
+def test_plan_create_rejects_bad_arguments():
+    import paper_2606_19059_b200 as se
+    good = dict(N=100, L=1.0, xi=10.0, rc=0.2, M=32, P=12)
+    bad = [dict(N=0), dict(L=0.0), dict(xi=-1.0), dict(rc=0.0), dict(P=11), dict(P=34), dict(M=31),
+           dict(M=10, P=12), dict(rc=0.4), dict(L=float("nan"))]
+    for b in bad:
+        kw = {**good, **b}
+        with pytest.raises(se.SeError) as ei:
+            se.Plan(**kw)
+        assert ei.value.status == 1, b
+    with pytest.raises(KeyError):
+        se.Plan(**good, precision="fp16")
