@@ -23,10 +23,10 @@ TOL = {
 }
 
 
-def check_all(c, x, f):
+def check_all(c, x, f, tol_override=None):
     o = oracle.se_eval(x, f, c.L, c.xi, c.rc, c.M, c.P, keep=True)
     g = run_stages(c, x, f)
-    tol = TOL[c.precision]
+    tol = dict(TOL[c.precision], **(tol_override or {}))
     N = c.N
     # K1: permutations are bijections, CSR offsets monotone and complete, particles in their cells
     for key in ("perm_near", "perm_grid"):
@@ -147,8 +147,12 @@ def test_minimum_cells_and_odd_grid_sizes():
     check_all(c, x, f)
     c = replace(W.CONFIGS[1], N=300, rc=0.3, xi=10.0, M=38, P=24)
     check_all(c, x, f)
-    c = replace(W.CONFIGS[1], N=300, rc=0.3, xi=10.0, M=24, P=24)      # P == M
-    check_all(c, x, f)
+    # P == M: eta = (xi/m)^2 = 1.47 > 1, so the multiplier of eq. (2.6) GROWS like
+    # (1 + k^2/4xi^2) exp((eta-1) k^2/4xi^2) ~ 3e4 at the grid corner and amplifies the 1e-16
+    # rounding difference between cuFFT and pocketfft in Hhat; G2P's window damps those modes again,
+    # so u^F and u keep the standard tolerance while H~hat and H~ get 1e-9 here.
+    c = replace(W.CONFIGS[1], N=300, rc=0.3, xi=10.0, M=24, P=24)
+    check_all(c, x, f, tol_override=dict(Hs=1e-9, Ht=1e-9))
 
 
 def test_coincident_particles_skipped():
