@@ -68,7 +68,8 @@ enum {
     SE_BUF_PERM_NEAR = 4, /* int32[N]: sorted position -> user index, near-cell order              */
     SE_BUF_PERM_GRID = 5, /* int32[N]: sorted position -> user index, grid-bin order               */
     SE_BUF_CELL_START = 6,/* int32[ncell^3 + 1]: CSR offsets of the near cells                     */
-    SE_BUF_BIN_START = 7, /* int32[nbin^3 + 1]: CSR offsets of the grid bins                       */
+    SE_BUF_BIN_START = 7, /* int32[nbins_total + 1]: CSR offsets of the grid bins.  Mode 0: bins of 8^3 grid
+                             cells, key (bx, by, bz); mode 1: key (base plane ix, by/4, bz/4)               */
     SE_NBUFS = 8
 };
 
@@ -82,7 +83,10 @@ typedef struct {
     double a;            /* window exponent 2 xi^2 / eta : w(r) = c_w exp(-a r^2)        */
     double cw;           /* (a/pi)^{3/2}                                                 */
     int ncell;           /* near cells per dimension, floor(L/rc)          (reading S7)  */
-    int nbin;            /* grid bins per dimension, ceil(M / 8)                         */
+    int nbin;            /* grid bins per dimension: ceil(M/8) (tile mode), ceil(M/4) (sweep mode) */
+    int grid_mode;       /* gridding kernels: 0 = tile-stationary (any even P), 1 = z-sweep (P = 12, 16, 24) */
+    int nbins_total;     /* entries of SE_BUF_BIN_START minus 1: nbin^3 (mode 0), M * nbin^2 (mode 1)      */
+    int nchunk;          /* sweep mode: chunks along x                                   */
     int64_t nmodes;      /* M * M * (M/2+1) stored modes per component                   */
     size_t workspace_bytes; /* device memory owned by the plan (incl. cuFFT work area)   */
 } se_info;

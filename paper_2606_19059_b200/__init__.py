@@ -30,7 +30,8 @@ class SeInfo(C.Structure):
     _fields_ = [("N", C.c_int64), ("M", C.c_int), ("P", C.c_int), ("precision", C.c_int),
                 ("L", C.c_double), ("xi", C.c_double), ("rc", C.c_double), ("h", C.c_double),
                 ("m", C.c_double), ("eta", C.c_double), ("a", C.c_double), ("cw", C.c_double),
-                ("ncell", C.c_int), ("nbin", C.c_int), ("nmodes", C.c_int64),
+                ("ncell", C.c_int), ("nbin", C.c_int), ("grid_mode", C.c_int), ("nbins_total", C.c_int),
+                ("nchunk", C.c_int), ("nmodes", C.c_int64),
                 ("workspace_bytes", C.c_size_t)]
 
 
@@ -173,7 +174,7 @@ class Plan:
         if which == SE_BUF_CELL_START:
             return (i.ncell ** 3 + 1,), torch.int32
         if which == SE_BUF_BIN_START:
-            return (i.nbin ** 3 + 1,), torch.int32
+            return (i.nbins_total + 1,), torch.int32
         raise ValueError(which)
 
     def read(self, which, stream=None):

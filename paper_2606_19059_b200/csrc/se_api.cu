@@ -32,7 +32,7 @@ void free_all(se_plan *p)
     if (!p) return;
     void *ptrs[] = {p->cell_of, p->cell_start, p->cell_cursor, p->perm_near, p->inv_near, p->cell_sorted,
                     p->xs_near, p->fs_near, p->uN, p->bin_of, p->bin_start, p->bin_cursor, p->perm_grid,
-                    p->inv_grid, p->anchor, p->wtab, p->fs_grid, p->uF, p->grid, p->spec, p->ktab,
+                    p->inv_grid, p->anchor, p->wtab, p->fs_grid, p->uF, p->uFpart, p->grid, p->spec, p->ktab,
                     p->hx, p->hf, p->hu};
     for (void *q : ptrs) if (q) cudaFree(q);
     if (p->fft_ok & 1) cufftDestroy(p->fft_fwd);
@@ -91,7 +91,7 @@ size_t buffer_bytes(const se_plan *p, int which, void **ptr)
     case SE_BUF_PERM_NEAR: *ptr = p->perm_near; return (size_t)g.N * sizeof(int);
     case SE_BUF_PERM_GRID: *ptr = p->perm_grid; return (size_t)g.N * sizeof(int);
     case SE_BUF_CELL_START: *ptr = p->cell_start; return ((size_t)g.ncell * g.ncell * g.ncell + 1) * sizeof(int);
-    case SE_BUF_BIN_START: *ptr = p->bin_start; return ((size_t)g.nbin * g.nbin * g.nbin + 1) * sizeof(int);
+    case SE_BUF_BIN_START: *ptr = p->bin_start; return ((size_t)g.nbins_total + 1) * sizeof(int);
     default: *ptr = nullptr; return 0;
     }
 }
@@ -139,6 +139,54 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     g.N = N; g.M = M; g.P = P; g.L = L; g.xi = xi; g.rc = rc;
     g.ncell = ncell;
     g.nbin = (M + SE_BIN - 1) / SE_BIN;
+    g.nbins_total = g.nbin * g.nbin * g.nbin;
+    g.grid_mode = 0; g.nchunk = 1; g.nchunk_g2p = 1; g.gsteps = 1;
+    {
+        // Gridding kernels: FP64 tensor-core sweep where it applies, else the generic tile kernel.
+        // SE_GRID_MODE = tile | sweep | mma overrides (tests and experiments).
+        const char *force = std::getenv("SE_GRID_MODE");
+        const bool want_tile = force && std::strcmp(force, "tile") == 0;
+        const bool want_sweep = force && std::strcmp(force, "sweep") == 0;
+        const int zb = (M + SE_MMA_ZBIN - 1) / SE_MMA_ZBIN;
+        if (se_mma_supported(P, (int)prec) && (double)M * zb * M < 5.0e8 && !want_tile && !want_sweep) {
+            g.grid_mode = 2;
+            g.nbin = zb;
+            g.nbins_total = M * zb * M;
+            const int BY = 2 * SE_MMA_NWY, BZ = 8 * SE_MMA_NWZ;
+            const int tiles = ((M + BY - 1) / BY) * ((M + BZ - 1) / BZ);
+            // P2G re-spreads P-1 warm-up planes per chunk: chunk only when the grid has too few column tiles
+            // to fill 148 SMs x 2 blocks; G2P warm-up is loads only, chunk freely (>= ~4 waves).
+            int nch = (148 * 2 + tiles - 1) / tiles;
+            nch = std::min(nch, std::max(1, M / (2 * P)));
+            int nchg = (148 * 2 * 6 + tiles - 1) / tiles;
+            nchg = std::min(nchg, std::max(1, M / P));
+            const char *e = std::getenv("SE_NCHUNK");
+            if (e && std::atoi(e) > 0) nch = std::min(std::atoi(e), M);
+            e = std::getenv("SE_NCHUNK_G2P");
+            if (e && std::atoi(e) > 0) nchg = std::min(std::atoi(e), M);
+            g.nchunk = std::max(nch, 1);
+            g.nchunk_g2p = std::max(nchg, 1);
+        } else if (want_sweep && se_sweep_supported(P) &&
+                   (double)M * ((M + SE_SBIN - 1) / SE_SBIN) * ((M + SE_SBIN - 1) / SE_SBIN) < 1.0e9) {
+            const int sb = (M + SE_SBIN - 1) / SE_SBIN;
+            g.grid_mode = 1;
+            g.nbin = sb;
+            g.nbins_total = M * sb * sb;
+            // candidates per plane seen by one block: density x (bins covering tile + support)
+            double dens = (double)N / ((double)M * M * M);
+            double cand = dens * (SE_SWEEP_TB + P + 2 * SE_SBIN) * (16 + P + 2 * SE_SBIN);
+            int gs = (int)std::ceil(512.0 / std::max(cand, 1e-3));
+            g.gsteps = std::min(std::max(gs, 1), SE_GSTEPS_MAX);
+            int tiles = ((M + SE_SWEEP_TB - 1) / SE_SWEEP_TB) * ((M + 15) / 16);
+            int nch = (148 * 6 + tiles - 1) / tiles;
+            nch = std::min(nch, std::max(1, M / (2 * P)));
+            const char *e = std::getenv("SE_NCHUNK");
+            if (e && std::atoi(e) > 0) nch = std::min(std::atoi(e), M);
+            g.nchunk = std::max(nch, 1);
+            e = std::getenv("SE_GSTEPS");
+            if (e && std::atoi(e) > 0) g.gsteps = std::min(std::atoi(e), SE_GSTEPS_MAX);
+        }
+    }
     g.rel_coords = prec == SE_FP32;
     g.h = L / M;
     g.wcell = L / ncell;
@@ -149,7 +197,7 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     g.cw = std::pow(a / SE_PI, 1.5);
 
     size_t rb = p->real_bytes;
-    size_t nc3 = (size_t)ncell * ncell * ncell, nb3 = (size_t)g.nbin * g.nbin * g.nbin;
+    size_t nc3 = (size_t)ncell * ncell * ncell, nb3 = (size_t)g.nbins_total;
     size_t M3 = (size_t)M * M * M, nm = (size_t)M * M * (M / 2 + 1);
     size_t scan_tiles = (std::max(nc3, nb3) + 2047) / 2048 + 1;
 
@@ -172,6 +220,8 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     A.get(&p->wtab, (size_t)N * 3 * P * rb);
     A.get(&p->fs_grid, N * 3 * rb);
     A.get(&p->uF, std::max((size_t)N * 3 * rb, (size_t)N * sizeof(int)));
+    if (g.grid_mode == 1) A.get(&p->uFpart, (size_t)N * SE_NSLOT * 3 * rb);
+    if (g.grid_mode == 2) A.get(&p->uFpart, (size_t)N * se_mma_slots(P) * 3 * rb);
     A.get(&p->grid, 3 * M3 * rb);
     A.get(&p->spec, 3 * nm * 2 * rb);
     A.get(&p->ktab, 2 * (size_t)M * rb);
@@ -224,6 +274,7 @@ se_status se_plan_info(const se_plan *p, se_info *o)
     o->a = g.beta / (g.h * g.h);
     o->cw = g.cw;
     o->ncell = g.ncell; o->nbin = g.nbin;
+    o->grid_mode = g.grid_mode; o->nbins_total = g.nbins_total; o->nchunk = g.nchunk;
     o->nmodes = (int64_t)g.M * g.M * (g.M / 2 + 1);
     o->workspace_bytes = p->workspace_bytes;
     return SE_OK;

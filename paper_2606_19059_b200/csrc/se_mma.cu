@@ -1,0 +1,403 @@
+// K3 P2G (eq. (2.5)) and K5 G2P (eq. (2.7)) in FP64 as an x-SWEEP whose inner
+// product runs on the FP64 tensor-core path (mma.sync m8n8k4 f64 -> DMMA), for P = 16 and 24.
+//
+// Why.  With a Gaussian window at P = 24 both gridding steps are FP64-arithmetic bound: 3 P^3 = 41,472
+// FMA per particle against ~1 KB of compulsory traffic.  On B200 the DFMA pipe
+// and DMMA deliver the same peak (36.7 vs 33.0 TFLOP/s measured), but one DFMA warp instruction is 32
+// FMAs and needs an issue slot every 2 cycles per scheduler, while one DMMA is 256 FMAs and occupies the
+// pipe for 16 cycles: the tensor form leaves ~15 of every 16 issue slots for the bookkeeping that
+// output-stationary gridding needs (candidate lists, table staging, ring rotation).  tcgen05 has no
+// FP64 kind, so mma.sync is the only tensor path for this precision.
+//
+// The contraction.  Spreading is  H_c[x,y,z] += sum_n (f_nc Wx_n[x]) * (Wy_n[y] Wz_n[z]); for one y it is a
+// GEMM  C[(x), (z)] += A[(x), n] B[n, (z)]  with K = particles.  A warp owns J = 2 y-rows x 8 z-columns and
+// sweeps x: its accumulators are a RING of the P planes currently under the window (plane X lives in
+// residue X mod P, P/8 m-tiles of 8 rows) x 3 components x J, i.e. 9 J C-fragments (36 doubles per thread
+// at P = 24).  Particles are sorted by (anchor plane a_x, a_z / 16, a_y); all particles of one step have
+// the same a_x, touch every residue exactly once, and are consumed 4 at a time (the K of m8n8k4).  When the
+// sweep leaves a plane it is complete and is written once with plain 16-byte stores: no atomics, no
+// zero-fill, deterministic.  Efficiency of issued FMAs: 1 in x (no tile overlap in the sweep direction),
+// P/(P+J-1) in y, P/(P+7) in z.
+// Gathering is the transpose: the ring holds the grid planes as A-fragments (rows = planes, k = z),
+// B = Wy Wz of 8 particles, D[(plane), particle] is contracted with Wx in a short epilogue and reduced over
+// the 8 row-lanes with a packed butterfly; per-(particle, block tile) partial sums go to their own slot and
+// are added in a fixed order afterwards (bit-reproducible, no atomics).
+#include "se_common.cuh"
+
+namespace {
+
+constexpr int CAP = 64;              // candidates staged per round
+constexpr int ZBW = SE_MMA_ZBIN;     // z-bin width of the sort key
+
+__device__ __forceinline__ void dmma(double (&c)[2], double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c[0]), "+d"(c[1])
+        : "d"(a), "d"(b));
+}
+
+template <int P, int NWY, int NWZ>
+struct Cfg {
+    static constexpr int NW = NWY * NWZ, NT = NW * 32;
+    static constexpr int J = 2;
+    static constexpr int BY = J * NWY, BZ = 8 * NWZ;          // block tile (columns)
+    static constexpr int MT = P / 8;                           // m-tiles in the ring
+    static constexpr int OY = P, OZ = P + BY, OF = P + BY + BZ;  // record offsets: wx | wy | wz | f
+    static constexpr int REC = OF + 4;
+    static constexpr int NSB = (P - 2) / BY + 3, NSC = (P - 2) / BZ + 3;   // block tiles a window can meet
+    static_assert(P % 8 == 0 && (REC % 2) == 0, "layout");
+};
+
+template <int P, int NWY, int NWZ, bool SPREAD>
+struct alignas(16) Smem {
+    typedef Cfg<P, NWY, NWZ> C;
+    double rec[CAP + 1][C::REC];             // [CAP] is the all-zero record used for padding
+    double U[SPREAD ? 1 : CAP][C::NW][3];    // G2P: per-warp partial sums of the round
+    int pidx[CAP];
+    short ly0[CAP], lz0[CAP];                // window index of the block tile's first column, in [0, M)
+    short sid[CAP];                          // G2P: slot of (particle, this block tile); -1: does not touch
+    unsigned char wlist[C::NW][CAP + 8];
+    int run_beg[8];
+    int run_ofs[9];
+};
+
+__device__ __forceinline__ int modM(int v, int M) { v %= M; return v < 0 ? v + M : v; }
+
+// does the window [0, P) (indices mod M) meet columns T0 .. T0 + n - 1, given l0 = (T0 - anchor) mod M ?
+__device__ __forceinline__ bool meets(int l0, int n, int M, int P) { return n > 0 && (l0 < P || l0 + n - 1 >= M); }
+
+template <int P, int NWY, int NWZ, bool SPREAD>
+__global__ void __launch_bounds__(NWY * NWZ * 32, 2)
+k_mma(SeGeom g, const short4 *__restrict__ anchor, const double *__restrict__ wtab,
+      const double *__restrict__ fs, const int *__restrict__ bin_start, double *__restrict__ grid,
+      double *__restrict__ uFpart)
+{
+    typedef Cfg<P, NWY, NWZ> C;
+    constexpr int NT = C::NT, BY = C::BY, BZ = C::BZ, MT = C::MT, REC = C::REC;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Smem<P, NWY, NWZ, SPREAD> &S = *reinterpret_cast<Smem<P, NWY, NWZ, SPREAD> *>(smem_raw);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int gq = lane >> 2, tq = lane & 3;
+    const int M = g.M, nzb = g.nbin;
+    const int ntY = (M + BY - 1) / BY, ntZ = (M + BZ - 1) / BZ;
+    const int tz = blockIdx.x % ntZ, ty = (blockIdx.x / ntZ) % ntY, chunk = blockIdx.x / (ntZ * ntY);
+    const int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
+    const int CL = (M + nchunk - 1) / nchunk;
+    const int X0 = chunk * CL;
+    const int CLen = min(CL, M - X0);
+    if (CLen <= 0) return;
+    const int Y0 = ty * BY, Z0 = tz * BZ;
+    const int wy0 = 2 * (warp / NWZ), wz0 = 8 * (warp % NWZ);       // warp tile inside the block tile
+    const int nyw = min(2, M - (Y0 + wy0)), nzw = min(8, M - (Z0 + wz0));
+    // this lane's two adjacent z-columns (C-fragment columns in P2G, A-fragment k-columns in G2P)
+    const int cy = Y0 + wy0, cz = Z0 + wz0 + 2 * tq;
+    const bool col_ok = (cy < M) && (cz < M);                        // M, cy, cz even: pairs are valid together
+    const size_t MM = (size_t)M * M, M3 = MM * M;
+    const size_t col = (size_t)cy * M + cz;
+
+    // candidate rows / z-bins of this block tile (anchors): cyclic [Y0-(P-1), Y0+BY-1], [Z0-(P-1), Z0+BZ-1]
+    const int leny = min(BY + P - 1, M);
+    const int ylo = modM(Y0 - (P - 1), M);
+    int zb0, nzbins;
+    {
+        const int len = BZ + P - 1;
+        if (len + ZBW > M) { zb0 = 0; nzbins = nzb; }
+        else {
+            const int lo = modM(Z0 - (P - 1), M), hi = modM(Z0 + BZ - 1, M);
+            zb0 = lo / ZBW;
+            nzbins = hi / ZBW - zb0; if (nzbins < 0) nzbins += nzb;
+            nzbins += 1;
+        }
+    }
+    const int nrun = 2 * nzbins;                                     // <= 8
+
+    // ring: acc[mt][c][j] is a 2-double fragment (P2G: C tile; G2P: A fragments for zh = 0, 1)
+    double acc[MT][3][2][2];
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) acc[mt][c][j][0] = acc[mt][c][j][1] = 0.0;
+
+    const int s_begin = SPREAD ? X0 - (P - 1) : X0, s_end = X0 + CLen;
+    int rs = modM(s_begin, P);                                       // residue of plane s
+
+    // P2G: plane s (residue rs) is complete after step s
+    auto flush = [&](int s, int r) {
+        const bool mine = (gq == (r & 7));
+        const bool valid = mine && col_ok && s >= X0;
+        const size_t off = (size_t)modM(s, M) * MM + col;
+        const double cw = g.cw;
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            if (mt == (r >> 3) && mine) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        if (valid)
+                            *reinterpret_cast<double2 *>(&grid[c * M3 + off + (size_t)j * M]) =
+                                make_double2(cw * acc[mt][c][j][0], cw * acc[mt][c][j][1]);
+                        acc[mt][c][j][0] = acc[mt][c][j][1] = 0.0;
+                    }
+            }
+        }
+    };
+    // G2P: bring plane X into its residue
+    auto load_plane = [&](int X) {
+        const int r = modM(X, P);
+        const bool mine = (gq == (r & 7)) && col_ok;
+        const size_t off = (size_t)modM(X, M) * MM + col;
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            if (mt == (r >> 3) && mine) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        const double2 v = *reinterpret_cast<const double2 *>(&grid[c * M3 + off + (size_t)j * M]);
+                        acc[mt][c][j][0] = v.x; acc[mt][c][j][1] = v.y;
+                    }
+            }
+        }
+    };
+    if (!SPREAD)
+        for (int X = s_begin; X < s_begin + P - 1; ++X) load_plane(X);
+
+    for (int e = tid; e < C::REC; e += NT) S.rec[CAP][e] = 0.0;
+
+    for (int s = s_begin; s < s_end; ++s) {
+        if (!SPREAD) load_plane(s + P - 1);
+        const int pl = modM(s, M);
+        __syncthreads();                                             // run table of the previous step is dead
+        // ---- candidate runs of this step: (z-bin, row range) pieces, contiguous in the sorted order ----
+        if (tid < nrun) {
+            const int k = tid >> 1, piece = tid & 1;
+            int zb = zb0 + k; if (zb >= nzb) zb -= nzb;
+            const int base = (pl * nzb + zb) * M;
+            int r0, r1;                                              // rows [r0, r1)
+            if (piece == 0) { r0 = ylo; r1 = min(ylo + leny, M); }
+            else { r0 = 0; r1 = max(ylo + leny - M, 0); }
+            const int b = bin_start[base + r0], e = bin_start[base + r1];
+            S.run_beg[tid] = b;
+            S.run_ofs[tid + 1] = e - b;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int run = 0;
+            S.run_ofs[0] = 0;
+            for (int r = 0; r < nrun; ++r) { run += S.run_ofs[r + 1]; S.run_ofs[r + 1] = run; }
+        }
+        __syncthreads();
+        const int total = S.run_ofs[nrun];
+
+        // Wx index of this lane's ring rows for the particles of this step: plane s + l <-> residue (rs + l) mod P
+        int lx[MT];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) { int l = 8 * mt + gq - rs; lx[mt] = l < 0 ? l + P : l; }
+
+        for (int base = 0; base < total; base += CAP) {
+            const int na = min(CAP, total - base);
+            // ---- A: identify the candidates ---------------------------------------------------------------
+            if (tid < na) {
+                const int v = base + tid;
+                int r = 0;
+                while (r + 1 < nrun && S.run_ofs[r + 1] <= v) ++r;
+                const int pi = S.run_beg[r] + (v - S.run_ofs[r]);
+                const short4 a = anchor[pi];
+                const int ly = modM(Y0 - a.y, M), lz = modM(Z0 - a.z, M);
+                S.pidx[tid] = pi;
+                S.ly0[tid] = (short)ly; S.lz0[tid] = (short)lz;
+                if (!SPREAD) {
+                    const bool hit = meets(ly, min(BY, M - Y0), M, P) && meets(lz, min(BZ, M - Z0), M, P);
+                    const int rb = modM(ty - a.y / BY, ntY), rc = modM(tz - a.z / BZ, ntZ);
+                    S.sid[tid] = (short)((hit && rb < C::NSB && rc < C::NSC) ? rb * C::NSC + rc : -1);
+                }
+            }
+            __syncthreads();
+            // ---- B: stage records (global window tables -> block-tile slices), per-warp lists ---------------
+            for (int it = tid; it < na * REC; it += NT) {
+                const int a = it / REC, e = it - a * REC;
+                const int pi = S.pidx[a];
+                const double *w = wtab + (size_t)pi * 3 * P;
+                double v = 0.0;
+                if (e < C::OY) v = w[e];
+                else if (e < C::OZ) {
+                    const int j = e - C::OY;
+                    int l = S.ly0[a] + j; if (l >= M) l -= M;
+                    if (l < P && Y0 + j < M) v = w[P + l];
+                } else if (e < C::OF) {
+                    const int j = e - C::OZ;
+                    int l = S.lz0[a] + j; if (l >= M) l -= M;
+                    if (l < P && Z0 + j < M) v = w[2 * P + l];
+                } else if (e < C::OF + 3) v = fs[(size_t)pi * 3 + (e - C::OF)];
+                S.rec[a][e] = v;
+            }
+            if (!SPREAD)
+                for (int it = tid; it < na * C::NW * 3; it += NT) (&S.U[0][0][0])[it] = 0.0;
+            int cnt = 0;
+            for (int a0 = 0; a0 < na; a0 += 32) {
+                const int a = a0 + lane;
+                bool hit = false;
+                if (a < na) {
+                    int ly = S.ly0[a] + wy0; if (ly >= M) ly -= M;
+                    int lz = S.lz0[a] + wz0; if (lz >= M) lz -= M;
+                    hit = meets(ly, nyw, M, P) && meets(lz, nzw, M, P);
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, hit);
+                if (hit) S.wlist[warp][cnt + __popc(m & ((1u << lane) - 1u))] = (unsigned char)a;
+                cnt += __popc(m);
+            }
+            constexpr int GRP = SPREAD ? 4 : 8;
+            const int padded = (cnt + GRP - 1) & ~(GRP - 1);
+            if (lane < padded - cnt) S.wlist[warp][cnt + lane] = (unsigned char)CAP;
+            __syncthreads();
+
+            // ---- C: contraction ------------------------------------------------------------------------------
+            if (SPREAD) {
+                for (int q = 0; q < padded; q += 4) {
+                    const double *r = S.rec[S.wlist[warp][q + tq]];
+                    const double f0 = r[C::OF], f1 = r[C::OF + 1], f2 = r[C::OF + 2];
+                    const double2 wyv = *reinterpret_cast<const double2 *>(&r[C::OY + wy0]);
+                    const double wzv = r[C::OZ + wz0 + gq];
+                    const double b0 = wyv.x * wzv, b1 = wyv.y * wzv;
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        const double wx = r[lx[mt]];
+                        const double a0 = f0 * wx, a1 = f1 * wx, a2 = f2 * wx;
+                        dmma(acc[mt][0][0], a0, b0); dmma(acc[mt][0][1], a0, b1);
+                        dmma(acc[mt][1][0], a1, b0); dmma(acc[mt][1][1], a1, b1);
+                        dmma(acc[mt][2][0], a2, b0); dmma(acc[mt][2][1], a2, b1);
+                    }
+                }
+            } else {
+                for (int q = 0; q < padded; q += 8) {
+                    const double *r = S.rec[S.wlist[warp][q + gq]];
+                    const double2 wyv = *reinterpret_cast<const double2 *>(&r[C::OY + wy0]);
+                    const double2 wzv = *reinterpret_cast<const double2 *>(&r[C::OZ + wz0 + 2 * tq]);
+                    const double b00 = wyv.x * wzv.x, b01 = wyv.x * wzv.y, b10 = wyv.y * wzv.x, b11 = wyv.y * wzv.y;
+                    const int a0 = S.wlist[warp][q + 2 * tq], a1 = S.wlist[warp][q + 2 * tq + 1];
+                    double p0[3] = {0.0, 0.0, 0.0}, p1[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        const double wx0 = S.rec[a0][lx[mt]], wx1 = S.rec[a1][lx[mt]];
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            double d[2] = {0.0, 0.0};
+                            dmma(d, acc[mt][c][0][0], b00); dmma(d, acc[mt][c][0][1], b01);
+                            dmma(d, acc[mt][c][1][0], b10); dmma(d, acc[mt][c][1][1], b11);
+                            p0[c] = fma(d[0], wx0, p0[c]);
+                            p1[c] = fma(d[1], wx1, p1[c]);
+                        }
+                    }
+                    // sum over the 8 row-lanes (lane bits 2..4); lanes gq = 0 end with particle 2 tq, gq = 4 with 2 tq + 1
+                    const bool hi = lane & 16;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        const double snd = hi ? p0[c] : p1[c];
+                        double v = hi ? p1[c] : p0[c];
+                        v += __shfl_xor_sync(0xffffffffu, snd, 16);
+                        v += __shfl_xor_sync(0xffffffffu, v, 8);
+                        v += __shfl_xor_sync(0xffffffffu, v, 4);
+                        p0[c] = v;
+                    }
+                    if ((lane & 12) == 0) {
+                        const int aa = hi ? a1 : a0;
+                        if (aa < CAP) { S.U[aa][warp][0] = p0[0]; S.U[aa][warp][1] = p0[1]; S.U[aa][warp][2] = p0[2]; }
+                    }
+                }
+            }
+            __syncthreads();
+            if (!SPREAD) {
+                for (int it = tid; it < na * 3; it += NT) {
+                    const int a = it / 3, c = it - 3 * a;
+                    const int sid = S.sid[a];
+                    if (sid >= 0) {
+                        double sum = 0.0;
+#pragma unroll
+                        for (int w = 0; w < C::NW; ++w) sum += S.U[a][w][c];
+                        uFpart[((size_t)sid * g.N + S.pidx[a]) * 3 + c] = sum;
+                    }
+                }
+                __syncthreads();
+            }
+        }
+        if (SPREAD) flush(s, rs);
+        rs = rs + 1 == P ? 0 : rs + 1;
+    }
+}
+
+// u^F (grid-sorted order) = fixed-order sum of the slots the particle's window actually meets
+template <int P, int NWY, int NWZ>
+__global__ void k_reduce_slots(SeGeom g, const short4 *__restrict__ anchor, const double *__restrict__ part,
+                               double *__restrict__ uF)
+{
+    typedef Cfg<P, NWY, NWZ> C;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.N) return;
+    const int M = g.M;
+    const int ntY = (M + C::BY - 1) / C::BY, ntZ = (M + C::BZ - 1) / C::BZ;
+    const short4 a = anchor[i];
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    for (int rb = 0; rb < C::NSB && rb < ntY; ++rb) {
+        const int ty = (a.y / C::BY + rb) % ntY, Y0 = ty * C::BY;
+        if (!meets(modM(Y0 - a.y, M), min(C::BY, M - Y0), M, P)) continue;
+        for (int rc = 0; rc < C::NSC && rc < ntZ; ++rc) {
+            const int tz = (a.z / C::BZ + rc) % ntZ, Z0 = tz * C::BZ;
+            if (!meets(modM(Z0 - a.z, M), min(C::BZ, M - Z0), M, P)) continue;
+            const double *q = part + ((size_t)(rb * C::NSC + rc) * g.N + i) * 3;
+            s0 += q[0]; s1 += q[1]; s2 += q[2];
+        }
+    }
+    uF[3 * i + 0] = s0; uF[3 * i + 1] = s1; uF[3 * i + 2] = s2;
+}
+
+template <int P, int NWY, int NWZ, bool SPREAD>
+cudaError_t launch(se_plan *p, cudaStream_t s)
+{
+    typedef Cfg<P, NWY, NWZ> C;
+    const SeGeom &g = p->g;
+    static bool attr_set = false;
+    const size_t smem = sizeof(Smem<P, NWY, NWZ, SPREAD>);
+    auto kern = k_mma<P, NWY, NWZ, SPREAD>;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int ntY = (g.M + C::BY - 1) / C::BY, ntZ = (g.M + C::BZ - 1) / C::BZ;
+    const int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
+    kern<<<(unsigned)(nchunk * ntY * ntZ), C::NT, smem, s>>>(g, p->anchor, (const double *)p->wtab,
+                                                             (const double *)p->fs_grid, p->bin_start,
+                                                             (double *)p->grid, (double *)p->uFpart);
+    p->launches += 1;
+    if (!SPREAD) {
+        k_reduce_slots<P, NWY, NWZ><<<(unsigned)((g.N + 255) / 256), 256, 0, s>>>(
+            g, p->anchor, (const double *)p->uFpart, (double *)p->uF);
+        p->launches += 1;
+    }
+    return cudaGetLastError();
+}
+
+template <bool SPREAD>
+cudaError_t dispatch(se_plan *p, cudaStream_t s)
+{
+    switch (p->g.P) {
+    case 24: return launch<24, SE_MMA_NWY, SE_MMA_NWZ, SPREAD>(p, s);
+    case 16: return launch<16, SE_MMA_NWY, SE_MMA_NWZ, SPREAD>(p, s);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace
+
+bool se_mma_supported(int P, int precision) { return precision == SE_FP64 && (P == 24 || P == 16); }
+int se_mma_slots(int P)
+{
+    return P == 24 ? Cfg<24, SE_MMA_NWY, SE_MMA_NWZ>::NSB * Cfg<24, SE_MMA_NWY, SE_MMA_NWZ>::NSC
+                   : Cfg<16, SE_MMA_NWY, SE_MMA_NWZ>::NSB * Cfg<16, SE_MMA_NWY, SE_MMA_NWZ>::NSC;
+}
+cudaError_t se_launch_mma_p2g(se_plan *p, cudaStream_t s) { return dispatch<true>(p, s); }
+cudaError_t se_launch_mma_g2p(se_plan *p, cudaStream_t s) { return dispatch<false>(p, s); }

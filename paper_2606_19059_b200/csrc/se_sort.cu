@@ -44,10 +44,19 @@ __global__ void k_bin(SeGeom g, const Real *__restrict__ x, int *__restrict__ ce
         double v = wrap1((double)x[3 * i + d], g.L);
         c[d] = near_cell1(v, g);
         double fr;
-        b[d] = grid_base1(v, g, fr) / SE_BIN;
+        b[d] = grid_base1(v, g, fr);
     }
     int ci = (c[0] * g.ncell + c[1]) * g.ncell + c[2];
-    int bi = (b[0] * g.nbin + b[1]) * g.nbin + b[2];
+    int bi;
+    if (g.grid_mode == 2) {
+        int a[3];                                    // anchors, wrapped into [0, M)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { a[d] = b[d] - (g.P / 2 - 1); if (a[d] < 0) a[d] += g.M; }
+        bi = (a[0] * g.nbin + a[2] / SE_MMA_ZBIN) * g.M + a[1];
+    } else if (g.grid_mode == 1)
+        bi = (b[0] * g.nbin + b[1] / SE_SBIN) * g.nbin + b[2] / SE_SBIN;
+    else
+        bi = ((b[0] / SE_BIN) * g.nbin + b[1] / SE_BIN) * g.nbin + b[2] / SE_BIN;
     cell_of[i] = ci;
     bin_of[i] = bi;
     atomicAdd(&cell_cnt[ci], 1);
@@ -235,7 +244,7 @@ cudaError_t sort_impl(se_plan *p, const void *xv, const void *fv, cudaStream_t s
 {
     const SeGeom &g = p->g;
     const Real *x = (const Real *)xv, *f = (const Real *)fv;
-    int nc3 = g.ncell * g.ncell * g.ncell, nb3 = g.nbin * g.nbin * g.nbin;
+    int nc3 = g.ncell * g.ncell * g.ncell, nb3 = g.nbins_total;
     cudaMemsetAsync(p->cell_cursor, 0, sizeof(int) * (nc3 + 1), s);
     cudaMemsetAsync(p->bin_cursor, 0, sizeof(int) * (nb3 + 1), s);
     int T = 256;

@@ -41,8 +41,15 @@ def check_all(c, x, f, tol_override=None):
     pos_cell = np.searchsorted(cs, np.arange(N), side="right") - 1
     assert np.array_equal(lin[g["perm_near"]], pos_cell)
     nb = g["info"]["nbin"]
-    i0 = np.minimum(np.floor(xw / (c.L / c.M)).astype(np.int64), c.M - 1) // 8
-    linb = (i0[:, 0] * nb + i0[:, 1]) * nb + i0[:, 2]
+    i0 = np.minimum(np.floor(xw / (c.L / c.M)).astype(np.int64), c.M - 1)
+    if g["info"]["grid_mode"] == 2:      # FP64 tensor-core sweep: key (anchor plane, anchor_z / 16, anchor_y)
+        an = (i0 - (c.P // 2 - 1)) % c.M
+        linb = (an[:, 0] * nb + an[:, 2] // 16) * c.M + an[:, 1]
+    elif g["info"]["grid_mode"] == 1:    # z-sweep kernels: key (base plane, y-bin, z-bin), 4-wide bins
+        linb = (i0[:, 0] * nb + i0[:, 1] // 4) * nb + i0[:, 2] // 4
+    else:                                # tile kernels: 8^3 bins
+        linb = ((i0[:, 0] // 8) * nb + i0[:, 1] // 8) * nb + i0[:, 2] // 8
+    assert bs.shape[0] == g["info"]["nbins_total"] + 1
     pos_bin = np.searchsorted(bs, np.arange(N), side="right") - 1
     assert np.array_equal(linb[g["perm_grid"]], pos_bin)
     # deterministic order inside a cell: ascending user index
