@@ -154,11 +154,11 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
             g.nbins_total = M * zb * M;
             const int BY = 2 * SE_MMA_NWY, BZ = 8 * SE_MMA_NWZ;
             const int tiles = ((M + BY - 1) / BY) * ((M + BZ - 1) / BZ);
-            // P2G re-spreads P-1 warm-up planes per chunk: chunk only when the grid has too few column tiles
-            // to fill 148 SMs x 2 blocks; G2P warm-up is loads only, chunk freely (>= ~4 waves).
-            int nch = (148 * 2 + tiles - 1) / tiles;
-            nch = std::min(nch, std::max(1, M / (2 * P)));
-            int nchg = (148 * 2 * 6 + tiles - 1) / tiles;
+            // One block per SM.  P2G re-spreads P-1 warm-up planes per chunk: chunk only as far as needed for
+            // ~4 waves; G2P warm-up is loads only, chunk freely (~8 waves).
+            int nch = (148 * 4 + tiles - 1) / tiles;
+            nch = std::min(nch, std::max(1, M / (4 * P)));
+            int nchg = (148 * 8 + tiles - 1) / tiles;
             nchg = std::min(nchg, std::max(1, M / P));
             const char *e = std::getenv("SE_NCHUNK");
             if (e && std::atoi(e) > 0) nch = std::min(std::atoi(e), M);
