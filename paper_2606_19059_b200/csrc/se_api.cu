@@ -152,7 +152,7 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
             g.grid_mode = 2;
             g.nbin = zb;
             g.nbins_total = M * zb * M;
-            const int BY = 2 * SE_MMA_NWY, BZ = 8 * SE_MMA_NWZ;
+            const int BY = 4 * SE_MMA_NWY, BZ = 4 * SE_MMA_NWZ;
             const int tiles = ((M + BY - 1) / BY) * ((M + BZ - 1) / BZ);
             // One block per SM.  P2G re-spreads P-1 warm-up planes per chunk: chunk only as far as needed for
             // ~4 waves; G2P warm-up is loads only, chunk freely (~8 waves).
@@ -217,7 +217,7 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     A.get(&p->perm_grid, N * sizeof(int));
     A.get(&p->inv_grid, N * sizeof(int));
     A.get(&p->anchor, N * sizeof(short4));
-    A.get(&p->wtab, (size_t)N * 3 * P * rb);
+    A.get(&p->wtab, g.grid_mode == 2 ? (size_t)N * SE_MMA_REC(P) * rb : (size_t)N * 3 * P * rb);
     A.get(&p->fs_grid, N * 3 * rb);
     A.get(&p->uF, std::max((size_t)N * 3 * rb, (size_t)N * sizeof(int)));
     if (g.grid_mode == 1) A.get(&p->uFpart, (size_t)N * SE_NSLOT * 3 * rb);

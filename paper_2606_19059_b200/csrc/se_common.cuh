@@ -28,9 +28,11 @@ constexpr int SE_NSLOT_B = 5, SE_NSLOT_C = 3;        // G2P partial-sum slots pe
 constexpr int SE_NSLOT = SE_NSLOT_B * SE_NSLOT_C;
 constexpr int SE_GSTEPS_MAX = 16;
 // FP64 tensor-core gridding kernels (se_mma.cu): particles sorted by (anchor plane, anchor_z / ZBIN, anchor_y);
-// a block of NWY x NWZ consumer warps (+ 4 producer warps) owns 2 NWY x 8 NWZ (y, z) columns
-constexpr int SE_MMA_ZBIN = 16;
-constexpr int SE_MMA_NWY = 4, SE_MMA_NWZ = 3;
+// a block of NWY x NWZ consumer warps (+ 1 producer warp) owns 4 NWY x 4 NWZ (y, z) columns.  Every particle has a
+// record of SE_MMA_REC(P) doubles in sorted order: Wx[P] | Wy[P] | Wz[P] | f[3] | (a_y, a_z) as two int32.
+constexpr int SE_MMA_ZBIN = 8;
+constexpr int SE_MMA_NWY = 2, SE_MMA_NWZ = 6;
+#define SE_MMA_REC(P) (3 * (P) + 4)
 
 struct SeGeom {
     int64_t N;

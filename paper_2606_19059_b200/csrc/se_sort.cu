@@ -216,7 +216,10 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
     double frac;
     int i0 = grid_base1(wrap1((double)x[3 * (int64_t)i + d], g.L), g, frac);
     double u = (double)(l - (g.P / 2 - 1)) - frac;
-    wtab[t] = (Real)exp(-g.beta * u * u);
+    const Real w = (Real)exp(-g.beta * u * u);
+    const bool recs = g.grid_mode == 2;              // se_mma.cu: one record per particle (fp64 only)
+    const int64_t rbase = p * SE_MMA_REC(g.P);
+    if (recs) wtab[rbase + e] = w; else wtab[t] = w;
     if (l == 0) {
         int a = i0 - (g.P / 2 - 1);
         if (a < 0) a += g.M;
@@ -224,6 +227,10 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
         ap[d] = (short)a;
         if (d == 0) ap[3] = 0;
         fs[3 * p + d] = f[3 * (int64_t)i + d];
+        if (recs) {
+            wtab[rbase + P3 + d] = f[3 * (int64_t)i + d];
+            if (d > 0) reinterpret_cast<int *>(&wtab[rbase + P3 + 3])[d - 1] = a;
+        }
     }
 }
 
