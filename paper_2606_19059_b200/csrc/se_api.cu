@@ -32,7 +32,7 @@ void free_all(se_plan *p)
     if (!p) return;
     void *ptrs[] = {p->cell_of, p->cell_start, p->cell_cursor, p->perm_near, p->inv_near, p->cell_sorted,
                     p->xs_near, p->fs_near, p->uN, p->bin_of, p->bin_start, p->bin_cursor, p->perm_grid,
-                    p->inv_grid, p->anchor, p->wtab, p->fs_grid, p->uF, p->uFpart, p->grid, p->spec, p->ktab,
+                    p->inv_grid, p->anchor, p->wtab, p->recg, p->fs_grid, p->uF, p->uFpart, p->grid, p->spec, p->ktab,
                     p->hx, p->hf, p->hu};
     for (void *q : ptrs) if (q) cudaFree(q);
     if (p->fft_ok & 1) cufftDestroy(p->fft_fwd);
@@ -217,7 +217,8 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     A.get(&p->perm_grid, N * sizeof(int));
     A.get(&p->inv_grid, N * sizeof(int));
     A.get(&p->anchor, N * sizeof(short4));
-    A.get(&p->wtab, g.grid_mode == 2 ? (size_t)N * SE_MMA_REC(P) * rb : (size_t)N * 3 * P * rb);
+    A.get(&p->wtab, g.grid_mode == 2 ? (size_t)N * SE_MMA_RECS(P) * rb : (size_t)N * 3 * P * rb);
+    if (g.grid_mode == 2) A.get(&p->recg, (size_t)N * SE_MMA_RECG(P) * rb);
     A.get(&p->fs_grid, N * 3 * rb);
     A.get(&p->uF, std::max((size_t)N * 3 * rb, (size_t)N * sizeof(int)));
     if (g.grid_mode == 1) A.get(&p->uFpart, (size_t)N * SE_NSLOT * 3 * rb);

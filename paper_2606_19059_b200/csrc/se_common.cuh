@@ -28,11 +28,15 @@ constexpr int SE_NSLOT_B = 5, SE_NSLOT_C = 3;        // G2P partial-sum slots pe
 constexpr int SE_NSLOT = SE_NSLOT_B * SE_NSLOT_C;
 constexpr int SE_GSTEPS_MAX = 16;
 // FP64 tensor-core gridding kernels (se_mma.cu): particles sorted by (anchor plane, anchor_z / ZBIN, anchor_y);
-// a block of NWY x NWZ consumer warps (+ 1 producer warp) owns 4 NWY x 4 NWZ (y, z) columns.  Every particle has a
-// record of SE_MMA_REC(P) doubles in sorted order: Wx[P] | Wy[P] | Wz[P] | f[3] | (a_y, a_z) as two int32.
+// a block of NWY x NWZ consumer warps (+ the producer warpgroup) owns 4 NWY x 4 NWZ (y, z) columns.  K1 writes two
+// 16-byte aligned records per particle in sorted order (anchors as two int32 in one double slot):
+//   spread record, SE_MMA_RECS(P) doubles: c_w f_x Wx[P] | c_w f_y Wx[P] | c_w f_z Wx[P] | Wy[P] | Wz[P] | (a_y, a_z) | pad
+//   gather record, SE_MMA_RECG(P) doubles: Wx[P] | Wy[P] | Wz[P] | (a_y, a_z) | pad
+// (sizes = 24 mod 32 four-byte words, so that consecutive records start in different shared-memory bank octets)
 constexpr int SE_MMA_ZBIN = 8;
 constexpr int SE_MMA_NWY = 2, SE_MMA_NWZ = 6;
-#define SE_MMA_REC(P) (3 * (P) + 4)
+#define SE_MMA_RECS(P) (5 * (P) + 4)
+#define SE_MMA_RECG(P) (3 * (P) + 4)
 
 struct SeGeom {
     int64_t N;
@@ -78,7 +82,8 @@ struct se_plan {
     int *perm_grid;                // [N]
     int *inv_grid;                 // [N]
     short4 *anchor;                // [N] (a_x, a_y, a_z, 0): anchor grid index in [0, M)
-    void *wtab;                    // [N][3][P] Real: 1-D window values of every particle
+    void *wtab;                    // [N][3][P] Real: 1-D window values of every particle (mma mode: spread records)
+    void *recg;                    // mma mode: gather records
     void *fs_grid;                 // [N][3] Real
     void *uF;                      // [N][3] Real, grid-sorted order (unscaled sum)
     void *uFpart;                  // sweep mode: [N][SE_NSLOT][3] Real per-(particle, tile) partial sums

@@ -17,19 +17,23 @@
 // exactly once, and are consumed 4 at a time (the K of m8n8k4).  When the sweep leaves a plane it is
 // complete and is written once with plain 16-byte stores: no atomics, no zero-fill, deterministic.
 // Efficiency of issued FMAs: 1 in x (no tile overlap in the sweep direction), P/(P+3) in y and in z.
-// Gathering is the transpose: the ring holds the grid planes as A-fragments (rows = planes, k = 4 z),
-// B = Wy Wz of 8 particles, D[(plane), particle] is contracted with Wx in a short epilogue and reduced
-// over the 8 row-lanes with a packed butterfly; per-(particle, block tile) partial sums go to their own
-// slot and are added in a fixed order afterwards (bit-reproducible, no atomics).
+// Gathering is the transpose: the ring holds the grid planes as B-fragments (k = 4 planes, n = 8 columns),
+// A = Wx of 8 particles, E[particle, (yz)] accumulates over the P/4 k-steps and is contracted with Wy Wz
+// in a short epilogue (4 FMA per component, 2 shuffles over the 4 column-lanes); per-(particle, block tile)
+// partial sums go to their own slot and are added in a fixed order afterwards (bit-reproducible, no atomics).
 //
-// Staging.  K1 writes one 16-byte aligned RECORD per particle in sorted order:
-//   Wx[P] | Wy[P] | Wz[P] | f[3] | (a_y, a_z)          (3P + 4 doubles = 608 bytes at P = 24)
+// Staging.  K1 writes 16-byte aligned RECORDS per particle in sorted order (se_common.cuh):
+//   spread: c_w f_c Wx[P] (c = x, y, z) | Wy[P] | Wz[P] | (a_y, a_z)     (992 bytes at P = 24)
+//   gather: Wx[P] | Wy[P] | Wz[P] | (a_y, a_z)                            (608 bytes at P = 24)
+// so that every DMMA operand except the Wy Wz product comes out of shared memory ready-made: an FP64
+// multiply in front of a DMMA queues behind the DMMAs in flight on the shared FP64 datapath.
 // The candidates of a (block tile, step) are at most 14 contiguous runs of the sorted order, so ONE
 // producer warp stages them with one bulk asynchronous copy (cp.async.bulk, the TMA engine) per run,
-// completing on the stage's `full` mbarrier; 12 consumer warps test the raw records against their own
-// patch, read window values straight from the record (zero outside the support) and release the stage
-// through its `empty` mbarrier.  In G2P the producer also adds the consumers' per-warp partial sums in
-// fixed order and writes the slot before it refills a stage.
+// completing on the stage's `full` mbarrier; 12 consumer warps (152 registers each after setmaxnreg) test
+// the raw records against their own patch, copy the 4 + 4 window values under the patch into a per-warp
+// table (zero outside the support) and release the stage through its `empty` mbarrier.  In G2P the other
+// three warps of the producer warpgroup add the consumers' per-warp partial sums in fixed order and write
+// the slot before the stage is refilled.
 #include <climits>
 #include <type_traits>
 
@@ -38,7 +42,6 @@
 namespace {
 
 constexpr int CAP = 48;              // candidates per round (one step's candidates, split if more)
-constexpr int NST = 4;               // stages
 constexpr int ZBW = SE_MMA_ZBIN;     // z-bin width of the sort key
 constexpr int NWY = SE_MMA_NWY, NWZ = SE_MMA_NWZ;
 
@@ -85,33 +88,50 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
                  : "memory");
 }
 
-template <int P>
+template <int P, bool SPREAD>
 struct Cfg {
-    static constexpr int NCW = NWY * NWZ;                      // consumer warps
-    static constexpr int NT = (NCW + 1) * 32;                  // + one producer warp
+    static constexpr int NCW = NWY * NWZ;                      // consumer warps (3 warpgroups)
+    static constexpr int NT = (NCW + 4) * 32;                  // + the producer warpgroup
     static constexpr int BY = 4 * NWY, BZ = 4 * NWZ;           // block tile (columns)
     static constexpr int MT = P / 8;                           // m-tiles in the ring
-    static constexpr int REC = SE_MMA_REC(P);                  // doubles per record
-    static constexpr int OY = P, OZ = 2 * P, OF = 3 * P, OM = 3 * P + 3;
+    static constexpr int REC = SPREAD ? SE_MMA_RECS(P) : SE_MMA_RECG(P);   // doubles per record
+    static constexpr int OY = SPREAD ? 3 * P : P, OZ = OY + P, OM = OZ + P; // offsets of Wy, Wz, (a_y, a_z)
+    static constexpr int NST = SPREAD ? 3 : 4;                 // stages
+    static constexpr int GRP = SPREAD ? 4 : 8;                 // candidates per K-group (P2G: k = 4; G2P: n = 8)
+    static constexpr int TS = SPREAD ? 36 : 72;                // doubles per group in the patch-window table
     static constexpr int NSB = (P + BY - 2) / BY + 2, NSC = (P + BZ - 2) / BZ + 2;   // block tiles a window can meet
-    static_assert(P % 8 == 0 && (REC % 2) == 0, "layout");
+    static_assert(P % 8 == 0 && (REC % 2) == 0 && NCW % 4 == 0 && CAP % GRP == 0, "layout");
 };
+// registers per thread after the warpgroups re-split the register file (setmaxnreg): per scheduler
+// 3 consumer warps + 1 producer-group warp share 512 registers per lane
+constexpr int REGS_CONSUMER = 152, REGS_PRODUCER = 56;
 
 template <int P, bool SPREAD>
 struct alignas(16) Stage {
-    typedef Cfg<P> C;
+    typedef Cfg<P, SPREAD> C;
     double rec[CAP + 1][C::REC];             // [CAP] stays all-zero: the padding record
     double U[SPREAD ? 1 : CAP][C::NCW][3];   // G2P: per-warp partial sums of the round
-    int pidx[CAP];                           // sorted index of the candidate (G2P slot write-out)
-    int s, na;                               // step (anchor plane, unwrapped) and candidate count
+    int pidx[SPREAD ? 1 : CAP];              // G2P: sorted index of the candidate (slot write-out)
+    int s, na, rs, pad;                      // step (anchor plane, unwrapped), candidate count, s mod P
+};
+
+// Per-warp scratch of a round: the hit list and, per hit, the 4 + 4 window values under the warp's patch
+// (zero outside the support), laid out [group][value][hit in group] so that the group loop reads them with
+// fixed per-lane offsets and without bank conflicts (TS = 4 mod 16 / 8 mod 16 doubles keeps the stores of
+// consecutive hits in different banks too).
+template <int P, bool SPREAD>
+struct alignas(16) WarpScratch {
+    typedef Cfg<P, SPREAD> C;
+    double tb[CAP / C::GRP][C::TS];
+    unsigned char wl[CAP + 8];
 };
 
 template <int P, bool SPREAD>
 struct alignas(16) Smem {
-    typedef Cfg<P> C;
-    Stage<P, SPREAD> st[NST];
-    uint64_t full[NST], empty[NST];
-    unsigned char wlist[C::NCW][CAP + 8];
+    typedef Cfg<P, SPREAD> C;
+    Stage<P, SPREAD> st[C::NST];
+    WarpScratch<P, SPREAD> ws[C::NCW];
+    uint64_t full[C::NST], empty[C::NST], drained[C::NST];
 };
 
 __device__ __forceinline__ int modM(int v, int M) { v %= M; return v < 0 ? v + M : v; }
@@ -127,12 +147,12 @@ __device__ __forceinline__ double wval(const double *w, int l0, int i, int M, in
 }
 
 template <int P, bool SPREAD>
-__global__ void __launch_bounds__((NWY * NWZ + 1) * 32, 1)
+__global__ void __launch_bounds__((NWY * NWZ + 4) * 32, 1)
 k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_start, double *__restrict__ grid,
       double *__restrict__ uFpart)
 {
-    typedef Cfg<P> C;
-    constexpr int NCW = C::NCW, BY = C::BY, BZ = C::BZ, MT = C::MT, REC = C::REC;
+    typedef Cfg<P, SPREAD> C;
+    constexpr int NCW = C::NCW, BY = C::BY, BZ = C::BZ, MT = C::MT, REC = C::REC, NST = C::NST, GRP = C::GRP;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Smem<P, SPREAD> &S = *reinterpret_cast<Smem<P, SPREAD> *>(smem_raw);
 
@@ -150,10 +170,42 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
 
     for (int e = tid; e < NST * REC; e += C::NT) S.st[e / REC].rec[CAP][e % REC] = 0.0;
     if (tid == 0)
-        for (int i = 0; i < NST; ++i) { mbar_init(&S.full[i], 1); mbar_init(&S.empty[i], NCW); }
+        for (int i = 0; i < NST; ++i) {
+            mbar_init(&S.full[i], 1); mbar_init(&S.empty[i], NCW); mbar_init(&S.drained[i], 3);
+        }
     __syncthreads();
 
-    if (warp == NCW) {
+    if (warp >= NCW) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_PRODUCER));
+        if (warp > NCW) {
+            // ============================ G2P WRITE-OUT WARPS ===================================================
+            // add the consumers' partial sums of every round in fixed order, one slot per (particle, block tile)
+            if (SPREAD) return;
+            const int wl = (warp - NCW - 1) * 32 + lane;             // 0 .. 95
+            for (int r = 0;; ++r) {
+                const int sg = r % NST;
+                Stage<P, SPREAD> &T = S.st[sg];
+                mbar_wait(&S.full[sg], (r / NST) & 1);
+                if (T.s >= s_end) return;
+                mbar_wait(&S.empty[sg], (r / NST) & 1);
+                const int n3 = T.na * 3;
+                for (int it = wl; it < n3; it += 96) {
+                    const int a = it / 3, c = it - 3 * a;
+                    const int2 an = *reinterpret_cast<const int2 *>(&T.rec[a][C::OM]);
+                    const int ly = modM(Y0 - an.x, M), lz = modM(Z0 - an.y, M);
+                    const bool hit = meets(ly, min(BY, M - Y0), M, P) && meets(lz, min(BZ, M - Z0), M, P);
+                    const int rb = modM(ty - an.x / BY, ntY), rc = modM(tz - an.y / BZ, ntZ);
+                    if (hit && rb < C::NSB && rc < C::NSC) {
+                        double sum = 0.0;
+#pragma unroll
+                        for (int w = 0; w < NCW; ++w) sum += T.U[a][w][c];
+                        uFpart[((size_t)(rb * C::NSC + rc) * g.N + T.pidx[a]) * 3 + c] = sum;
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&S.drained[sg]);
+            }
+        }
         // =================================== PRODUCER ==========================================================
         // candidate rows / z-bins of this block tile (anchors): cyclic [Y0-(P-1), Y0+BY-1], [Z0-(P-1), Z0+BZ-1]
         const int leny = min(BY + P - 1, M);
@@ -175,298 +227,320 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
         const int nrun = 2 * nzbins;
         const int sl = lane >> 4, rl = lane & 15;
         int rcount = 0;                                              // rounds issued so far
-
-        // G2P: add the consumers' partial sums of the round that last used stage `sg`, one slot per block tile
-        auto writeout = [&](Stage<P, SPREAD> &T) {
-            if (SPREAD) return;
-            const int n3 = T.na * 3;
-            for (int it = lane; it < n3; it += 32) {
-                const int a = it / 3, c = it - 3 * a;
-                const int2 an = *reinterpret_cast<const int2 *>(&T.rec[a][C::OM]);
-                const int ly = modM(Y0 - an.x, M), lz = modM(Z0 - an.y, M);
-                const bool hit = meets(ly, min(BY, M - Y0), M, P) && meets(lz, min(BZ, M - Z0), M, P);
-                const int rb = modM(ty - an.x / BY, ntY), rc = modM(tz - an.y / BZ, ntZ);
-                if (hit && rb < C::NSB && rc < C::NSC) {
-                    double sum = 0.0;
-#pragma unroll
-                    for (int w = 0; w < NCW; ++w) sum += T.U[a][w][c];
-                    uFpart[((size_t)(rb * C::NSC + rc) * g.N + T.pidx[a]) * 3 + c] = sum;
-                }
+        // this lane's run of step s: [beg, beg + len) in the sorted order
+        int r0 = 0, r1 = 0, zoff = 0;
+        if (rl < nrun) {
+            const int k = rl >> 1, piece = rl & 1;
+            int zb = zb0 + k; if (zb >= nzb) zb -= nzb;
+            zoff = zb * M;
+            if (piece == 0) { r0 = ylo; r1 = min(ylo + leny, M); }
+            else { r0 = 0; r1 = max(ylo + leny - M, 0); }
+        }
+        auto run_of = [&](int s, int &beg, int &len) {
+            beg = 0; len = 0;
+            if (s < s_end && r1 > r0) {
+                const int base = modM(s, M) * nzb * M + zoff;
+                beg = __ldg(&bin_start[base + r0]);
+                len = __ldg(&bin_start[base + r1]) - beg;
             }
         };
-        // wait until the consumers have released stage sg (if it was used), flush its sums, make it ours again
+        // wait until stage r % NST has been released (P2G: by the consumers; G2P: by the write-out warps)
         auto acquire = [&](int r) {
-            const int sg = r & (NST - 1);
-            if (r >= NST) {
-                mbar_wait(&S.empty[sg], ((r / NST) - 1) & 1);
-                writeout(S.st[sg]);
-                __syncwarp();
-            }
+            const int sg = r % NST;
+            if (r >= NST) mbar_wait(SPREAD ? &S.empty[sg] : &S.drained[sg], ((r / NST) - 1) & 1);
         };
 
-        {
-            for (int sb = s_begin; sb < s_end; sb += 2) {
-                const int s = sb + sl;
-                int beg = 0, len = 0;
-                if (s < s_end && rl < nrun) {
-                    const int k = rl >> 1, piece = rl & 1;
-                    int zb = zb0 + k; if (zb >= nzb) zb -= nzb;
-                    const int base = (modM(s, M) * nzb + zb) * M;
-                    int r0, r1;                                      // rows [r0, r1)
-                    if (piece == 0) { r0 = ylo; r1 = min(ylo + leny, M); }
-                    else { r0 = 0; r1 = max(ylo + leny - M, 0); }
-                    beg = __ldg(&bin_start[base + r0]);
-                    len = __ldg(&bin_start[base + r1]) - beg;
-                }
-                // exclusive prefix of len over the 16 lanes of the step
-                int inc = len;
+        int nbeg, nlen;
+        run_of(s_begin + sl, nbeg, nlen);
+        for (int sb = s_begin; sb < s_end; sb += 2) {
+            const int beg = nbeg, len = nlen;
+            run_of(sb + 2 + sl, nbeg, nlen);                         // next iteration's offsets: latency overlaps this one
+            // exclusive prefix of len over the 16 lanes of the step
+            int inc = len;
 #pragma unroll
-                for (int o = 1; o < 16; o <<= 1) {
-                    const int y = __shfl_up_sync(0xffffffffu, inc, o, 16);
-                    if (rl >= o) inc += y;
-                }
-                const int ofs = inc - len;
-                for (int k = 0; k < 2 && sb + k < s_end; ++k) {
-                    const int total = __shfl_sync(0xffffffffu, inc, 16 * k + 15);
-                    for (int first = 0; first < total; first += CAP, ++rcount) {
-                        const int na = min(CAP, total - first);
-                        acquire(rcount);
-                        Stage<P, SPREAD> &T = S.st[rcount & (NST - 1)];
-                        uint64_t *bar = &S.full[rcount & (NST - 1)];
-                        if (lane == 0) {
-                            T.s = sb + k; T.na = na;
-                            mbar_arrive_expect_tx(bar, (unsigned)(na * REC * 8));
-                        }
-                        __syncwarp();
-                        if (sl == k) {
-                            const int lo = max(first, ofs), hi = min(first + na, ofs + len);
-                            if (lo < hi) {
-                                const int src = beg + (lo - ofs);
-                                bulk_g2s(T.rec[lo - first], recs + (size_t)src * REC, (unsigned)((hi - lo) * REC * 8), bar);
-                                if (!SPREAD)
-                                    for (int v = lo; v < hi; ++v) T.pidx[v - first] = src + (v - lo);
-                            }
+            for (int o = 1; o < 16; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, inc, o, 16);
+                if (rl >= o) inc += y;
+            }
+            const int ofs = inc - len;
+            for (int k = 0; k < 2 && sb + k < s_end; ++k) {
+                const int total = __shfl_sync(0xffffffffu, inc, 16 * k + 15);
+                for (int first = 0; first < total; first += CAP, ++rcount) {
+                    const int na = min(CAP, total - first);
+                    acquire(rcount);
+                    Stage<P, SPREAD> &T = S.st[rcount % NST];
+                    uint64_t *bar = &S.full[rcount % NST];
+                    if (lane == 0) {
+                        T.s = sb + k; T.na = na; T.rs = modM(sb + k, P);
+                        mbar_arrive_expect_tx(bar, (unsigned)(na * REC * 8));
+                    }
+                    __syncwarp();
+                    if (sl == k) {
+                        const int lo = max(first, ofs), hi = min(first + na, ofs + len);
+                        if (lo < hi) {
+                            const int src = beg + (lo - ofs);
+                            bulk_g2s(T.rec[lo - first], recs + (size_t)src * REC, (unsigned)((hi - lo) * REC * 8), bar);
+                            if (!SPREAD)
+                                for (int v = lo; v < hi; ++v) T.pidx[v - first] = src + (v - lo);
                         }
                     }
                 }
             }
         }
-        // terminal round: lets the consumers finish the sweep
-        {
-            acquire(rcount);
-            Stage<P, SPREAD> &T = S.st[rcount & (NST - 1)];
-            if (lane == 0) { T.s = s_end; T.na = 0; mbar_arrive(&S.full[rcount & (NST - 1)]); }
-            ++rcount;
+        // terminal round: lets the consumers (and the write-out warps) finish
+        acquire(rcount);
+        if (lane == 0) {
+            Stage<P, SPREAD> &T = S.st[rcount % NST];
+            T.s = s_end; T.na = 0; T.rs = 0;
+            mbar_arrive(&S.full[rcount % NST]);
         }
-        // G2P: slots of the rounds still in flight
-        if (!SPREAD)
-            for (int r = max(rcount - NST, 0); r < rcount; ++r) {
-                const int sg = r & (NST - 1);
-                mbar_wait(&S.empty[sg], (r / NST) & 1);
-                writeout(S.st[sg]);
-                __syncwarp();
-            }
         return;
     }
 
     // ======================================= CONSUMER ==============================================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_CONSUMER));
     const int gq = lane >> 2, tq = lane & 3;
     const int wy0 = 4 * (warp / NWZ), wz0 = 4 * (warp % NWZ);       // warp patch inside the block tile
     const int Yw = Y0 + wy0, Zw = Z0 + wz0;
     const int nyw = min(4, M - Yw), nzw = min(4, M - Zw);           // valid rows / columns of the patch
     const size_t MM = (size_t)M * M, M3 = MM * M;
+    WarpScratch<P, SPREAD> &WS = S.ws[warp];
+    // Both kernels see the patch as two n-tiles of 8 columns: column n of n-tile j is row 2j + (n >> 2),
+    // z-column n & 3 of the patch.
 
-    // ring: P2G  acc[mt][c][j]  = C fragment of n-tile j (rows 2j, 2j+1 of the patch; columns 2(tq&1), +1)
-    //       G2P  acc[mt][c][ky] = A fragments (row ky of the patch, column tq), two k-steps per double pair
-    double acc[MT][3][2][2];
-#pragma unroll
-    for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-            for (int j = 0; j < 2; ++j) acc[mt][c][j][0] = acc[mt][c][j][1] = 0.0;
-
-    // ---- P2G: this lane's C columns: n = 2 tq, 2 tq + 1 -> y = 2j + (tq >> 1), z = 2 (tq & 1) + {0, 1}
-    const int cyl = tq >> 1, czl = 2 * (tq & 1);
-    const bool cz_ok = czl < nzw;                                    // M, Zw even: the pair is valid together
-    const size_t colS = (size_t)(Yw + cyl) * M + (Zw + czl);
-    auto flush_mt = [&](auto mtc, int X, bool valid) {
-        constexpr int mt = decltype(mtc)::value;
-        const size_t off = (size_t)modM(X, M) * MM + colS;
-        const double cw = g.cw;
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                if (valid && 2 * j + cyl < nyw)
-                    *reinterpret_cast<double2 *>(&grid[c * M3 + off + (size_t)(2 * j) * M]) =
-                        make_double2(cw * acc[mt][c][j][0], cw * acc[mt][c][j][1]);
-                acc[mt][c][j][0] = acc[mt][c][j][1] = 0.0;
-            }
-    };
-    auto flush = [&](int X) {
-        const int r = modM(X, P);
-        if (gq != (r & 7)) return;
-        const bool valid = cz_ok && X >= X0;
-        switch (r >> 3) {
-        case 0: flush_mt(std::integral_constant<int, 0>{}, X, valid); break;
-        case 1: flush_mt(std::integral_constant<int, 1>{}, X, valid); break;
-        case 2: if constexpr (MT > 2) flush_mt(std::integral_constant<int, 2>{}, X, valid); break;
-        case 3: if constexpr (MT > 3) flush_mt(std::integral_constant<int, 3>{}, X, valid); break;
-        }
-    };
-    // ---- G2P: this lane's A elements: plane row gq, k = tq -> column z = tq of patch row ky
-    const bool gz_ok = tq < nzw;
-    const size_t colG = (size_t)Yw * M + (Zw + tq);
-    double pre[3][4];                                                // plane prefetched one step ahead
-    int pre_X = INT_MIN;
-    auto fetch_plane = [&](int X) {                                  // issue the loads of plane X into `pre`
-        pre_X = X;
-        if (gq != (modM(X, P) & 7)) return;
-        const size_t off = (size_t)modM(X, M) * MM + colG;
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-            for (int ky = 0; ky < 4; ++ky)
-                pre[c][ky] = (gz_ok && ky < nyw) ? __ldg(&grid[c * M3 + off + (size_t)ky * M]) : 0.0;
-    };
-    auto commit_mt = [&](auto mtc) {
-        constexpr int mt = decltype(mtc)::value;
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            acc[mt][c][0][0] = pre[c][0]; acc[mt][c][0][1] = pre[c][1];
-            acc[mt][c][1][0] = pre[c][2]; acc[mt][c][1][1] = pre[c][3];
-        }
-    };
-    auto commit_plane = [&]() {                                      // move `pre` into its residue of the ring
-        const int r = modM(pre_X, P);
-        if (gq != (r & 7)) return;
-        switch (r >> 3) {
-        case 0: commit_mt(std::integral_constant<int, 0>{}); break;
-        case 1: commit_mt(std::integral_constant<int, 1>{}); break;
-        case 2: if constexpr (MT > 2) commit_mt(std::integral_constant<int, 2>{}); break;
-        case 3: if constexpr (MT > 3) commit_mt(std::integral_constant<int, 3>{}); break;
-        }
+    // cur: P2G first plane not yet flushed; G2P first plane not yet in the ring.  curP = cur mod P, curM = cur mod M.
+    int cur = s_begin, curP = modM(s_begin, P), curM = modM(s_begin, M);
+    auto advance = [&]() {
+        ++cur;
+        if (++curP == P) curP = 0;
+        if (++curM == M) curM = 0;
     };
 
-    int cur = s_begin;            // P2G: first plane not yet flushed; G2P: first plane not yet in the ring
-    for (int r = 0;; ++r) {
-        const int sg = r & (NST - 1);
-        Stage<P, SPREAD> &T = S.st[sg];
-        mbar_wait(&S.full[sg], (r / NST) & 1);
-        const int s = T.s, na = T.na;
-        if (s >= s_end) {                                            // terminal round
-            if (SPREAD) while (cur < s_end) { flush(cur); ++cur; }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&S.empty[sg]);
-            break;
-        }
-        if (SPREAD) {
-            while (cur < s) { flush(cur); ++cur; }
-        } else {
-            // planes s .. s+P-1 must be in the ring; plane cur-1 may be waiting in `pre`
-            if (cur < s) { cur = s; pre_X = INT_MIN; }               // planes nobody gathers from are skipped
-            while (cur < s + P) {
-                if (pre_X != cur) fetch_plane(cur);
-                commit_plane();
-                ++cur;
-            }
-            if (pre_X != s + P) fetch_plane(s + P);                  // next step's new plane, consumed next round
-        }
-
-        // ---- this warp's candidates, padded to whole K-groups with the zero record -------------------------
+    // this warp's hits of a round: list + patch-window table, padded to whole K-groups with the zero record
+    auto build_hits = [&](Stage<P, SPREAD> &T, int na) -> int {
         int cnt = 0;
         for (int a0 = 0; a0 < na; a0 += 32) {
             const int a = a0 + lane;
             bool hit = false;
+            int ly = 0, lz = 0;
+            const double *rp = T.rec[min(a, CAP)];
             if (a < na) {
-                const int2 an = *reinterpret_cast<const int2 *>(&T.rec[a][C::OM]);
-                int ly = Yw - an.x; if (ly < 0) ly += M;
-                int lz = Zw - an.y; if (lz < 0) lz += M;
+                const int2 an = *reinterpret_cast<const int2 *>(&rp[C::OM]);
+                ly = Yw - an.x; if (ly < 0) ly += M;
+                lz = Zw - an.y; if (lz < 0) lz += M;
                 hit = meets(ly, nyw, M, P) && meets(lz, nzw, M, P);
                 if (!SPREAD && !hit) { T.U[a][warp][0] = 0.0; T.U[a][warp][1] = 0.0; T.U[a][warp][2] = 0.0; }
             }
             const unsigned m = __ballot_sync(0xffffffffu, hit);
-            if (hit) S.wlist[warp][cnt + __popc(m & ((1u << lane) - 1u))] = (unsigned char)a;
+            if (hit) {
+                const int h = cnt + __popc(m & ((1u << lane) - 1u));
+                WS.wl[h] = (unsigned char)a;
+                double *t = &WS.tb[h / GRP][h % GRP];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    t[i * GRP] = wval(rp + C::OY, ly, i, M, P);
+                    t[(4 + i) * GRP] = wval(rp + C::OZ, lz, i, M, P);
+                }
+            }
             cnt += __popc(m);
         }
-        constexpr int GRP = SPREAD ? 4 : 8;
         const int padded = (cnt + GRP - 1) & ~(GRP - 1);
-        if (lane < padded - cnt) S.wlist[warp][cnt + lane] = (unsigned char)CAP;
-        __syncwarp();
-
-        // Wx index of this lane's ring rows: plane s + l <-> residue (s + l) mod P
-        const int rs = modM(s, P);
-        int lx[MT];
+        if (lane < padded - cnt) {
+            const int h = cnt + lane;
+            WS.wl[h] = (unsigned char)CAP;
+            double *t = &WS.tb[h / GRP][h % GRP];
 #pragma unroll
-        for (int mt = 0; mt < MT; ++mt) { int l = 8 * mt + gq - rs; lx[mt] = l < 0 ? l + P : l; }
-
-        if (SPREAD) {
-            // B[k = tq][n = gq]: particle tq of the group, column n -> y = 2j + (gq >> 2), z = gq & 3
-            const int byl = gq >> 2, bzl = gq & 3;
-            for (int q = 0; q < padded; q += 4) {
-                const double *rp = T.rec[S.wlist[warp][q + tq]];
-                const double2 f01 = *reinterpret_cast<const double2 *>(&rp[C::OF]);
-                const double2 f2m = *reinterpret_cast<const double2 *>(&rp[C::OF + 2]);
-                const long long an = __double_as_longlong(f2m.y);                // (a_y, a_z)
-                int ly = Yw - (int)(an & 0xffffffffll); if (ly < 0) ly += M;
-                int lz = Zw - (int)(an >> 32); if (lz < 0) lz += M;
-                const double wzv = wval(rp + C::OZ, lz, bzl, M, P);
-                const double b0 = wval(rp + C::OY, ly, byl, M, P) * wzv;
-                const double b1 = wval(rp + C::OY, ly, byl + 2, M, P) * wzv;
-#pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    const double wx = rp[lx[mt]];
-                    const double a0 = f01.x * wx, a1 = f01.y * wx, a2 = f2m.x * wx;
-                    dmma(acc[mt][0][0], a0, b0); dmma(acc[mt][0][1], a0, b1);
-                    dmma(acc[mt][1][0], a1, b0); dmma(acc[mt][1][1], a1, b1);
-                    dmma(acc[mt][2][0], a2, b0); dmma(acc[mt][2][1], a2, b1);
-                }
-            }
-        } else {
-            // B[k = tq][n = gq]: column z = tq of patch row ky, particle gq of the group
-            for (int q = 0; q < padded; q += 8) {
-                const double *rp = T.rec[S.wlist[warp][q + gq]];
-                const int2 an = *reinterpret_cast<const int2 *>(&rp[C::OM]);
-                int ly = Yw - an.x; if (ly < 0) ly += M;
-                int lz = Zw - an.y; if (lz < 0) lz += M;
-                const double wzv = wval(rp + C::OZ, lz, tq, M, P);
-                double b[4];
-#pragma unroll
-                for (int ky = 0; ky < 4; ++ky) b[ky] = wval(rp + C::OY, ly, ky, M, P) * wzv;
-                const int a0 = S.wlist[warp][q + 2 * tq], a1 = S.wlist[warp][q + 2 * tq + 1];
-                double p0[3] = {0.0, 0.0, 0.0}, p1[3] = {0.0, 0.0, 0.0};
-#pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    const double wx0 = T.rec[a0][lx[mt]], wx1 = T.rec[a1][lx[mt]];
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        double d[2] = {0.0, 0.0};
-                        dmma(d, acc[mt][c][0][0], b[0]); dmma(d, acc[mt][c][0][1], b[1]);
-                        dmma(d, acc[mt][c][1][0], b[2]); dmma(d, acc[mt][c][1][1], b[3]);
-                        p0[c] = fma(d[0], wx0, p0[c]);
-                        p1[c] = fma(d[1], wx1, p1[c]);
-                    }
-                }
-                // sum over the 8 row-lanes (lane bits 2..4); lanes gq = 0 end with particle 2 tq, gq = 4 with 2 tq + 1
-                const bool hi = lane & 16;
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const double snd = hi ? p0[c] : p1[c];
-                    double v = hi ? p1[c] : p0[c];
-                    v += __shfl_xor_sync(0xffffffffu, snd, 16);
-                    v += __shfl_xor_sync(0xffffffffu, v, 8);
-                    v += __shfl_xor_sync(0xffffffffu, v, 4);
-                    p0[c] = v;
-                }
-                if ((lane & 12) == 0) {
-                    const int aa = hi ? a1 : a0;
-                    if (aa < CAP) { T.U[aa][warp][0] = p0[0]; T.U[aa][warp][1] = p0[1]; T.U[aa][warp][2] = p0[2]; }
-                }
-            }
+            for (int i = 0; i < 8; ++i) t[i * GRP] = 0.0;
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&S.empty[sg]);
+        return padded;
+    };
+
+    if constexpr (SPREAD) {
+        // ---------------------------------------- P2G ---------------------------------------------------------
+        // C[row = plane residue][n] += A[row][k = hit] B[k][n]:  A = c_w f_c Wx straight from the record,
+        // B = Wy Wz.  Ring acc[mt][c][j]: C fragment of m-tile mt, component c, n-tile j; this lane holds
+        // columns n = 2 tq, 2 tq + 1 -> patch row 2j + (tq >> 1), z-columns 2 (tq & 1), + 1.
+        double acc[MT][3][2][2];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int j = 0; j < 2; ++j) acc[mt][c][j][0] = acc[mt][c][j][1] = 0.0;
+        const int cyl = tq >> 1, czl = 2 * (tq & 1);
+        const bool cz_ok = czl < nzw;                                // M, Zw even: the pair is valid together
+        const size_t colS = (size_t)(Yw + cyl) * M + (Zw + czl);
+        auto flush_mt = [&](auto mtc, int XM, bool valid) {
+            constexpr int mt = decltype(mtc)::value;
+            const size_t off = (size_t)XM * MM + colS;
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    if (valid && 2 * j + cyl < nyw)
+                        *reinterpret_cast<double2 *>(&grid[c * M3 + off + (size_t)(2 * j) * M]) =
+                            make_double2(acc[mt][c][j][0], acc[mt][c][j][1]);
+                    acc[mt][c][j][0] = acc[mt][c][j][1] = 0.0;
+                }
+        };
+        auto flush = [&]() {                                         // plane cur is complete: write it, clear its residue
+            if (gq == (curP & 7)) {
+                const bool valid = cz_ok && cur >= X0;
+                switch (curP >> 3) {
+                case 0: flush_mt(std::integral_constant<int, 0>{}, curM, valid); break;
+                case 1: flush_mt(std::integral_constant<int, 1>{}, curM, valid); break;
+                case 2: if constexpr (MT > 2) flush_mt(std::integral_constant<int, 2>{}, curM, valid); break;
+                case 3: if constexpr (MT > 3) flush_mt(std::integral_constant<int, 3>{}, curM, valid); break;
+                }
+            }
+        };
+        for (int r = 0;; ++r) {
+            const int sg = r % NST;
+            Stage<P, SPREAD> &T = S.st[sg];
+            mbar_wait(&S.full[sg], (r / NST) & 1);
+            const int s = T.s, na = T.na, rs = T.rs;
+            if (s >= s_end) {                                        // terminal round
+                while (cur < s_end) { flush(); advance(); }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&S.empty[sg]);
+                break;
+            }
+            while (cur < s) { flush(); advance(); }
+            const int padded = build_hits(T, na);
+            // Wx index of this lane's ring rows: plane s + l <-> residue (s + l) mod P
+            int lx[MT];
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) { int l = 8 * mt + gq - rs; lx[mt] = l < 0 ? l + P : l; }
+            // B[k = tq][n = gq].  No FP64 arithmetic feeds a DMMA of the same group: the two B products of
+            // group q + 1 are formed while group q issues.
+            const double *tq0 = &WS.tb[0][(gq >> 2) * 4 + tq], *tqz = &WS.tb[0][(4 + (gq & 3)) * 4 + tq];
+            double b0 = 0.0, b1 = 0.0;
+            if (padded > 0) { const double wz = tqz[0]; b0 = tq0[0] * wz; b1 = tq0[8] * wz; }
+            for (int q = 0; q < padded; q += 4) {
+                const double *rp = T.rec[WS.wl[q + tq]];
+                double a[MT][3];
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) a[mt][c] = rp[c * P + lx[mt]];
+                const double c0 = b0, c1 = b1;
+                if (q + 4 < padded) {
+                    const int o = (q / 4 + 1) * C::TS;
+                    const double wz = tqz[o];
+                    b0 = tq0[o] * wz; b1 = tq0[o + 8] * wz;
+                }
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    dmma(acc[mt][0][0], a[mt][0], c0); dmma(acc[mt][0][1], a[mt][0], c1);
+                    dmma(acc[mt][1][0], a[mt][1], c0); dmma(acc[mt][1][1], a[mt][1], c1);
+                    dmma(acc[mt][2][0], a[mt][2], c0); dmma(acc[mt][2][1], a[mt][2], c1);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&S.empty[sg]);
+        }
+    } else {
+        // ---------------------------------------- G2P ---------------------------------------------------------
+        // E[hit][n] = sum_planes A[hit][k = plane] B[k][n]:  A = Wx of 8 hits straight from the record, B = the
+        // ring of grid planes, rg[ks][c][j] = plane residue 4 ks + tq, column n = gq of n-tile j, component c.
+        // All P/4 k-steps of a group accumulate in 6 independent chains (c, j); the epilogue multiplies by
+        // Wy Wz of the hit, sums this lane's two columns of both n-tiles and reduces over the 4 tq lanes.
+        constexpr int KS = P / 4;
+        double rg[KS][3][2];
+#pragma unroll
+        for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) rg[ks][c][0] = rg[ks][c][1] = 0.0;
+        const int gyl = gq >> 2, gzl = gq & 3;                       // this lane's column of an n-tile
+        const bool gz_ok = gzl < nzw;
+        const size_t colG = (size_t)(Yw + gyl) * M + (Zw + gzl);
+        double pre[3][2];                                            // plane prefetched one step ahead
+        int pre_X = INT_MIN, preP = 0;
+        auto fetch_plane = [&](int X, int XP, int XM) {              // issue the loads of plane X into `pre`
+            pre_X = X; preP = XP;
+            if (tq != (XP & 3)) return;
+            const size_t off = (size_t)XM * MM + colG;
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int j = 0; j < 2; ++j)
+                    pre[c][j] = (gz_ok && 2 * j + gyl < nyw) ? __ldg(&grid[c * M3 + off + (size_t)(2 * j) * M]) : 0.0;
+        };
+        auto commit_ks = [&](auto ksc) {
+            constexpr int ks = decltype(ksc)::value;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { rg[ks][c][0] = pre[c][0]; rg[ks][c][1] = pre[c][1]; }
+        };
+        auto commit_plane = [&]() {                                  // move `pre` into its residue of the ring
+            if (tq != (preP & 3)) return;
+            switch (preP >> 2) {
+            case 0: commit_ks(std::integral_constant<int, 0>{}); break;
+            case 1: commit_ks(std::integral_constant<int, 1>{}); break;
+            case 2: commit_ks(std::integral_constant<int, 2>{}); break;
+            case 3: commit_ks(std::integral_constant<int, 3>{}); break;
+            case 4: if constexpr (KS > 4) commit_ks(std::integral_constant<int, 4>{}); break;
+            case 5: if constexpr (KS > 5) commit_ks(std::integral_constant<int, 5>{}); break;
+            case 6: if constexpr (KS > 6) commit_ks(std::integral_constant<int, 6>{}); break;
+            case 7: if constexpr (KS > 7) commit_ks(std::integral_constant<int, 7>{}); break;
+            }
+        };
+        for (int r = 0;; ++r) {
+            const int sg = r % NST;
+            Stage<P, SPREAD> &T = S.st[sg];
+            mbar_wait(&S.full[sg], (r / NST) & 1);
+            const int s = T.s, na = T.na, rs = T.rs;
+            if (s >= s_end) {                                        // terminal round
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&S.empty[sg]);
+                break;
+            }
+            // planes s .. s+P-1 must be in the ring; plane cur may be waiting in `pre`
+            if (cur < s) { cur = s; curP = rs; curM = modM(s, M); pre_X = INT_MIN; }   // planes nobody gathers from
+            while (cur < s + P) {
+                if (pre_X != cur) fetch_plane(cur, curP, curM);
+                commit_plane();
+                advance();
+            }
+            if (pre_X != cur) fetch_plane(cur, curP, curM);          // plane s + P: consumed at the next step
+            const int padded = build_hits(T, na);
+            // Wx index of this lane's k-column: residue 4 ks + tq <-> plane s + l
+            int lx[KS];
+#pragma unroll
+            for (int ks = 0; ks < KS; ++ks) { int l = 4 * ks + tq - rs; lx[ks] = l < 0 ? l + P : l; }
+            // epilogue weights of hit gq at this lane's D columns n = 2 tq, 2 tq + 1 of n-tile j:
+            // row 2j + (tq >> 1), z-columns 2 (tq & 1), + 1
+            const double *ty = &WS.tb[0][(tq >> 1) * 8 + gq], *tz = &WS.tb[0][(4 + 2 * (tq & 1)) * 8 + gq];
+            for (int q = 0; q < padded; q += 8) {
+                const int o = (q / 8) * C::TS;
+                const int a = WS.wl[q + gq];
+                const double *rp = T.rec[a];
+                double wx[KS];
+#pragma unroll
+                for (int ks = 0; ks < KS; ++ks) wx[ks] = rp[lx[ks]];
+                const double wy0 = ty[o], wy1 = ty[o + 16], wz0 = tz[o], wz1 = tz[o + 8];
+                const double w00 = wy0 * wz0, w01 = wy0 * wz1, w10 = wy1 * wz0, w11 = wy1 * wz1;
+                double d[3][2][2];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) d[c][0][0] = d[c][0][1] = d[c][1][0] = d[c][1][1] = 0.0;
+#pragma unroll
+                for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) { dmma(d[c][0], wx[ks], rg[ks][c][0]); dmma(d[c][1], wx[ks], rg[ks][c][1]); }
+                double pc[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    double v = d[c][0][0] * w00;
+                    v = fma(d[c][0][1], w01, v); v = fma(d[c][1][0], w10, v); v = fma(d[c][1][1], w11, v);
+                    v += __shfl_xor_sync(0xffffffffu, v, 1);
+                    v += __shfl_xor_sync(0xffffffffu, v, 2);
+                    pc[c] = v;
+                }
+                if (tq == 0 && a < CAP) { T.U[a][warp][0] = pc[0]; T.U[a][warp][1] = pc[1]; T.U[a][warp][2] = pc[2]; }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&S.empty[sg]);
+        }
     }
 }
 
@@ -475,7 +549,7 @@ template <int P>
 __global__ void k_reduce_slots(SeGeom g, const short4 *__restrict__ anchor, const double *__restrict__ part,
                                double *__restrict__ uF)
 {
-    typedef Cfg<P> C;
+    typedef Cfg<P, false> C;
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.N) return;
     const int M = g.M;
@@ -498,10 +572,11 @@ __global__ void k_reduce_slots(SeGeom g, const short4 *__restrict__ anchor, cons
 template <int P, bool SPREAD>
 cudaError_t launch(se_plan *p, cudaStream_t s)
 {
-    typedef Cfg<P> C;
+    typedef Cfg<P, SPREAD> C;
     const SeGeom &g = p->g;
     static bool attr_set = false;
-    const size_t smem = sizeof(Smem<P, SPREAD>);
+    constexpr size_t smem = sizeof(Smem<P, SPREAD>);
+    static_assert(smem <= 227 * 1024, "shared memory per block");
     auto kern = k_mma<P, SPREAD>;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -510,7 +585,7 @@ cudaError_t launch(se_plan *p, cudaStream_t s)
     }
     const int ntY = (g.M + C::BY - 1) / C::BY, ntZ = (g.M + C::BZ - 1) / C::BZ;
     const int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
-    kern<<<(unsigned)(nchunk * ntY * ntZ), C::NT, smem, s>>>(g, (const double *)p->wtab, p->bin_start,
+    kern<<<(unsigned)(nchunk * ntY * ntZ), C::NT, smem, s>>>(g, (const double *)(SPREAD ? p->wtab : p->recg), p->bin_start,
                                                              (double *)p->grid, (double *)p->uFpart);
     p->launches += 1;
     if (!SPREAD) {
@@ -534,6 +609,6 @@ cudaError_t dispatch(se_plan *p, cudaStream_t s)
 }  // namespace
 
 bool se_mma_supported(int P, int precision) { return precision == SE_FP64 && (P == 24 || P == 16); }
-int se_mma_slots(int P) { return P == 24 ? Cfg<24>::NSB * Cfg<24>::NSC : Cfg<16>::NSB * Cfg<16>::NSC; }
+int se_mma_slots(int P) { return P == 24 ? Cfg<24, false>::NSB * Cfg<24, false>::NSC : Cfg<16, false>::NSB * Cfg<16, false>::NSC; }
 cudaError_t se_launch_mma_p2g(se_plan *p, cudaStream_t s) { return dispatch<true>(p, s); }
 cudaError_t se_launch_mma_g2p(se_plan *p, cudaStream_t s) { return dispatch<false>(p, s); }

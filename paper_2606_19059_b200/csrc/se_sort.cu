@@ -200,36 +200,45 @@ __global__ void k_gather_near(SeGeom g, const Real *__restrict__ x, const Real *
 
 // one thread per (sorted particle, dim, l): window value exp(-beta (l - (P/2-1) - frac)^2)
 // = exp(-a t_l^2), t_l = (anchor + l) h - x  (reading S11).  Always evaluated in
-// double and rounded once to Real.
+// double and rounded once to Real.  In mma mode (fp64) the values go into the per-particle spread and
+// gather records of se_mma.cu (layout in se_common.cuh) instead of the plain [N][3][P] table.
 template <typename Real>
 __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *__restrict__ f,
                               const int *__restrict__ perm, short4 *__restrict__ anchor,
-                              Real *__restrict__ wtab, Real *__restrict__ fs)
+                              Real *__restrict__ wtab, Real *__restrict__ recg, Real *__restrict__ fs)
 {
     int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    int P3 = 3 * g.P;
+    const int P = g.P, P3 = 3 * P;
     int64_t p = t / P3;
     if (p >= g.N) return;
     int e = (int)(t - p * P3);
-    int d = e / g.P, l = e - d * g.P;
+    int d = e / P, l = e - d * P;
     int i = perm[p];
     double frac;
     int i0 = grid_base1(wrap1((double)x[3 * (int64_t)i + d], g.L), g, frac);
-    double u = (double)(l - (g.P / 2 - 1)) - frac;
+    double u = (double)(l - (P / 2 - 1)) - frac;
     const Real w = (Real)exp(-g.beta * u * u);
-    const bool recs = g.grid_mode == 2;              // se_mma.cu: one record per particle (fp64 only)
-    const int64_t rbase = p * SE_MMA_REC(g.P);
-    if (recs) wtab[rbase + e] = w; else wtab[t] = w;
+    const bool recs = g.grid_mode == 2;
+    Real *rs = wtab + p * SE_MMA_RECS(P), *rg = recg + p * SE_MMA_RECG(P);
+    if (recs) {
+        rg[e] = w;
+        if (d == 0) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) rs[c * P + l] = (Real)g.cw * f[3 * (int64_t)i + c] * w;   // c_w of eq. (2.5) folded in
+        } else
+            rs[(d + 2) * P + l] = w;
+    } else
+        wtab[t] = w;
     if (l == 0) {
-        int a = i0 - (g.P / 2 - 1);
+        int a = i0 - (P / 2 - 1);
         if (a < 0) a += g.M;
         short *ap = reinterpret_cast<short *>(&anchor[p]);
         ap[d] = (short)a;
         if (d == 0) ap[3] = 0;
         fs[3 * p + d] = f[3 * (int64_t)i + d];
-        if (recs) {
-            wtab[rbase + P3 + d] = f[3 * (int64_t)i + d];
-            if (d > 0) reinterpret_cast<int *>(&wtab[rbase + P3 + 3])[d - 1] = a;
+        if (recs && d > 0) {
+            reinterpret_cast<int *>(&rs[5 * P])[d - 1] = a;
+            reinterpret_cast<int *>(&rg[P3])[d - 1] = a;
         }
     }
 }
@@ -275,7 +284,7 @@ cudaError_t sort_impl(se_plan *p, const void *xv, const void *fv, cudaStream_t s
                                            (Real *)p->fs_near, p->cell_sorted);
     int64_t nt = g.N * 3 * g.P;
     k_gather_grid<Real><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(g, x, f, p->perm_grid, p->anchor,
-                                                                  (Real *)p->wtab, (Real *)p->fs_grid);
+                                                                  (Real *)p->wtab, (Real *)p->recg, (Real *)p->fs_grid);
     p->launches += 8;
     return cudaGetLastError();
 }
