@@ -31,8 +31,8 @@ void free_all(se_plan *p)
 {
     if (!p) return;
     void *ptrs[] = {p->cell_of, p->cell_start, p->cell_cursor, p->perm_near, p->inv_near, p->cell_sorted,
-                    p->xs_near, p->fs_near, p->uN, p->bin_of, p->bin_start, p->bin_cursor, p->perm_grid,
-                    p->inv_grid, p->anchor, p->wtab, p->recg, p->fs_grid, p->uF, p->uFpart, p->grid, p->spec, p->ktab,
+                    p->src_near, p->xq, p->uN, p->bin_of, p->bin_start, p->bin_cursor, p->perm_grid,
+                    p->inv_grid, p->anchor, p->wtab, p->recg, p->fs_grid, p->uF, p->uFpart, p->grid, p->spec, p->ktab, p->mtab,
                     p->hx, p->hf, p->hu};
     for (void *q : ptrs) if (q) cudaFree(q);
     if (p->fft_ok & 1) cufftDestroy(p->fft_fwd);
@@ -208,8 +208,8 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     A.get(&p->perm_near, N * sizeof(int));
     A.get(&p->inv_near, N * sizeof(int));
     A.get(&p->cell_sorted, N * sizeof(int));
-    A.get(&p->xs_near, N * 3 * rb);
-    A.get(&p->fs_near, N * 3 * rb);
+    A.get(&p->src_near, N * 6 * rb);
+    A.get(&p->xq, N * sizeof(float4));
     A.get(&p->uN, N * 3 * rb);
     A.get(&p->bin_of, N * sizeof(int));
     A.get(&p->bin_start, (nb3 + 1 + scan_tiles) * sizeof(int));
@@ -249,6 +249,7 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     p->workspace_bytes += p->fft_work_bytes;
 
     if (se_build_ktab(p) != cudaSuccess) { cudaGetLastError(); free_all(p); return SE_ECUDA; }
+    if (se_build_mtab(p) != cudaSuccess) { cudaGetLastError(); free_all(p); return SE_ECUDA; }
     for (int i = 0; i <= SE_NSTAGES; ++i)
         if (cudaEventCreate(&p->ev[i]) != cudaSuccess) { free_all(p); return SE_ECUDA; }
     p->ev_ok = 1;

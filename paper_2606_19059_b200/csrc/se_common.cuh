@@ -71,9 +71,9 @@ struct se_plan {
     int *cell_cursor;              // [ncell^3 + 1] scatter cursors
     int *perm_near;                // [N] sorted pos -> user index
     int *inv_near;                 // [N] user index -> sorted pos
-    int *cell_sorted;              // [N] near cell of sorted particle
-    void *xs_near;                 // [N][3] Real  (absolute fp64 / cell-relative fp32)
-    void *fs_near;                 // [N][3] Real
+    int *cell_sorted;              // [N] packed cell coordinates (cx << 20 | cy << 10 | cz) of sorted particle
+    void *src_near;                // [N][6] Real: x, y, z (absolute fp64 / cell-relative fp32), f_x, f_y, f_z
+    void *xq;                      // [N] float4: cell-relative x, y, z and absolute z in FP32 (K2 candidate filter)
     void *uN;                      // [N][3] Real, near-sorted order
     // grid path (K1b, K3, K5)
     int *bin_of;                   // [N]
@@ -91,6 +91,7 @@ struct se_plan {
     void *grid;                    // [3][M][M][M] Real
     void *spec;                    // [3][M][M][M/2+1] complex Real
     void *ktab;                    // [2][M] Real : k value, exp factor per 1-D index
+    double *mtab;                  // K2 function tables (se_p2p.cu): erfcx pieces + exp polynomial, always double
     cufftHandle fft_fwd, fft_inv;
     int fft_ok;
     size_t fft_work_bytes;
@@ -109,6 +110,7 @@ cudaError_t se_launch_scale(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_g2p(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_sum(se_plan *p, const void *f, void *u, cudaStream_t s);
 cudaError_t se_build_ktab(se_plan *p);
+cudaError_t se_build_mtab(se_plan *p);      // allocates and fills p->mtab
 cudaError_t se_launch_sweep_p2g(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_sweep_g2p(se_plan *p, cudaStream_t s);
 bool se_sweep_supported(int P);

@@ -1,44 +1,96 @@
 // K2: near-field P2P,  u^N_i = sum_j sum_p [0 < |r| <= rc] G^N(r) f_j,  r = x_i - x_j + p
 // (eq. (2.2), eq. (2.3)), over the 27 colleague cells.
 //
-// Design (differs from the paper's thread-per-target kernels): only ~15% of
-// the candidates in the 27 cells are inside the cutoff sphere, so a thread-per-target loop
-// runs the expensive erfc/exp code at ~15% lane utilisation.  Here ONE WARP owns a target:
-//   phase A (cheap): lanes stride over the candidate sources, compute r and r^2, and
-//            compact the in-range ones (ballot + popc) into a per-warp shared-memory queue;
-//   phase B (heavy): whenever 32 pairs are queued, every lane evaluates one pair with all
-//            lanes busy; G^N is evaluated in registers as
+// Design.  Only ~15% of the candidates in the 27 colleague cells are inside the cutoff sphere, so the paper's
+// thread-per-target loop runs the expensive erfc/exp code at ~15% lane utilisation, and on
+// B200 the FP64 pipe (64 lanes per SM) is the scarce resource.  Here a LANE owns a target (32 consecutive
+// targets of the near-sorted order per warp) and the work is split by pipe:
+//   phase A (filter; FP32 pipe, one broadcast 16-byte load per source): the warp walks the sources of the
+//            colleague cells; every lane forms r^2 to its own target in FP32 from the compact copy `xq` K1
+//            wrote (coordinates relative to the particle's cell, so periodic images cost nothing) and, if
+//            r^2 <= rc^2 (1 + margin), appends the source index to ITS OWN ring queue in shared memory
+//            (one predicated store; no ballot, no compaction, ~11 instructions per 32 pair tests).  The
+//            margin bounds the FP32 rounding, so no in-range pair is lost; the few extra ones are rejected
+//            exactly in phase B;
+//   phase B (heavy; FP64 pipe, FP32 for fp32 plans): in a round every lane pops one pair of its own queue:
+//            exact r from the full-precision coordinates in the form of eq. (2.2), x_i - (x_j + p), the exact
+//            test 0 < r^2 <= rc^2 (reading S6), and G^N evaluated in registers as
 //              C1 = A - B,  C2 = (A + B)/r^2,  A = e^{-xi^2 r^2} erfcx(xi r)/r,  B = 2 xi e^{-xi^2 r^2}/sqrt(pi)
-//            (erfc(x) = e^{-x^2} erfcx(x): one exponential serves both terms of (2.3));
-//   per target one butterfly reduction of the three accumulators.
-// The z-row of three colleague cells is contiguous in the sorted order and is scanned as one
-// run.  fp64 uses absolute positions + the image shift exactly as eq. (2.2); fp32 uses
-// cell-relative positions so that r keeps full float precision across periodic images.
+//            (erfc(x) = e^{-x^2} erfcx(x): one exponential serves both terms of (2.3)).  Rounds run only when
+//            the fullest queue of the warp needs room, so that all lanes stay busy; the lane adds into its own
+//            three accumulators (no reduction) and writes u^N_i itself.
+// A warp whose targets span several cells processes them in passes: the targets of one z-row of cells whose
+// cell index is within P2P_ZSPAN of the first; a lane only accepts sources of its own 27 colleague cells.
+// A queue entry is 16 bits: (virtual cell << 9) | offset, a virtual cell being <= 512 consecutive sources of one
+// colleague cell; a per-warp table maps it to the first source index and to the periodic image p of that cell.  fp32 plans use cell-relative positions in phase B too, so that r keeps full
+// float precision across images.
+#include <cmath>
+
 #include "se_common.cuh"
 
 namespace {
 
 constexpr int P2P_WARPS = 4;
-constexpr int P2P_TPW = 8;          // targets per warp
-constexpr int P2P_Q = 64;           // queue slots per warp (circular)
+constexpr int P2P_QC = 128;         // ring-queue slots per lane (power of two), 16-bit entries
+constexpr int P2P_CHUNK = 32;       // sources scanned between two queue-room checks
+constexpr int P2P_VBITS = 9;        // a queue entry = (virtual cell << VBITS) | offset: virtual cells of <= 512 sources
+constexpr int P2P_NV = 128;         // virtual-cell table entries per warp ((NV << VBITS) = 2^16)
+constexpr int P2P_ZSPAN = 6;        // cells along z a pass may span (<= 29: one lane per source cell)
+
+// ---- function tables (built on the host in long double at plan creation, copied to shared memory per block) ----
+// erfcx(x) = e^{x^2} erfc(x) on [0, 8): 32 pieces of width 1/4, each a degree-10 polynomial in the local
+// variable u = 8 x - (2 i + 1) in [-1, 1] (interpolation at Chebyshev nodes, converted to monomials; measured
+// relative error < 4e-16).  Row stride 11 doubles = 22 words: 16 consecutive rows start in 16 different bank
+// pairs, so lanes in different pieces read their coefficients without bank conflicts.  For x >= 8 the argument
+// is clamped; e^{-x^2} < 2e-28 there.
+// e^t on [-ln2/2, ln2/2]: degree-11 polynomial (Chebyshev interpolant, relative error < 1e-17).
+constexpr int MT_NP = 32, MT_DEG = 10, MT_ROW = MT_DEG + 1;
+constexpr int MT_EXP = MT_NP * MT_ROW, MT_EXPDEG = 11;
+constexpr int MT_SIZE = MT_EXP + MT_EXPDEG + 1;
 
 template <typename Real> struct NearMath;
 
 template <> struct NearMath<double> {
-    static __device__ __forceinline__ void coeffs(double r2, double xi, double c2, double &C1, double &C2)
+    // e^{-y}, y >= 0
+    static __device__ __forceinline__ double exp_neg(double y, const double *mt)
     {
-        double rinv = rsqrt(r2);
-        double x2 = xi * xi * r2;
-        double e = exp(-x2);
-        double A = e * erfcx(xi * (r2 * rinv)) * rinv;
-        double B = c2 * e;
+        y = fmin(y, 700.0);
+        const double SH = 6755399441055744.0;                    // 1.5 * 2^52: round-to-nearest integer shifter
+        const double t = fma(y, -1.4426950408889634074, SH);
+        const int n = __double2loint(t);                         // n = rint(-y log2 e) <= 0
+        const double nf = t - SH;
+        double r = fma(nf, -6.93147180369123816490e-01, -y);     // r = -y - n ln2 (ln2 split hi + lo)
+        r = fma(nf, -1.90821492927058770002e-10, r);
+        const double *c = mt + MT_EXP;
+        double p = c[MT_EXPDEG];
+#pragma unroll
+        for (int k = MT_EXPDEG - 1; k >= 0; --k) p = fma(p, r, c[k]);
+        return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
+    }
+    static __device__ __forceinline__ double erfcx_tab(double x, const double *mt)
+    {
+        const double xm = fmin(x, 7.99999999);
+        const int i = (int)(4.0 * xm);
+        const double u = fma(8.0, xm, -(double)(2 * i + 1));
+        const double *c = mt + i * MT_ROW;
+        double p = c[MT_DEG];
+#pragma unroll
+        for (int k = MT_DEG - 1; k >= 0; --k) p = fma(p, u, c[k]);
+        return p;
+    }
+    static __device__ __forceinline__ void coeffs(double r2, double xi, double c2, const double *mt, double &C1, double &C2)
+    {
+        const double rinv = rsqrt(r2);
+        const double e = exp_neg(xi * xi * r2, mt);
+        const double A = e * erfcx_tab(xi * (r2 * rinv), mt) * rinv;
+        const double B = c2 * e;
         C1 = A - B;
         C2 = (A + B) * (rinv * rinv);
     }
 };
 
 template <> struct NearMath<float> {
-    static __device__ __forceinline__ void coeffs(float r2, float xi, float c2, float &C1, float &C2)
+    static __device__ __forceinline__ void coeffs(float r2, float xi, float c2, const double *, float &C1, float &C2)
     {
         float rinv = rsqrtf(r2);
         float x2 = xi * xi * r2;
@@ -51,135 +103,253 @@ template <> struct NearMath<float> {
 };
 
 template <typename Real>
-__global__ void __launch_bounds__(P2P_WARPS * 32)
-k_p2p(SeGeom g, const Real *__restrict__ xs, const Real *__restrict__ fs,
-      const int *__restrict__ cell_sorted, const int *__restrict__ cell_start, Real *__restrict__ uN)
+__global__ void __launch_bounds__(P2P_WARPS * 32, 4)
+k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, const int *__restrict__ cellp,
+      const int *__restrict__ cell_start, const double *__restrict__ mtab, Real *__restrict__ uN, float rc2m)
 {
-    __shared__ Real qx[P2P_WARPS][P2P_Q], qy[P2P_WARPS][P2P_Q], qz[P2P_WARPS][P2P_Q];
-    __shared__ int qj[P2P_WARPS][P2P_Q];
+    __shared__ double mt[MT_SIZE];
+    for (int e = threadIdx.x; e < MT_SIZE; e += P2P_WARPS * 32) mt[e] = mtab[e];
+    __syncthreads();
+    __shared__ unsigned short qsm[P2P_WARPS][P2P_QC][32];
+    __shared__ int vtab[P2P_WARPS][P2P_NV];                      // virtual cell -> sorted index of its first source
+    __shared__ int vcode[P2P_WARPS][P2P_NV];                     // virtual cell -> packed offsets / image shifts (below)
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const unsigned lt_mask = (1u << lane) - 1u;
     const int nc = g.ncell;
     const Real rc2 = (Real)(g.rc * g.rc);
     const Real xi = (Real)g.xi;
     const Real c2 = (Real)(2.0 * g.xi / sqrt(SE_PI));
     const Real Lr = (Real)g.L, wc = (Real)g.wcell;
-    const bool rel = g.rel_coords != 0;
+    const float wf = (float)g.wcell;
+    constexpr float FAR = 1.0e18f;                               // coordinate of a lane that must not match
+    char *const Qb = reinterpret_cast<char *>(&qsm[w][0][lane]); // this lane's queue column, slot stride 64 B
+    constexpr int QSTRIDE = 64, QBYTES = P2P_QC * QSTRIDE;
+    int *const VT = vtab[w], *const VC = vcode[w];
+    int nv = 0, nv_drained = 0;                                  // virtual cells opened / opened at the last full drain
 
-    const int64_t first = ((int64_t)blockIdx.x * P2P_WARPS + w) * P2P_TPW;
+    const int64_t i = ((int64_t)blockIdx.x * P2P_WARPS + w) * 32 + lane;
+    const bool valid = i < g.N;
+    const int64_t ic = valid ? i : g.N - 1;
+    const float4 qi = xq[ic];
+    const int pci = cellp[ic];
+    const int cx = pci >> 20, cy = (pci >> 10) & 1023, cz = pci & 1023;
+    const Real X0 = src[6 * ic + 0], X1 = src[6 * ic + 1], X2 = src[6 * ic + 2];
+    Real a0 = 0, a1 = 0, a2 = 0;
+    int woff = 0, roff = 0;                                      // ring write / read offsets (bytes); empty when equal
 
-    for (int t = 0; t < P2P_TPW; ++t) {
-        const int64_t i = first + t;
-        if (i >= g.N) break;                                     // warp-uniform
-        const Real xi0 = xs[3 * i + 0], xi1 = xs[3 * i + 1], xi2 = xs[3 * i + 2];
-        const int ci = cell_sorted[i];
-        const int cz = ci % nc, cy = (ci / nc) % nc, cx = ci / (nc * nc);
-        Real a0 = 0, a1 = 0, a2 = 0;
-        int head = 0, qn = 0;
-
-        auto heavy = [&](int nvalid) {
-            __syncwarp();
-            if (lane < nvalid) {
-                int k = (head + lane) & (P2P_Q - 1);
-                Real rx = qx[w][k], ry = qy[w][k], rz = qz[w][k];
-                int j = qj[w][k];
-                Real f0 = fs[3 * (int64_t)j + 0], f1 = fs[3 * (int64_t)j + 1], f2 = fs[3 * (int64_t)j + 2];
-                Real r2 = rx * rx + ry * ry + rz * rz;
-                Real C1, C2;
-                NearMath<Real>::coeffs(r2, xi, c2, C1, C2);
-                Real rf = C2 * (rx * f0 + ry * f1 + rz * f2);
-                a0 += C1 * f0 + rf * rx;
-                a1 += C1 * f1 + rf * ry;
-                a2 += C1 * f2 + rf * rz;
+    auto queued = [&]() { return ((woff - roff) & (QBYTES - 1)) / QSTRIDE; };
+    // One round of phase B.  Mode A (balanced): every lane with a queued pair pops and evaluates one of its own.
+    // Mode B (imbalanced: fewer non-empty queues than the fullest one could feed): the 32 lanes evaluate up to 32
+    // pairs of the fullest queue together and a butterfly sum hands the result to its owner.  The choice is a pure
+    // function of the queue lengths, so the summation order stays deterministic.
+    auto round = [&]() {
+        const int c = queued();
+        const unsigned m1 = __ballot_sync(0xffffffffu, c > 0);
+        const int cmax = __reduce_max_sync(0xffffffffu, c);
+        const int cB = min(cmax, 32);
+        const bool modeB = cB > __popc(m1);                      // warp-uniform
+        Real T0 = X0, T1 = X1, T2 = X2;
+        int tp = pci, ro = roff, o = lane;
+        bool have = c > 0;
+        if (modeB) {
+            o = __ffs(__ballot_sync(0xffffffffu, c == cmax)) - 1;
+            T0 = __shfl_sync(0xffffffffu, X0, o); T1 = __shfl_sync(0xffffffffu, X1, o); T2 = __shfl_sync(0xffffffffu, X2, o);
+            tp = __shfl_sync(0xffffffffu, pci, o);
+            ro = (__shfl_sync(0xffffffffu, roff, o) + lane * QSTRIDE) & (QBYTES - 1);
+            have = lane < cB;
+        }
+        Real d0 = 0, d1 = 0, d2 = 0;
+        if (have) {
+            const int e = *reinterpret_cast<const unsigned short *>(Qb + (o - lane) * 2 + ro);
+            const int j = VT[e >> P2P_VBITS] + (e & ((1 << P2P_VBITS) - 1));
+            const Real *sp = src + 6 * (int64_t)j;
+            Real xj, yj, zj, f0, f1, f2;
+            if (sizeof(Real) == 8) {
+                const double2 p0 = __ldg(reinterpret_cast<const double2 *>(sp));
+                const double2 p1 = __ldg(reinterpret_cast<const double2 *>(sp + 2));
+                const double2 p2 = __ldg(reinterpret_cast<const double2 *>(sp + 4));
+                xj = (Real)p0.x; yj = (Real)p0.y; zj = (Real)p1.x; f0 = (Real)p1.y; f1 = (Real)p2.x; f2 = (Real)p2.y;
+            } else {
+                const float2 p0 = __ldg(reinterpret_cast<const float2 *>(sp));
+                const float2 p1 = __ldg(reinterpret_cast<const float2 *>(sp + 2));
+                const float2 p2 = __ldg(reinterpret_cast<const float2 *>(sp + 4));
+                xj = (Real)p0.x; yj = (Real)p0.y; zj = (Real)p1.x; f0 = (Real)p1.y; f1 = (Real)p2.x; f2 = (Real)p2.y;
             }
-            __syncwarp();
-        };
+            // periodic image of the source as this target sees it, from the virtual cell's packed code
+            const int code = VC[e >> P2P_VBITS];
+            Real sx, sy, sz;
+            if (g.rel_coords) {
+                sx = (Real)((code & 3) - 1) * wc; sy = (Real)(((code >> 2) & 3) - 1) * wc;
+                sz = (Real)((code >> 10) - 1 - (tp & 1023)) * wc;
+            } else {
+                sx = (Real)(((code >> 4) & 3) - 1) * Lr; sy = (Real)(((code >> 6) & 3) - 1) * Lr;
+                sz = (Real)(((code >> 8) & 3) - 1) * Lr;
+            }
+            const Real rx = T0 - (xj + sx), ry = T1 - (yj + sy), rz = T2 - (zj + sz);
+            Real r2 = rx * rx + ry * ry + rz * rz;
+            const bool ok = (r2 <= rc2) && (r2 > (Real)0);
+            if (!ok) r2 = (Real)1;
+            Real C1, C2;
+            NearMath<Real>::coeffs(r2, xi, c2, mt, C1, C2);
+            if (!ok) { C1 = (Real)0; C2 = (Real)0; }
+            const Real rf = C2 * (rx * f0 + ry * f1 + rz * f2);
+            d0 = C1 * f0 + rf * rx;
+            d1 = C1 * f1 + rf * ry;
+            d2 = C1 * f2 + rf * rz;
+        }
+        if (modeB) {
+#pragma unroll
+            for (int sh = 16; sh > 0; sh >>= 1) {
+                d0 += __shfl_xor_sync(0xffffffffu, d0, sh);
+                d1 += __shfl_xor_sync(0xffffffffu, d1, sh);
+                d2 += __shfl_xor_sync(0xffffffffu, d2, sh);
+            }
+            if (lane == o) { a0 += d0; a1 += d1; a2 += d2; roff = (roff + cB * QSTRIDE) & (QBYTES - 1); }
+        } else if (have) {
+            a0 += d0; a1 += d1; a2 += d2;
+            roff = (roff + QSTRIDE) & (QBYTES - 1);
+        }
+    };
 
-        for (int dx = -1; dx <= 1; ++dx) {
-            int nx = cx + dx;
-            Real sx = 0;
-            if (nx < 0) { nx += nc; sx = -Lr; } else if (nx >= nc) { nx -= nc; sx = Lr; }
-            if (rel) sx = (Real)dx * wc;
-            for (int dy = -1; dy <= 1; ++dy) {
-                int ny = cy + dy;
-                Real sy = 0;
-                if (ny < 0) { ny += nc; sy = -Lr; } else if (ny >= nc) { ny -= nc; sy = Lr; }
-                if (rel) sy = (Real)dy * wc;
-                const int row = (nx * nc + ny) * nc;
-                // z-row segments: contiguous cells [zlo, zhi], first cell has offset dzlo
-                int nseg, zlo[2], zhi[2], dzlo[2];
-                Real sseg[2];
-                if (cz > 0 && cz < nc - 1) {
-                    nseg = 1; zlo[0] = cz - 1; zhi[0] = cz + 1; dzlo[0] = -1; sseg[0] = 0;
-                } else if (cz == 0) {
-                    nseg = 2;
-                    zlo[0] = nc - 1; zhi[0] = nc - 1; dzlo[0] = -1; sseg[0] = -Lr;
-                    zlo[1] = 0; zhi[1] = 1; dzlo[1] = 0; sseg[1] = 0;
-                } else {
-                    nseg = 2;
-                    zlo[0] = nc - 2; zhi[0] = nc - 1; dzlo[0] = -1; sseg[0] = 0;
-                    zlo[1] = 0; zhi[1] = 0; dzlo[1] = 1; sseg[1] = Lr;
-                }
-                for (int sg = 0; sg < nseg; ++sg) {
-                    const int jb = cell_start[row + zlo[sg]];
-                    const int je = cell_start[row + zhi[sg] + 1];
-                    // boundaries between the cells of the run (for the per-lane z offset, fp32 path)
-                    const int b1 = (zhi[sg] > zlo[sg]) ? cell_start[row + zlo[sg] + 1] : 0x7fffffff;
-                    const int b2 = (zhi[sg] > zlo[sg] + 1) ? cell_start[row + zlo[sg] + 2] : 0x7fffffff;
-                    for (int j0 = jb; j0 < je; j0 += 32) {
-                        const int j = j0 + lane;
-                        bool in = false;
-                        Real rx = 0, ry = 0, rz = 0;
-                        if (j < je) {
-                            Real sz = sseg[sg];
-                            if (rel) sz = (Real)(dzlo[sg] + (j >= b1) + (j >= b2)) * wc;
-                            rx = xi0 - (xs[3 * (int64_t)j + 0] + sx);
-                            ry = xi1 - (xs[3 * (int64_t)j + 1] + sy);
-                            rz = xi2 - (xs[3 * (int64_t)j + 2] + sz);
-                            Real r2 = rx * rx + ry * ry + rz * rz;
-                            in = (r2 <= rc2) && (r2 > (Real)0);
-                        }
-                        const unsigned m = __ballot_sync(0xffffffffu, in);
-                        if (in) {
-                            int k = (head + qn + __popc(m & lt_mask)) & (P2P_Q - 1);
-                            qx[w][k] = rx; qy[w][k] = ry; qz[w][k] = rz; qj[w][k] = j;
-                        }
-                        qn += __popc(m);
-                        if (qn >= 32) {
-                            heavy(32);
-                            head = (head + 32) & (P2P_Q - 1);
-                            qn -= 32;
+    unsigned remaining = __ballot_sync(0xffffffffu, valid);
+    while (remaining) {
+        // ---- pass: the targets of the first remaining lane's z-row whose cell is at most P2P_ZSPAN further ----
+        const int leader = __ffs(remaining) - 1;
+        const int pl = __shfl_sync(0xffffffffu, pci, leader);
+        const int cxl = pl >> 20, cyl = (pl >> 10) & 1023, czl = pl & 1023;
+        const int dzl = cz - czl;                                // this lane's cell, in cells from the leader's
+        const bool member = valid && (pci >> 10) == (pl >> 10) && dzl >= 0 && dzl <= P2P_ZSPAN;
+        const unsigned act = __ballot_sync(0xffffffffu, member) & remaining;
+        const int span = __reduce_max_sync(0xffffffffu, member ? dzl : 0);
+        const int ncl = span + 3;                                // source cells k = 0 .. ncl-1 <-> cell czl - 1 + k
+        const float tx0 = ((act >> lane) & 1u) ? qi.x : FAR;
+
+        // colleague rows in centre-out order, alternating sides, and the cells of a row centre-out as well: every
+        // lane then receives its hits at a roughly steady rate, which keeps all 32 queues non-empty
+#pragma unroll 1
+        for (int rr = 0; rr < 9; ++rr) {
+            const int dx = ((0x22161 >> (2 * rr)) & 3) - 1, dy = ((0x0a215 >> (2 * rr)) & 3) - 1;
+            int nx = cxl + dx, ny = cyl + dy;
+            if (nx < 0) nx += nc; else if (nx >= nc) nx -= nc;
+            if (ny < 0) ny += nc; else if (ny >= nc) ny -= nc;
+            const float tx = tx0 - (float)dx * wf, ty = qi.y - (float)dy * wf;
+            // lane k holds the CSR range of source cell k of this row
+            int cb = 0, ce = 0;
+            if (lane < ncl) {
+                int zc = czl - 1 + lane;
+                zc %= nc; if (zc < 0) zc += nc;
+                const int *cs = cell_start + (size_t)(nx * nc + ny) * nc + zc;
+                cb = __ldg(cs); ce = __ldg(cs + 1);
+            }
+            const int mid = ncl >> 1;
+#pragma unroll 1
+            for (int kk = 0; kk < ncl; ++kk) {
+                const int k = mid + ((kk & 1) ? -((kk + 1) >> 1) : (kk >> 1));
+                const int jb = __shfl_sync(0xffffffffu, cb, k), je = __shfl_sync(0xffffffffu, ce, k);
+                // a lane accepts the cell only if it is one of its own three colleague cells of this row
+                const int dk = k - 1 - dzl;
+                const float tz = (dk >= -1 && dk <= 1) ? qi.z - (float)dk * wf : FAR;
+#pragma unroll 1
+                for (int v0 = jb; v0 < je; v0 += (1 << P2P_VBITS)) {
+                    // open a virtual cell; its table slot may still be referenced by queued entries of the
+                    // virtual cell P2P_NV earlier: drain everything before wrapping around
+                    if (nv - nv_drained >= P2P_NV) {
+                        while (__any_sync(0xffffffffu, woff != roff)) round();
+                        nv_drained = nv;
+                    }
+                    const int vslot = nv & (P2P_NV - 1);
+                    ++nv;
+                    __syncwarp();
+                    if (lane == 0) {
+                        // (dx+1) | (dy+1) << 2 | image shift multipliers (+1) of x, y, z << 4, 6, 8 | (unwrapped z cell + 1) << 10
+                        const int zu = czl - 1 + k;
+                        const int xs = cxl + dx < 0 ? 0 : (cxl + dx >= nc ? 2 : 1), ys = cyl + dy < 0 ? 0 : (cyl + dy >= nc ? 2 : 1);
+                        const int zs = zu < 0 ? 0 : (zu >= nc ? 2 : 1);
+                        VT[vslot] = v0;
+                        VC[vslot] = (dx + 1) | ((dy + 1) << 2) | (xs << 4) | (ys << 6) | (zs << 8) | ((zu + 1) << 10);
+                    }
+                    __syncwarp();
+                    const int ve = min(je, v0 + (1 << P2P_VBITS));
+#pragma unroll 1
+                    for (int j0 = v0; j0 < ve; j0 += P2P_CHUNK) {
+                        while (__any_sync(0xffffffffu, queued() > P2P_QC - 1 - P2P_CHUNK)) round();
+                        const int n = min(P2P_CHUNK, ve - j0);
+                        const float4 *sq = xq + j0;
+                        const int ebase = (vslot << P2P_VBITS) + (j0 - v0);
+#pragma unroll 4
+                        for (int jj = 0; jj < n; ++jj) {
+                            const float4 q = __ldg(sq + jj);
+                            const float rx = tx - q.x, ry = ty - q.y, rz = tz - q.z;
+                            if (rx * rx + ry * ry + rz * rz <= rc2m) {
+                                *reinterpret_cast<unsigned short *>(Qb + woff) = (unsigned short)(ebase + jj);
+                                woff = (woff + QSTRIDE) & (QBYTES - 1);
+                            }
                         }
                     }
                 }
             }
         }
-        if (qn > 0) heavy(qn);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            a0 += __shfl_xor_sync(0xffffffffu, a0, o);
-            a1 += __shfl_xor_sync(0xffffffffu, a1, o);
-            a2 += __shfl_xor_sync(0xffffffffu, a2, o);
-        }
-        if (lane == 0) { uN[3 * i + 0] = a0; uN[3 * i + 1] = a1; uN[3 * i + 2] = a2; }
-        __syncwarp();
+        remaining &= ~act;
     }
+    while (__any_sync(0xffffffffu, woff != roff)) round();
+    if (valid) { uN[3 * i + 0] = a0; uN[3 * i + 1] = a1; uN[3 * i + 2] = a2; }
 }
 
 template <typename Real>
 cudaError_t p2p_impl(se_plan *p, cudaStream_t s)
 {
     const SeGeom &g = p->g;
-    int64_t per_block = (int64_t)P2P_WARPS * P2P_TPW;
+    int64_t per_block = (int64_t)P2P_WARPS * 32;
     unsigned nblk = (unsigned)((g.N + per_block - 1) / per_block);
-    k_p2p<Real><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const Real *)p->xs_near, (const Real *)p->fs_near,
-                                               p->cell_sorted, p->cell_start, (Real *)p->uN);
+    // FP32 filter margin: the cell-relative coordinates are < 2 wcell in magnitude, each rounded to 6e-8
+    // relative, so |dr| < 1e-6 wcell per component and |d r^2| < 2 sqrt(3) rc 1e-6 wcell
+    const double rc2m = g.rc * g.rc * (1.0 + 1e-5) + 4e-6 * g.rc * g.wcell;
+    k_p2p<Real><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)p->xq, (const Real *)p->src_near, p->cell_sorted,
+                                               p->cell_start, p->mtab, (Real *)p->uN, (float)rc2m);
     p->launches += 1;
     return cudaGetLastError();
 }
 
 }  // namespace
+
+// Host side of the function tables: interpolate at Chebyshev nodes in long double, convert to monomials.
+static void cheb_fit(long double (*fn)(long double), long double c, long double hw, int deg, double *out)
+{
+    const int n = deg + 1;
+    const long double PI = 3.14159265358979323846264338327950288L;
+    long double fv[24], ch[24], T[24][24] = {}, mono[24] = {};
+    for (int k = 0; k < n; ++k) fv[k] = fn(c + hw * cosl(PI * (k + 0.5L) / n));
+    for (int j = 0; j < n; ++j) {
+        long double a = 0;
+        for (int k = 0; k < n; ++k) a += fv[k] * cosl(PI * j * (k + 0.5L) / n);
+        ch[j] = (j == 0 ? 1.0L : 2.0L) * a / n;
+    }
+    T[0][0] = 1; if (n > 1) T[1][1] = 1;
+    for (int j = 2; j < n; ++j)
+        for (int i = 0; i <= j; ++i) T[j][i] = (i > 0 ? 2 * T[j - 1][i - 1] : 0) - T[j - 2][i];
+    for (int j = 0; j < n; ++j)
+        for (int i = 0; i <= j; ++i) mono[i] += ch[j] * T[j][i];
+    for (int i = 0; i < n; ++i) out[i] = (double)mono[i];
+}
+static long double erfcx_l(long double x) { return expl(x * x) * erfcl(x); }
+static long double exp_l(long double x) { return expl(x); }
+
+cudaError_t se_build_mtab(se_plan *p)
+{
+    static_assert(MT_DEG < 24 && MT_EXPDEG < 24, "cheb_fit scratch");
+    double h[MT_SIZE];
+    for (int i = 0; i < MT_NP; ++i) cheb_fit(erfcx_l, 0.25L * i + 0.125L, 0.125L, MT_DEG, h + i * MT_ROW);
+    // the polynomial is evaluated in t itself, not in t / hw: rescale the monomials
+    double e[MT_EXPDEG + 1];
+    const long double hw = 0.34657359027997265470861606072908828L * 1.0001L;   // ln2 / 2 and a little slack
+    cheb_fit(exp_l, 0.0L, hw, MT_EXPDEG, e);
+    long double s = 1;
+    for (int k = 0; k <= MT_EXPDEG; ++k) { h[MT_EXP + k] = (double)(e[k] / s); s *= hw; }
+    cudaError_t err = cudaMalloc(&p->mtab, sizeof(h));
+    if (err != cudaSuccess) return err;
+    p->workspace_bytes += sizeof(h);
+    return cudaMemcpy(p->mtab, h, sizeof(h), cudaMemcpyHostToDevice);
+}
 
 cudaError_t se_launch_p2p(se_plan *p, cudaStream_t s)
 {

@@ -178,24 +178,31 @@ __global__ void k_rank_in_cell(int64_t N, const int *__restrict__ key_of, const 
     inv[i] = s + r;
 }
 
+// Near-sorted copies for K2: src[p] = (x, y, z, f_x, f_y, f_z) in the plan's precision (absolute wrapped
+// coordinates for fp64 plans, cell-relative for fp32 plans), xq[p] = (x, y, z relative to the cell origin, absolute z)
+// in FP32 for the candidate filter, cellp[p] = packed cell coordinates (cx << 20 | cy << 10 | cz; ncell <= 1024).
 template <typename Real>
 __global__ void k_gather_near(SeGeom g, const Real *__restrict__ x, const Real *__restrict__ f,
                               const int *__restrict__ perm, const int *__restrict__ cell_of,
-                              Real *__restrict__ xs, Real *__restrict__ fs, int *__restrict__ cell_sorted)
+                              Real *__restrict__ src, float4 *__restrict__ xq, int *__restrict__ cellp)
 {
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= g.N) return;
     int i = perm[p];
     int ci = cell_of[i];
     int c[3] = {ci / (g.ncell * g.ncell), (ci / g.ncell) % g.ncell, ci % g.ncell};
+    float q[4];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         double v = wrap1((double)x[3 * (int64_t)i + d], g.L);
-        if (g.rel_coords) v -= (double)c[d] * g.wcell;     // cell-relative (fp32 path), rounded once
-        xs[3 * p + d] = (Real)v;
-        fs[3 * p + d] = f[3 * (int64_t)i + d];
+        double rel = v - (double)c[d] * g.wcell;            // cell-relative, rounded once
+        q[d] = (float)rel;
+        if (d == 2) q[3] = (float)v;
+        src[6 * p + d] = (Real)(g.rel_coords ? rel : v);
+        src[6 * p + 3 + d] = f[3 * (int64_t)i + d];
     }
-    cell_sorted[p] = ci;
+    xq[p] = make_float4(q[0], q[1], q[2], q[3]);
+    cellp[p] = (c[0] << 20) | (c[1] << 10) | c[2];
 }
 
 // one thread per (sorted particle, dim, l): window value exp(-beta (l - (P/2-1) - frac)^2)
@@ -280,8 +287,8 @@ cudaError_t sort_impl(se_plan *p, const void *xv, const void *fv, cudaStream_t s
                                  tmp_near, p->inv_near, tmp_grid, p->inv_grid);
     k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, p->cell_of, p->cell_start, tmp_near, p->perm_near, p->inv_near);
     k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, p->bin_of, p->bin_start, tmp_grid, p->perm_grid, p->inv_grid);
-    k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, p->perm_near, p->cell_of, (Real *)p->xs_near,
-                                           (Real *)p->fs_near, p->cell_sorted);
+    k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, p->perm_near, p->cell_of, (Real *)p->src_near,
+                                           (float4 *)p->xq, p->cell_sorted);
     int64_t nt = g.N * 3 * g.P;
     k_gather_grid<Real><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(g, x, f, p->perm_grid, p->anchor,
                                                                   (Real *)p->wtab, (Real *)p->recg, (Real *)p->fs_grid);
