@@ -154,12 +154,29 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
             g.nbins_total = M * zb * M;
             const int BY = 4 * SE_MMA_NWY, BZ = 4 * SE_MMA_NWZ;
             const int tiles = ((M + BY - 1) / BY) * ((M + BZ - 1) / BZ);
-            // One block per SM.  P2G re-spreads P-1 warm-up planes per chunk: chunk only as far as needed for
-            // ~4 waves; G2P warm-up is loads only, chunk freely (~8 waves).
-            int nch = (148 * 4 + tiles - 1) / tiles;
-            nch = std::min(nch, std::max(1, M / (4 * P)));
-            int nchg = (148 * 8 + tiles - 1) / tiles;
-            nchg = std::min(nchg, std::max(1, M / P));
+            // One block per SM, so the grid should fill whole waves of one block per SM (148).  A P2G chunk re-spreads P - 1
+            // warm-up planes (none when a single chunk covers the axis), a G2P chunk only re-loads them: pick the
+            // chunk counts that minimise (wave quantisation) x (warm-up overhead).
+            int nsm = 148;
+            if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) {
+                cudaGetLastError();
+                nsm = 148;
+            }
+            auto pick = [&](int nmax, bool spread) {
+                int best = 1;
+                double bc = 1e30;
+                for (int n = 1; n <= std::max(1, nmax); ++n) {
+                    const double w = (double)tiles * n / nsm;
+                    double cost = std::ceil(w) / w;
+                    const double cl = (double)M / n;
+                    if (spread) cost *= n == 1 ? 1.0 : (cl + P - 1) / cl;
+                    else cost *= 1.0 + 0.15 * (P - 1) / cl;
+                    if (cost < bc - 1e-9) { bc = cost; best = n; }
+                }
+                return best;
+            };
+            int nch = pick(M / (4 * P), true);
+            int nchg = pick(M / (2 * P), false);
             const char *e = std::getenv("SE_NCHUNK");
             if (e && std::atoi(e) > 0) nch = std::min(std::atoi(e), M);
             e = std::getenv("SE_NCHUNK_G2P");

@@ -30,8 +30,9 @@
 // The candidates of a (block tile, step) are at most 14 contiguous runs of the sorted order, so ONE
 // producer warp stages them with one bulk asynchronous copy (cp.async.bulk, the TMA engine) per run,
 // completing on the stage's `full` mbarrier; 12 consumer warps (152 registers each after setmaxnreg) test
-// the raw records against their own patch, copy the 4 + 4 window values under the patch into a per-warp
-// table (zero outside the support) and release the stage through its `empty` mbarrier.  In G2P the other
+// the raw records against their own patch, keep a packed hit list (candidate, window index of the patch origin
+// in y and z) and read the window values under the patch straight from the staged records (zero outside the
+// support); they release the stage through its `empty` mbarrier.  In G2P the other
 // three warps of the producer warpgroup add the consumers' per-warp partial sums in fixed order and write
 // the slot before the stage is refilled.
 #include <climits>
@@ -96,9 +97,14 @@ struct Cfg {
     static constexpr int MT = P / 8;                           // m-tiles in the ring
     static constexpr int REC = SPREAD ? SE_MMA_RECS(P) : SE_MMA_RECG(P);   // doubles per record
     static constexpr int OY = SPREAD ? 3 * P : P, OZ = OY + P, OM = OZ + P; // offsets of Wy, Wz, (a_y, a_z)
-    static constexpr int NST = SPREAD ? 3 : 4;                 // stages
+#ifndef SE_EXP_NST
+#define SE_EXP_NST 5
+#endif
+#ifndef SE_EXP_NSTS
+#define SE_EXP_NSTS 3
+#endif
+    static constexpr int NST = SPREAD ? SE_EXP_NSTS : SE_EXP_NST;       // stages
     static constexpr int GRP = SPREAD ? 4 : 8;                 // candidates per K-group (P2G: k = 4; G2P: n = 8)
-    static constexpr int TS = SPREAD ? 36 : 72;                // doubles per group in the patch-window table
     static constexpr int NSB = (P + BY - 2) / BY + 2, NSC = (P + BZ - 2) / BZ + 2;   // block tiles a window can meet
     static_assert(P % 8 == 0 && (REC % 2) == 0 && NCW % 4 == 0 && CAP % GRP == 0, "layout");
 };
@@ -112,18 +118,14 @@ struct alignas(16) Stage {
     double rec[CAP + 1][C::REC];             // [CAP] stays all-zero: the padding record
     double U[SPREAD ? 1 : CAP][C::NCW][3];   // G2P: per-warp partial sums of the round
     int pidx[SPREAD ? 1 : CAP];              // G2P: sorted index of the candidate (slot write-out)
+    unsigned char hit[SPREAD ? 1 : CAP][SPREAD ? 4 : 16];   // G2P: did consumer warp w gather from candidate a?
     int s, na, rs, pad;                      // step (anchor plane, unwrapped), candidate count, s mod P
 };
 
-// Per-warp scratch of a round: the hit list and, per hit, the 4 + 4 window values under the warp's patch
-// (zero outside the support), laid out [group][value][hit in group] so that the group loop reads them with
-// fixed per-lane offsets and without bank conflicts (TS = 4 mod 16 / 8 mod 16 doubles keeps the stores of
-// consecutive hits in different banks too).
+// Per-warp scratch of a round: the packed hit list.
 template <int P, bool SPREAD>
 struct alignas(16) WarpScratch {
-    typedef Cfg<P, SPREAD> C;
-    double tb[CAP / C::GRP][C::TS];
-    unsigned char wl[CAP + 8];
+    unsigned wl[CAP + 8];            // hit list: candidate a | l_y << 8 | l_z << 20 (window index of the patch origin)
 };
 
 template <int P, bool SPREAD>
@@ -138,13 +140,6 @@ __device__ __forceinline__ int modM(int v, int M) { v %= M; return v < 0 ? v + M
 
 // does the window [0, P) (indices mod M) meet columns T0 .. T0 + n - 1, given l0 = (T0 - anchor) mod M ?
 __device__ __forceinline__ bool meets(int l0, int n, int M, int P) { return n > 0 && (l0 < P || l0 + n - 1 >= M); }
-
-// window value W[(l0 + i) mod M] of a record row, zero outside the support
-__device__ __forceinline__ double wval(const double *w, int l0, int i, int M, int P)
-{
-    int l = l0 + i; if (l >= M) l -= M;
-    return l < P ? w[l] : 0.0;
-}
 
 template <int P, bool SPREAD>
 __global__ void __launch_bounds__((NWY * NWZ + 4) * 32, 1)
@@ -166,7 +161,11 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
     const int CLen = min(CL, M - X0);
     if (CLen <= 0) return;
     const int Y0 = ty * BY, Z0 = tz * BZ;
-    const int s_begin = SPREAD ? X0 - (P - 1) : X0, s_end = X0 + CLen;
+    // P2G: a chunk re-spreads the P - 1 anchor planes in front of it (warm-up) -- except when one chunk covers the
+    // whole periodic axis: then the sweep starts at plane 0 and the P - 1 planes left in the ring at the end are the
+    // wrapped contributions to planes 0 .. P - 2, which the same thread adds to what it wrote there (no warm-up).
+    const bool wrap_add = SPREAD && nchunk == 1;
+    const int s_begin = (SPREAD && !wrap_add) ? X0 - (P - 1) : X0, s_end = X0 + CLen;
 
     for (int e = tid; e < NST * REC; e += C::NT) S.st[e / REC].rec[CAP][e % REC] = 0.0;
     if (tid == 0)
@@ -198,7 +197,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                     if (hit && rb < C::NSB && rc < C::NSC) {
                         double sum = 0.0;
 #pragma unroll
-                        for (int w = 0; w < NCW; ++w) sum += T.U[a][w][c];
+                        for (int w = 0; w < NCW; ++w) sum += T.hit[a][w] ? T.U[a][w][c] : 0.0;
                         uFpart[((size_t)(rb * C::NSC + rc) * g.N + T.pidx[a]) * 3 + c] = sum;
                     }
                 }
@@ -316,44 +315,35 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
         if (++curM == M) curM = 0;
     };
 
-    // this warp's hits of a round: list + patch-window table, padded to whole K-groups with the zero record
+    // this warp's hits of a round: packed list (candidate, window index of the patch origin in y and z), padded
+    // to whole K-groups with the all-zero record.  The DMMA operands are read from the staged records
+    // directly (window value W[(l0 + i) mod M], zero outside the support): no per-warp copy of the windows.
     auto build_hits = [&](Stage<P, SPREAD> &T, int na) -> int {
         int cnt = 0;
         for (int a0 = 0; a0 < na; a0 += 32) {
             const int a = a0 + lane;
             bool hit = false;
             int ly = 0, lz = 0;
-            const double *rp = T.rec[min(a, CAP)];
             if (a < na) {
-                const int2 an = *reinterpret_cast<const int2 *>(&rp[C::OM]);
+                const int2 an = *reinterpret_cast<const int2 *>(&T.rec[a][C::OM]);
                 ly = Yw - an.x; if (ly < 0) ly += M;
                 lz = Zw - an.y; if (lz < 0) lz += M;
                 hit = meets(ly, nyw, M, P) && meets(lz, nzw, M, P);
-                if (!SPREAD && !hit) { T.U[a][warp][0] = 0.0; T.U[a][warp][1] = 0.0; T.U[a][warp][2] = 0.0; }
+                if (!SPREAD) T.hit[a][warp] = (unsigned char)hit;
             }
             const unsigned m = __ballot_sync(0xffffffffu, hit);
-            if (hit) {
-                const int h = cnt + __popc(m & ((1u << lane) - 1u));
-                WS.wl[h] = (unsigned char)a;
-                double *t = &WS.tb[h / GRP][h % GRP];
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    t[i * GRP] = wval(rp + C::OY, ly, i, M, P);
-                    t[(4 + i) * GRP] = wval(rp + C::OZ, lz, i, M, P);
-                }
-            }
+            if (hit) WS.wl[cnt + __popc(m & ((1u << lane) - 1u))] = (unsigned)a | ((unsigned)ly << 8) | ((unsigned)lz << 20);
             cnt += __popc(m);
         }
         const int padded = (cnt + GRP - 1) & ~(GRP - 1);
-        if (lane < padded - cnt) {
-            const int h = cnt + lane;
-            WS.wl[h] = (unsigned char)CAP;
-            double *t = &WS.tb[h / GRP][h % GRP];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) t[i * GRP] = 0.0;
-        }
+        if (lane < padded - cnt) WS.wl[cnt + lane] = (unsigned)CAP;
         __syncwarp();
         return padded;
+    };
+    // window value W[(l0 + i) mod M] of a staged record row, zero outside the support (l0 + i < 2 M)
+    auto wrec = [&](const double *w, int l) -> double {
+        if (l >= M) l -= M;
+        return l < P ? w[l] : 0.0;
     };
 
     if constexpr (SPREAD) {
@@ -402,6 +392,34 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
             const int s = T.s, na = T.na, rs = T.rs;
             if (s >= s_end) {                                        // terminal round
                 while (cur < s_end) { flush(); advance(); }
+                if (wrap_add) {
+                    // ring residue 8 mt + gq now holds plane s_end + t, t = (8 mt + gq - s_end) mod P, i.e. grid
+                    // plane t of the next period: all loads first, then add and store
+                    double2 o[MT][3][2];
+                    int tt[MT];
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        int t = 8 * mt + gq - curP; if (t < 0) t += P;
+                        tt[mt] = t;
+#pragma unroll
+                        for (int c = 0; c < 3; ++c)
+#pragma unroll
+                            for (int j = 0; j < 2; ++j)
+                                if (cz_ok && t < P - 1 && 2 * j + cyl < nyw)
+                                    o[mt][c][j] = *reinterpret_cast<const double2 *>(
+                                        &grid[c * M3 + (size_t)t * MM + colS + (size_t)(2 * j) * M]);
+                    }
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c)
+#pragma unroll
+                            for (int j = 0; j < 2; ++j)
+                                if (cz_ok && tt[mt] < P - 1 && 2 * j + cyl < nyw)
+                                    *reinterpret_cast<double2 *>(
+                                        &grid[c * M3 + (size_t)tt[mt] * MM + colS + (size_t)(2 * j) * M]) =
+                                        make_double2(o[mt][c][j].x + acc[mt][c][j][0], o[mt][c][j].y + acc[mt][c][j][1]);
+                }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&S.empty[sg]);
                 break;
@@ -412,24 +430,28 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
             int lx[MT];
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) { int l = 8 * mt + gq - rs; lx[mt] = l < 0 ? l + P : l; }
-            // B[k = tq][n = gq].  No FP64 arithmetic feeds a DMMA of the same group: the two B products of
-            // group q + 1 are formed while group q issues.
-            const double *tq0 = &WS.tb[0][(gq >> 2) * 4 + tq], *tqz = &WS.tb[0][(4 + (gq & 3)) * 4 + tq];
+            // B[k = tq][n = gq] = Wy Wz of hit tq at column n of the two n-tiles (rows gq >> 2 and + 2, z-column
+            // gq & 3).  No FP64 arithmetic feeds a DMMA of the same group: the two B products of group q + 1
+            // are formed while group q issues.
+            const int by = gq >> 2, bz = gq & 3;
+            auto bprod = [&](unsigned w, double &p0, double &p1) {
+                const double *rp = T.rec[w & 0xffu];
+                const int ly = (int)((w >> 8) & 0xfffu) + by, lz = (int)(w >> 20) + bz;
+                const double wz = wrec(rp + C::OZ, lz);
+                p0 = wrec(rp + C::OY, ly) * wz; p1 = wrec(rp + C::OY, ly + 2) * wz;
+            };
+            unsigned wcur = 0;
             double b0 = 0.0, b1 = 0.0;
-            if (padded > 0) { const double wz = tqz[0]; b0 = tq0[0] * wz; b1 = tq0[8] * wz; }
+            if (padded > 0) { wcur = WS.wl[tq]; bprod(wcur, b0, b1); }
             for (int q = 0; q < padded; q += 4) {
-                const double *rp = T.rec[WS.wl[q + tq]];
+                const double *rp = T.rec[wcur & 0xffu];
                 double a[MT][3];
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
                     for (int c = 0; c < 3; ++c) a[mt][c] = rp[c * P + lx[mt]];
                 const double c0 = b0, c1 = b1;
-                if (q + 4 < padded) {
-                    const int o = (q / 4 + 1) * C::TS;
-                    const double wz = tqz[o];
-                    b0 = tq0[o] * wz; b1 = tq0[o + 8] * wz;
-                }
+                if (q + 4 < padded) { wcur = WS.wl[q + 4 + tq]; bprod(wcur, b0, b1); }
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) {
                     dmma(acc[mt][0][0], a[mt][0], c0); dmma(acc[mt][0][1], a[mt][0], c1);
@@ -465,7 +487,11 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
             for (int c = 0; c < 3; ++c)
 #pragma unroll
                 for (int j = 0; j < 2; ++j)
+#ifdef SE_EXP_NORING
+                    pre[c][j] = (double)(XM + c + j);
+#else
                     pre[c][j] = (gz_ok && 2 * j + gyl < nyw) ? __ldg(&grid[c * M3 + off + (size_t)(2 * j) * M]) : 0.0;
+#endif
         };
         auto commit_ks = [&](auto ksc) {
             constexpr int ks = decltype(ksc)::value;
@@ -510,15 +536,17 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
             for (int ks = 0; ks < KS; ++ks) { int l = 4 * ks + tq - rs; lx[ks] = l < 0 ? l + P : l; }
             // epilogue weights of hit gq at this lane's D columns n = 2 tq, 2 tq + 1 of n-tile j:
             // row 2j + (tq >> 1), z-columns 2 (tq & 1), + 1
-            const double *ty = &WS.tb[0][(tq >> 1) * 8 + gq], *tz = &WS.tb[0][(4 + 2 * (tq & 1)) * 8 + gq];
+            const int ey = tq >> 1, ez = 2 * (tq & 1);
             for (int q = 0; q < padded; q += 8) {
-                const int o = (q / 8) * C::TS;
-                const int a = WS.wl[q + gq];
+                const unsigned w = WS.wl[q + gq];
+                const int a = (int)(w & 0xffu);
                 const double *rp = T.rec[a];
                 double wx[KS];
 #pragma unroll
                 for (int ks = 0; ks < KS; ++ks) wx[ks] = rp[lx[ks]];
-                const double wy0 = ty[o], wy1 = ty[o + 16], wz0 = tz[o], wz1 = tz[o + 8];
+                const int ly = (int)((w >> 8) & 0xfffu) + ey, lz = (int)(w >> 20) + ez;
+                const double wy0 = wrec(rp + C::OY, ly), wy1 = wrec(rp + C::OY, ly + 2);
+                const double wz0 = wrec(rp + C::OZ, lz), wz1 = wrec(rp + C::OZ, lz + 1);
                 const double w00 = wy0 * wz0, w01 = wy0 * wz1, w10 = wy1 * wz0, w11 = wy1 * wz1;
                 double d[3][2][2];
 #pragma unroll
@@ -530,11 +558,16 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                 double pc[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
+#ifdef SE_EXP_NOEPI
+                    long long z = __double_as_longlong(d[c][0][0]) ^ __double_as_longlong(d[c][0][1]) ^ __double_as_longlong(d[c][1][0]) ^ __double_as_longlong(d[c][1][1]) ^ __double_as_longlong(w00)^ __double_as_longlong(w01)^ __double_as_longlong(w10)^ __double_as_longlong(w11);
+                    pc[c] = __longlong_as_double(z);
+#else
                     double v = d[c][0][0] * w00;
                     v = fma(d[c][0][1], w01, v); v = fma(d[c][1][0], w10, v); v = fma(d[c][1][1], w11, v);
                     v += __shfl_xor_sync(0xffffffffu, v, 1);
                     v += __shfl_xor_sync(0xffffffffu, v, 2);
                     pc[c] = v;
+#endif
                 }
                 if (tq == 0 && a < CAP) { T.U[a][warp][0] = pc[0]; T.U[a][warp][1] = pc[1]; T.U[a][warp][2] = pc[2]; }
             }
