@@ -165,3 +165,23 @@ def random_spectrum(seed: int, M: int, ncomp: int = 3):
     rng = np.random.default_rng(seed)
     shp = (ncomp, M, M, M // 2 + 1)
     return (rng.standard_normal(shp) + 1j * rng.standard_normal(shp)).astype(np.complex128)
+
+
+# ---- index-defined synthetic fields (full-size stand-alone K4 / K5 parity) ------------------------
+# Closed-form functions of the integer grid indices, so that the same field can be written on the device
+# (xp = torch) and evaluated on the host (xp = numpy) at any size without storing or moving it.  No
+# arithmetic of the method: plain cosines of index combinations.
+def index_grid(xp, c, i, j, k, M):
+    """Smooth real grid value of component c at (i, j, k): a few low wavenumbers of the periodic box,
+    written as products of 1-D factors so that broadcasting index arrays keeps the cosines one-dimensional."""
+    w = 2.0 * np.pi / M
+    return (xp.cos(w * 2.0 * i + 0.3 * c) * xp.cos(w * j) * xp.cos(w * 3.0 * k)
+            + 0.5 * xp.cos(w * i - 0.7 * c) * xp.sin(w * 2.0 * j)
+            + 0.25 * xp.cos(w * 2.0 * i) * xp.cos(w * 3.0 * k + 1.1))
+
+
+def index_spectrum(xp, c, i, j, k):
+    """Complex half-spectrum value of component c at mode indices (i, j, k): (re, im), O(1) everywhere."""
+    re = xp.cos(0.37 * i + 0.5 * c) * xp.cos(0.11 * j) + 0.5 * xp.cos(0.73 * k + 0.2)
+    im = xp.cos(0.23 * i + 1.3) * xp.cos(0.19 * k + 0.9 * c) - 0.5 * xp.cos(0.41 * j)
+    return re, im
