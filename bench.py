@@ -31,7 +31,7 @@ METRIC = "particles/s, full Stokes SE sum"
 UNIT = "particles/s"
 # FP64 / FP32 FMA peak of one B200 from unit counts and clocks:
 # 148 SMs x 64 (128) FMA lanes x 2 flop x 1.965 GHz.  A register-only DFMA/FFMA chain measured
-# 36.7 / 72.0 TFLOP/s on this pool (profiles/r01_peaks.md).
+# 36.7 / 72.0 TFLOP/s on this pool (profiles/r01b_mma_ws.md).
 ALU_PEAK_TFLOPS = {"fp64": 148 * 64 * 2 * 1.965e9 / 1e12, "fp32": 148 * 128 * 2 * 1.965e9 / 1e12}
 SAMPLE_CFG = 2          # the oracle's bounded sample: config 2 in full
 
