@@ -5,7 +5,8 @@
 // thread-per-target loop runs the expensive erfc/exp code at ~15% lane utilisation, and on
 // B200 the FP64 pipe (64 lanes per SM) is the scarce resource.  Here a LANE owns a target (32 consecutive
 // targets of the near-sorted order per warp) and the work is split by pipe:
-//   phase A (filter; FP32 pipe, one broadcast 16-byte load per source): the warp walks the sources of the
+//   phase A (filter; FP32 pipe; sources fetched 32 at a time, one coalesced 16-byte load per lane one chunk ahead,
+//            and broadcast from a shared-memory line): the warp walks the sources of the
 //            colleague cells; every lane forms r^2 to its own target in FP32 from the compact copy `xq` K1
 //            wrote (coordinates relative to the particle's cell, so periodic images cost nothing) and, if
 //            r^2 <= rc^2 (1 + margin), appends the source index to ITS OWN ring queue in shared memory
@@ -22,8 +23,10 @@
 // A warp whose targets span several cells processes them in passes: the targets of one z-row of cells whose
 // cell index is within P2P_ZSPAN of the first; a lane only accepts sources of its own 27 colleague cells.
 // A queue entry is 16 bits: (virtual cell << 9) | offset, a virtual cell being <= 512 consecutive sources of one
-// colleague cell; a per-warp table maps it to the first source index and to the periodic image p of that cell.  fp32 plans use cell-relative positions in phase B too, so that r keeps full
-// float precision across images.
+// colleague cell; a per-warp table maps it to the first source index and to the periodic image shift p of that
+// cell (three reals, written once when the virtual cell is opened).  fp32 plans use cell-relative positions in
+// phase B too, so that r keeps full float precision across images; their erfcx is a degree-5 table of the same
+// form as the double one (the fresh single-precision path: no libm erfc, no division).
 #include <cmath>
 
 #include "se_common.cuh"
@@ -34,25 +37,34 @@ constexpr int P2P_WARPS = 4;
 constexpr int P2P_QC = 128;         // ring-queue slots per lane (power of two), 16-bit entries
 constexpr int P2P_CHUNK = 32;       // sources scanned between two queue-room checks
 constexpr int P2P_VBITS = 9;        // a queue entry = (virtual cell << VBITS) | offset: virtual cells of <= 512 sources
-constexpr int P2P_NV = 128;         // virtual-cell table entries per warp ((NV << VBITS) = 2^16)
+constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV << VBITS) = 2^15)
 constexpr int P2P_ZSPAN = 6;        // cells along z a pass may span (<= 29: one lane per source cell)
 
-// ---- function tables (built on the host in long double at plan creation, copied to shared memory per block) ----
-// erfcx(x) = e^{x^2} erfc(x) on [0, 8): 32 pieces of width 1/4, each a degree-10 polynomial in the local
-// variable u = 8 x - (2 i + 1) in [-1, 1] (interpolation at Chebyshev nodes, converted to monomials; measured
-// relative error < 4e-16).  Row stride 11 doubles = 22 words: 16 consecutive rows start in 16 different bank
-// pairs, so lanes in different pieces read their coefficients without bank conflicts.  For x >= 8 the argument
-// is clamped; e^{-x^2} < 2e-28 there.
-// e^t on [-ln2/2, ln2/2]: degree-11 polynomial (Chebyshev interpolant, relative error < 1e-17).
-constexpr int MT_NP = 32, MT_DEG = 10, MT_ROW = MT_DEG + 1;
-constexpr int MT_EXP = MT_NP * MT_ROW, MT_EXPDEG = 11;
-constexpr int MT_SIZE = MT_EXP + MT_EXPDEG + 1;
+// ---- function tables (built on the host in long double at plan creation) --------------------------------------
+// erfcx(x) = e^{x^2} erfc(x) on [0, 8]: 33 pieces centred at i/4 (half-width 1/8), each a polynomial in the local
+// variable v = x - i/4 (interpolation at Chebyshev nodes, converted to monomials): degree 10 in double (measured
+// relative error < 4e-16), degree 5 in float (< 2e-8 before rounding).  The piece index comes out of the
+// round-to-nearest shifter trick (no float <-> int conversion instructions).  Row stride 11 doubles = 22 words: 16
+// consecutive rows start in 16 different bank pairs.  For x >= 8 the argument is clamped; e^{-x^2} < 2e-28 there.
+// e^t on [-ln2/2, ln2/2]: degree-11 polynomial (Chebyshev interpolant, relative error < 1e-17), kept in constant
+// memory so that its coefficients are FMA operands, not loads.
+constexpr int MT_NP = 33, MT_DEG = 10, MT_ROW = MT_DEG + 1;
+constexpr int MT_DEGF = 5, MT_ROWF = MT_DEGF + 1;
+constexpr int MT_F32 = MT_NP * MT_ROW;                           // offset of the float table, in doubles
+constexpr int MT_SIZE = MT_F32 + (MT_NP * MT_ROWF + 1) / 2;      // doubles in p->mtab
+constexpr int MT_EXPDEG = 11;
+__constant__ double c_exp[MT_EXPDEG + 1];
 
 template <typename Real> struct NearMath;
 
 template <> struct NearMath<double> {
+    static constexpr int TAB = MT_NP * MT_ROW;                   // table entries in shared memory
+    static __device__ __forceinline__ void load(double *mt, const double *mtab, int tid, int nt)
+    {
+        for (int e = tid; e < TAB; e += nt) mt[e] = mtab[e];
+    }
     // e^{-y}, y >= 0
-    static __device__ __forceinline__ double exp_neg(double y, const double *mt)
+    static __device__ __forceinline__ double exp_neg(double y)
     {
         y = fmin(y, 700.0);
         const double SH = 6755399441055744.0;                    // 1.5 * 2^52: round-to-nearest integer shifter
@@ -61,27 +73,35 @@ template <> struct NearMath<double> {
         const double nf = t - SH;
         double r = fma(nf, -6.93147180369123816490e-01, -y);     // r = -y - n ln2 (ln2 split hi + lo)
         r = fma(nf, -1.90821492927058770002e-10, r);
-        const double *c = mt + MT_EXP;
-        double p = c[MT_EXPDEG];
+        double p = c_exp[MT_EXPDEG];
 #pragma unroll
-        for (int k = MT_EXPDEG - 1; k >= 0; --k) p = fma(p, r, c[k]);
+        for (int k = MT_EXPDEG - 1; k >= 0; --k) p = fma(p, r, c_exp[k]);
         return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
     }
     static __device__ __forceinline__ double erfcx_tab(double x, const double *mt)
     {
-        const double xm = fmin(x, 7.99999999);
-        const int i = (int)(4.0 * xm);
-        const double u = fma(8.0, xm, -(double)(2 * i + 1));
-        const double *c = mt + i * MT_ROW;
+        const double SH = 6755399441055744.0;
+        const double xm = fmin(x, 8.0);
+        const double t = fma(xm, 4.0, SH);                       // piece i = rint(4 x), v = x - i/4
+        const double v = fma(t - SH, -0.25, xm);
+        const double *c = mt + __double2loint(t) * MT_ROW;
         double p = c[MT_DEG];
 #pragma unroll
-        for (int k = MT_DEG - 1; k >= 0; --k) p = fma(p, u, c[k]);
+        for (int k = MT_DEG - 1; k >= 0; --k) p = fma(p, v, c[k]);
         return p;
+    }
+    // 1/sqrt(x), x > 0 finite: hardware seed (2^-22) and one third-order correction, no special cases
+    static __device__ __forceinline__ double rsq(double x)
+    {
+        double y;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+        const double e = fma(-(x * y), y, 1.0);
+        return fma(y * e, fma(0.375, e, 0.5), y);
     }
     static __device__ __forceinline__ void coeffs(double r2, double xi, double c2, const double *mt, double &C1, double &C2)
     {
-        const double rinv = rsqrt(r2);
-        const double e = exp_neg(xi * xi * r2, mt);
+        const double rinv = rsq(r2);
+        const double e = exp_neg(xi * xi * r2);
         const double A = e * erfcx_tab(xi * (r2 * rinv), mt) * rinv;
         const double B = c2 * e;
         C1 = A - B;
@@ -90,12 +110,30 @@ template <> struct NearMath<double> {
 };
 
 template <> struct NearMath<float> {
-    static __device__ __forceinline__ void coeffs(float r2, float xi, float c2, const double *, float &C1, float &C2)
+    static constexpr int TAB = MT_NP * MT_ROWF;
+    static __device__ __forceinline__ void load(float *mt, const double *mtab, int tid, int nt)
+    {
+        const float *src = reinterpret_cast<const float *>(mtab + MT_F32);
+        for (int e = tid; e < TAB; e += nt) mt[e] = src[e];
+    }
+    static __device__ __forceinline__ float erfcx_tab(float x, const float *mt)
+    {
+        const float SH = 12582912.0f;                            // 1.5 * 2^23
+        const float xm = fminf(x, 8.0f);
+        const float t = fmaf(xm, 4.0f, SH);
+        const float v = fmaf(t - SH, -0.25f, xm);
+        const float *c = mt + (__float_as_int(t) - __float_as_int(SH)) * MT_ROWF;
+        float p = c[MT_DEGF];
+#pragma unroll
+        for (int k = MT_DEGF - 1; k >= 0; --k) p = fmaf(p, v, c[k]);
+        return p;
+    }
+    static __device__ __forceinline__ void coeffs(float r2, float xi, float c2, const float *mt, float &C1, float &C2)
     {
         float rinv = rsqrtf(r2);
         float x2 = xi * xi * r2;
         float e = expf(-x2);
-        float A = e * erfcxf(xi * (r2 * rinv)) * rinv;
+        float A = e * erfcx_tab(xi * (r2 * rinv), mt) * rinv;
         float B = c2 * e;
         C1 = A - B;
         C2 = (A + B) * (rinv * rinv);
@@ -107,12 +145,13 @@ __global__ void __launch_bounds__(P2P_WARPS * 32, 4)
 k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, const int *__restrict__ cellp,
       const int *__restrict__ cell_start, const double *__restrict__ mtab, Real *__restrict__ uN, float rc2m)
 {
-    __shared__ double mt[MT_SIZE];
-    for (int e = threadIdx.x; e < MT_SIZE; e += P2P_WARPS * 32) mt[e] = mtab[e];
+    __shared__ Real mt[NearMath<Real>::TAB];
+    NearMath<Real>::load(mt, mtab, threadIdx.x, P2P_WARPS * 32);
     __syncthreads();
     __shared__ unsigned short qsm[P2P_WARPS][P2P_QC][32];
     __shared__ int vtab[P2P_WARPS][P2P_NV];                      // virtual cell -> sorted index of its first source
-    __shared__ int vcode[P2P_WARPS][P2P_NV];                     // virtual cell -> packed offsets / image shifts (below)
+    __shared__ Real vshift[P2P_WARPS][P2P_NV][3];                // virtual cell -> periodic image shift of its sources
+    __shared__ float4 sbuf[P2P_WARPS][P2P_CHUNK];                // the chunk of sources being tested (broadcast reads)
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int nc = g.ncell;
@@ -124,7 +163,9 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     constexpr float FAR = 1.0e18f;                               // coordinate of a lane that must not match
     char *const Qb = reinterpret_cast<char *>(&qsm[w][0][lane]); // this lane's queue column, slot stride 64 B
     constexpr int QSTRIDE = 64, QBYTES = P2P_QC * QSTRIDE;
-    int *const VT = vtab[w], *const VC = vcode[w];
+    int *const VT = vtab[w];
+    Real (*const VS)[3] = vshift[w];
+    float4 *const SB = sbuf[w];
     int nv = 0, nv_drained = 0;                                  // virtual cells opened / opened at the last full drain
 
     const int64_t i = ((int64_t)blockIdx.x * P2P_WARPS + w) * 32 + lane;
@@ -135,6 +176,7 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     const int cx = pci >> 20, cy = (pci >> 10) & 1023, cz = pci & 1023;
     const Real X0 = src[6 * ic + 0], X1 = src[6 * ic + 1], X2 = src[6 * ic + 2];
     Real a0 = 0, a1 = 0, a2 = 0;
+    const Real czw = g.rel_coords ? (Real)cz * wc : (Real)0;    // z offset of this target's cell (cell-relative plans)
     int woff = 0, roff = 0;                                      // ring write / read offsets (bytes); empty when equal
 
     auto queued = [&]() { return ((woff - roff) & (QBYTES - 1)) / QSTRIDE; };
@@ -148,13 +190,13 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
         const int cmax = __reduce_max_sync(0xffffffffu, c);
         const int cB = min(cmax, 32);
         const bool modeB = cB > __popc(m1);                      // warp-uniform
-        Real T0 = X0, T1 = X1, T2 = X2;
-        int tp = pci, ro = roff, o = lane;
+        Real T0 = X0, T1 = X1, T2 = X2, tcz = czw;
+        int ro = roff, o = lane;
         bool have = c > 0;
         if (modeB) {
             o = __ffs(__ballot_sync(0xffffffffu, c == cmax)) - 1;
             T0 = __shfl_sync(0xffffffffu, X0, o); T1 = __shfl_sync(0xffffffffu, X1, o); T2 = __shfl_sync(0xffffffffu, X2, o);
-            tp = __shfl_sync(0xffffffffu, pci, o);
+            tcz = __shfl_sync(0xffffffffu, czw, o);
             ro = (__shfl_sync(0xffffffffu, roff, o) + lane * QSTRIDE) & (QBYTES - 1);
             have = lane < cB;
         }
@@ -175,16 +217,10 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                 const float2 p2 = __ldg(reinterpret_cast<const float2 *>(sp + 4));
                 xj = (Real)p0.x; yj = (Real)p0.y; zj = (Real)p1.x; f0 = (Real)p1.y; f1 = (Real)p2.x; f2 = (Real)p2.y;
             }
-            // periodic image of the source as this target sees it, from the virtual cell's packed code
-            const int code = VC[e >> P2P_VBITS];
-            Real sx, sy, sz;
-            if (g.rel_coords) {
-                sx = (Real)((code & 3) - 1) * wc; sy = (Real)(((code >> 2) & 3) - 1) * wc;
-                sz = (Real)((code >> 10) - 1 - (tp & 1023)) * wc;
-            } else {
-                sx = (Real)(((code >> 4) & 3) - 1) * Lr; sy = (Real)(((code >> 6) & 3) - 1) * Lr;
-                sz = (Real)(((code >> 8) & 3) - 1) * Lr;
-            }
+            // periodic image of the source as this target sees it: the virtual cell's shift (absolute coordinates:
+            // a multiple of L per axis; cell-relative coordinates: the cell offset, in z from the target's own cell)
+            const Real *vs = VS[e >> P2P_VBITS];
+            const Real sx = vs[0], sy = vs[1], sz = vs[2] - tcz;
             const Real rx = T0 - (xj + sx), ry = T1 - (yj + sy), rz = T2 - (zj + sz);
             Real r2 = rx * rx + ry * ry + rz * rz;
             const bool ok = (r2 <= rc2) && (r2 > (Real)0);
@@ -260,31 +296,42 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                     const int vslot = nv & (P2P_NV - 1);
                     ++nv;
                     __syncwarp();
-                    if (lane == 0) {
-                        // (dx+1) | (dy+1) << 2 | image shift multipliers (+1) of x, y, z << 4, 6, 8 | (unwrapped z cell + 1) << 10
-                        const int zu = czl - 1 + k;
-                        const int xs = cxl + dx < 0 ? 0 : (cxl + dx >= nc ? 2 : 1), ys = cyl + dy < 0 ? 0 : (cyl + dy >= nc ? 2 : 1);
-                        const int zs = zu < 0 ? 0 : (zu >= nc ? 2 : 1);
-                        VT[vslot] = v0;
-                        VC[vslot] = (dx + 1) | ((dy + 1) << 2) | (xs << 4) | (ys << 6) | (zs << 8) | ((zu + 1) << 10);
+                    if (lane < 3) {
+                        // lane a writes the shift along axis a (x, y, z)
+                        const int zu = czl - 1 + k;              // unwrapped z cell of the sources
+                        const int cu = lane == 0 ? cxl + dx : (lane == 1 ? cyl + dy : zu);
+                        Real sh;
+                        if (g.rel_coords) sh = (Real)(lane == 0 ? dx : (lane == 1 ? dy : zu)) * wc;
+                        else sh = cu < 0 ? -Lr : (cu >= nc ? Lr : (Real)0);
+                        VS[vslot][lane] = sh;
+                        if (lane == 0) VT[vslot] = v0;
                     }
                     __syncwarp();
                     const int ve = min(je, v0 + (1 << P2P_VBITS));
+                    // the 32 sources of a chunk are fetched with one coalesced 16-byte load per lane, one chunk
+                    // ahead (the load of chunk k + 1 is in flight while chunk k is tested), and broadcast through
+                    // a per-warp shared-memory line
+                    float4 nxt = make_float4(FAR, FAR, FAR, 0.f);
+                    if (v0 + lane < ve) nxt = __ldg(xq + v0 + lane);
 #pragma unroll 1
                     for (int j0 = v0; j0 < ve; j0 += P2P_CHUNK) {
+                        const float4 cur = nxt;
+                        if (j0 + P2P_CHUNK + lane < ve) nxt = __ldg(xq + j0 + P2P_CHUNK + lane);
                         while (__any_sync(0xffffffffu, queued() > P2P_QC - 1 - P2P_CHUNK)) round();
                         const int n = min(P2P_CHUNK, ve - j0);
-                        const float4 *sq = xq + j0;
+                        SB[lane] = cur;
+                        __syncwarp();
                         const int ebase = (vslot << P2P_VBITS) + (j0 - v0);
-#pragma unroll 4
+#pragma unroll 8
                         for (int jj = 0; jj < n; ++jj) {
-                            const float4 q = __ldg(sq + jj);
+                            const float4 q = SB[jj];
                             const float rx = tx - q.x, ry = ty - q.y, rz = tz - q.z;
                             if (rx * rx + ry * ry + rz * rz <= rc2m) {
                                 *reinterpret_cast<unsigned short *>(Qb + woff) = (unsigned short)(ebase + jj);
                                 woff = (woff + QSTRIDE) & (QBYTES - 1);
                             }
                         }
+                        __syncwarp();
                     }
                 }
             }
@@ -337,15 +384,27 @@ static long double exp_l(long double x) { return expl(x); }
 cudaError_t se_build_mtab(se_plan *p)
 {
     static_assert(MT_DEG < 24 && MT_EXPDEG < 24, "cheb_fit scratch");
-    double h[MT_SIZE];
-    for (int i = 0; i < MT_NP; ++i) cheb_fit(erfcx_l, 0.25L * i + 0.125L, 0.125L, MT_DEG, h + i * MT_ROW);
-    // the polynomial is evaluated in t itself, not in t / hw: rescale the monomials
-    double e[MT_EXPDEG + 1];
+    double h[MT_SIZE] = {};
+    float *hf = reinterpret_cast<float *>(h + MT_F32);
+    for (int i = 0; i < MT_NP; ++i) {
+        // pieces centred at i/4, half-width 1/8; monomials in v = x - i/4: divide by (1/8)^k (exact)
+        double row[MT_ROW], rowf[MT_ROWF];
+        cheb_fit(erfcx_l, 0.25L * i, 0.125L, MT_DEG, row);
+        cheb_fit(erfcx_l, 0.25L * i, 0.125L, MT_DEGF, rowf);
+        double s = 1.0;
+        for (int k = 0; k <= MT_DEG; ++k) { h[i * MT_ROW + k] = row[k] * s; s *= 8.0; }
+        s = 1.0;
+        for (int k = 0; k <= MT_DEGF; ++k) { hf[i * MT_ROWF + k] = (float)(rowf[k] * s); s *= 8.0; }
+    }
+    // e^t: the polynomial is evaluated in t itself, not in t / hw: rescale the monomials
+    double e[MT_EXPDEG + 1], ec[MT_EXPDEG + 1];
     const long double hw = 0.34657359027997265470861606072908828L * 1.0001L;   // ln2 / 2 and a little slack
     cheb_fit(exp_l, 0.0L, hw, MT_EXPDEG, e);
     long double s = 1;
-    for (int k = 0; k <= MT_EXPDEG; ++k) { h[MT_EXP + k] = (double)(e[k] / s); s *= hw; }
-    cudaError_t err = cudaMalloc(&p->mtab, sizeof(h));
+    for (int k = 0; k <= MT_EXPDEG; ++k) { ec[k] = (double)(e[k] / s); s *= hw; }
+    cudaError_t err = cudaMemcpyToSymbol(c_exp, ec, sizeof(ec));
+    if (err != cudaSuccess) return err;
+    err = cudaMalloc(&p->mtab, sizeof(h));
     if (err != cudaSuccess) return err;
     p->workspace_bytes += sizeof(h);
     return cudaMemcpy(p->mtab, h, sizeof(h), cudaMemcpyHostToDevice);
