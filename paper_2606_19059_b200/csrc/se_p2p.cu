@@ -38,6 +38,9 @@ constexpr int P2P_QC = 128;         // ring-queue slots per lane (power of two),
 constexpr int P2P_CHUNK = 32;       // sources scanned between two queue-room checks
 constexpr int P2P_VBITS = 9;        // a queue entry = (virtual cell << VBITS) | offset: virtual cells of <= 512 sources
 constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV << VBITS) = 2^15)
+#ifndef P2P_TWO
+#define P2P_TWO 1
+#endif
 constexpr int P2P_ZSPAN = 6;        // cells along z a pass may span (<= 29: one lane per source cell)
 
 // ---- function tables (built on the host in long double at plan creation) --------------------------------------
@@ -184,56 +187,51 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     // Mode B (imbalanced: fewer non-empty queues than the fullest one could feed): the 32 lanes evaluate up to 32
     // pairs of the fullest queue together and a butterfly sum hands the result to its owner.  The choice is a pure
     // function of the queue lengths, so the summation order stays deterministic.
+    // one pair: queue entry at byte offset qo of this lane's (or, mode B, the owner's) column -> contribution d
+    auto pair = [&](int qo, Real T0, Real T1, Real T2, Real tcz, Real &d0, Real &d1, Real &d2) {
+        const int e = *reinterpret_cast<const unsigned short *>(Qb + qo);
+        const int j = VT[e >> P2P_VBITS] + (e & ((1 << P2P_VBITS) - 1));
+        const Real *sp = src + 6 * (int64_t)j;
+        Real xj, yj, zj, f0, f1, f2;
+        if (sizeof(Real) == 8) {
+            const double2 p0 = __ldg(reinterpret_cast<const double2 *>(sp));
+            const double2 p1 = __ldg(reinterpret_cast<const double2 *>(sp + 2));
+            const double2 p2 = __ldg(reinterpret_cast<const double2 *>(sp + 4));
+            xj = (Real)p0.x; yj = (Real)p0.y; zj = (Real)p1.x; f0 = (Real)p1.y; f1 = (Real)p2.x; f2 = (Real)p2.y;
+        } else {
+            const float2 p0 = __ldg(reinterpret_cast<const float2 *>(sp));
+            const float2 p1 = __ldg(reinterpret_cast<const float2 *>(sp + 2));
+            const float2 p2 = __ldg(reinterpret_cast<const float2 *>(sp + 4));
+            xj = (Real)p0.x; yj = (Real)p0.y; zj = (Real)p1.x; f0 = (Real)p1.y; f1 = (Real)p2.x; f2 = (Real)p2.y;
+        }
+        // periodic image of the source as this target sees it: the virtual cell's shift (absolute coordinates:
+        // a multiple of L per axis; cell-relative coordinates: the cell offset, in z from the target's own cell)
+        const Real *vs = VS[e >> P2P_VBITS];
+        const Real sx = vs[0], sy = vs[1], sz = vs[2] - tcz;
+        const Real rx = T0 - (xj + sx), ry = T1 - (yj + sy), rz = T2 - (zj + sz);
+        Real r2 = rx * rx + ry * ry + rz * rz;
+        const bool ok = (r2 <= rc2) && (r2 > (Real)0);
+        if (!ok) r2 = (Real)1;
+        Real C1, C2;
+        NearMath<Real>::coeffs(r2, xi, c2, mt, C1, C2);
+        if (!ok) { C1 = (Real)0; C2 = (Real)0; }
+        const Real rf = C2 * (rx * f0 + ry * f1 + rz * f2);
+        d0 = C1 * f0 + rf * rx;
+        d1 = C1 * f1 + rf * ry;
+        d2 = C1 * f2 + rf * rz;
+    };
     auto round = [&]() {
         const int c = queued();
         const unsigned m1 = __ballot_sync(0xffffffffu, c > 0);
         const int cmax = __reduce_max_sync(0xffffffffu, c);
         const int cB = min(cmax, 32);
-        const bool modeB = cB > __popc(m1);                      // warp-uniform
-        Real T0 = X0, T1 = X1, T2 = X2, tcz = czw;
-        int ro = roff, o = lane;
-        bool have = c > 0;
-        if (modeB) {
-            o = __ffs(__ballot_sync(0xffffffffu, c == cmax)) - 1;
-            T0 = __shfl_sync(0xffffffffu, X0, o); T1 = __shfl_sync(0xffffffffu, X1, o); T2 = __shfl_sync(0xffffffffu, X2, o);
-            tcz = __shfl_sync(0xffffffffu, czw, o);
-            ro = (__shfl_sync(0xffffffffu, roff, o) + lane * QSTRIDE) & (QBYTES - 1);
-            have = lane < cB;
-        }
-        Real d0 = 0, d1 = 0, d2 = 0;
-        if (have) {
-            const int e = *reinterpret_cast<const unsigned short *>(Qb + (o - lane) * 2 + ro);
-            const int j = VT[e >> P2P_VBITS] + (e & ((1 << P2P_VBITS) - 1));
-            const Real *sp = src + 6 * (int64_t)j;
-            Real xj, yj, zj, f0, f1, f2;
-            if (sizeof(Real) == 8) {
-                const double2 p0 = __ldg(reinterpret_cast<const double2 *>(sp));
-                const double2 p1 = __ldg(reinterpret_cast<const double2 *>(sp + 2));
-                const double2 p2 = __ldg(reinterpret_cast<const double2 *>(sp + 4));
-                xj = (Real)p0.x; yj = (Real)p0.y; zj = (Real)p1.x; f0 = (Real)p1.y; f1 = (Real)p2.x; f2 = (Real)p2.y;
-            } else {
-                const float2 p0 = __ldg(reinterpret_cast<const float2 *>(sp));
-                const float2 p1 = __ldg(reinterpret_cast<const float2 *>(sp + 2));
-                const float2 p2 = __ldg(reinterpret_cast<const float2 *>(sp + 4));
-                xj = (Real)p0.x; yj = (Real)p0.y; zj = (Real)p1.x; f0 = (Real)p1.y; f1 = (Real)p2.x; f2 = (Real)p2.y;
-            }
-            // periodic image of the source as this target sees it: the virtual cell's shift (absolute coordinates:
-            // a multiple of L per axis; cell-relative coordinates: the cell offset, in z from the target's own cell)
-            const Real *vs = VS[e >> P2P_VBITS];
-            const Real sx = vs[0], sy = vs[1], sz = vs[2] - tcz;
-            const Real rx = T0 - (xj + sx), ry = T1 - (yj + sy), rz = T2 - (zj + sz);
-            Real r2 = rx * rx + ry * ry + rz * rz;
-            const bool ok = (r2 <= rc2) && (r2 > (Real)0);
-            if (!ok) r2 = (Real)1;
-            Real C1, C2;
-            NearMath<Real>::coeffs(r2, xi, c2, mt, C1, C2);
-            if (!ok) { C1 = (Real)0; C2 = (Real)0; }
-            const Real rf = C2 * (rx * f0 + ry * f1 + rz * f2);
-            d0 = C1 * f0 + rf * rx;
-            d1 = C1 * f1 + rf * ry;
-            d2 = C1 * f2 + rf * rz;
-        }
-        if (modeB) {
+        if (cB > __popc(m1)) {                                   // mode B (warp-uniform)
+            const int o = __ffs(__ballot_sync(0xffffffffu, c == cmax)) - 1;
+            const Real T0 = __shfl_sync(0xffffffffu, X0, o), T1 = __shfl_sync(0xffffffffu, X1, o);
+            const Real T2 = __shfl_sync(0xffffffffu, X2, o), tcz = __shfl_sync(0xffffffffu, czw, o);
+            const int ro = (__shfl_sync(0xffffffffu, roff, o) + lane * QSTRIDE) & (QBYTES - 1);
+            Real d0 = 0, d1 = 0, d2 = 0;
+            if (lane < cB) pair((o - lane) * 2 + ro, T0, T1, T2, tcz, d0, d1, d2);
 #pragma unroll
             for (int sh = 16; sh > 0; sh >>= 1) {
                 d0 += __shfl_xor_sync(0xffffffffu, d0, sh);
@@ -241,7 +239,21 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                 d2 += __shfl_xor_sync(0xffffffffu, d2, sh);
             }
             if (lane == o) { a0 += d0; a1 += d1; a2 += d2; roff = (roff + cB * QSTRIDE) & (QBYTES - 1); }
-        } else if (have) {
+        } else if (P2P_TWO && __popc(__ballot_sync(0xffffffffu, c > 1)) * 4 >= __popc(m1) * 3) {
+            // mode A2: most queues hold two pairs: every lane pops up to two of its own, evaluated side by side
+            // (two independent dependency chains per lane); a lane with one pair evaluates it twice and drops one
+            if (c > 0) {
+                Real d0, d1, d2, e0, e1, e2;
+                const int r1 = (roff + QSTRIDE) & (QBYTES - 1);
+                pair(roff, X0, X1, X2, czw, d0, d1, d2);
+                pair(c > 1 ? r1 : roff, X0, X1, X2, czw, e0, e1, e2);
+                a0 += d0; a1 += d1; a2 += d2;
+                if (c > 1) { a0 += e0; a1 += e1; a2 += e2; }
+                roff = c > 1 ? ((r1 + QSTRIDE) & (QBYTES - 1)) : r1;
+            }
+        } else if (c > 0) {                                      // mode A: every lane pops one pair of its own
+            Real d0, d1, d2;
+            pair(roff, X0, X1, X2, czw, d0, d1, d2);
             a0 += d0; a1 += d1; a2 += d2;
             roff = (roff + QSTRIDE) & (QBYTES - 1);
         }
