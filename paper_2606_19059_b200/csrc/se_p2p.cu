@@ -39,7 +39,10 @@ constexpr int P2P_CHUNK = 32;       // sources scanned between two queue-room ch
 constexpr int P2P_VBITS = 9;        // a queue entry = (virtual cell << VBITS) | offset: virtual cells of <= 512 sources
 constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV << VBITS) = 2^15)
 #ifndef P2P_TWO
-#define P2P_TWO 1
+#define P2P_TWO 2
+#endif
+#ifndef P2P_BLOCKS
+#define P2P_BLOCKS 4
 #endif
 constexpr int P2P_ZSPAN = 6;        // cells along z a pass may span (<= 29: one lane per source cell)
 
@@ -144,7 +147,7 @@ template <> struct NearMath<float> {
 };
 
 template <typename Real>
-__global__ void __launch_bounds__(P2P_WARPS * 32, 4)
+__global__ void __launch_bounds__(P2P_WARPS * 32, P2P_BLOCKS)
 k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, const int *__restrict__ cellp,
       const int *__restrict__ cell_start, const double *__restrict__ mtab, Real *__restrict__ uN, float rc2m)
 {
@@ -239,17 +242,21 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                 d2 += __shfl_xor_sync(0xffffffffu, d2, sh);
             }
             if (lane == o) { a0 += d0; a1 += d1; a2 += d2; roff = (roff + cB * QSTRIDE) & (QBYTES - 1); }
-        } else if (P2P_TWO && __popc(__ballot_sync(0xffffffffu, c > 1)) * 4 >= __popc(m1) * 3) {
-            // mode A2: most queues hold two pairs: every lane pops up to two of its own, evaluated side by side
-            // (two independent dependency chains per lane); a lane with one pair evaluates it twice and drops one
+        } else if (P2P_TWO > 1 && __popc(__ballot_sync(0xffffffffu, c >= P2P_TWO)) * 4 >= __popc(m1) * 3) {
+            // mode A2: most queues hold P2P_TWO pairs: every lane pops up to that many of its own, evaluated side
+            // by side (independent dependency chains); a lane with fewer re-evaluates its last one and drops it
             if (c > 0) {
-                Real d0, d1, d2, e0, e1, e2;
-                const int r1 = (roff + QSTRIDE) & (QBYTES - 1);
-                pair(roff, X0, X1, X2, czw, d0, d1, d2);
-                pair(c > 1 ? r1 : roff, X0, X1, X2, czw, e0, e1, e2);
-                a0 += d0; a1 += d1; a2 += d2;
-                if (c > 1) { a0 += e0; a1 += e1; a2 += e2; }
-                roff = c > 1 ? ((r1 + QSTRIDE) & (QBYTES - 1)) : r1;
+                Real d[P2P_TWO][3];
+                int ro = roff;
+#pragma unroll
+                for (int k = 0; k < P2P_TWO; ++k) {
+                    pair(ro, X0, X1, X2, czw, d[k][0], d[k][1], d[k][2]);
+                    if (k + 1 < c) ro = (ro + QSTRIDE) & (QBYTES - 1);
+                }
+#pragma unroll
+                for (int k = 0; k < P2P_TWO; ++k)
+                    if (k < c) { a0 += d[k][0]; a1 += d[k][1]; a2 += d[k][2]; }
+                roff = (roff + min(c, P2P_TWO) * QSTRIDE) & (QBYTES - 1);
             }
         } else if (c > 0) {                                      // mode A: every lane pops one pair of its own
             Real d0, d1, d2;
