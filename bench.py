@@ -273,7 +273,8 @@ def run_b200(args):
             continue
         if w["bound"] == "alu":
             ach = w["work"] / (ms * 1e-3) / 1e12
-            peak = ALU_PEAK_TFLOPS[c.precision]
+            # fp32 plans grid on the FP64 tensor path too (double records and accumulators, float grid)
+            peak = ALU_PEAK_TFLOPS["fp64" if info.grid_mode == 2 else c.precision]
         else:
             ach = w["work"] / (ms * 1e-3) / 1e9
             peak = hbm_peak
@@ -284,7 +285,7 @@ def run_b200(args):
     roof = dict(per_stage[dom])
     roof["kernel"] = {"p2g": "k_p2g (K3)", "g2p": "k_g2p (K5)", "scale": "k_scale (K4)", "sort": "K1", "sum": "K6"}[dom]
     roof["peak_source"] = ("unit counts x clock: 148 SM x %d FMA/clk x 2 x 1.965 GHz (DESIGN.md)" %
-                           (64 if c.precision == "fp64" else 128)) if roof["bound"] == "alu" else hbm_src
+                           (64 if (c.precision == "fp64" or info.grid_mode == 2) else 128)) if roof["bound"] == "alu" else hbm_src
     # P2P: plain-ALU kernel whose work is data dependent -- reported as in-range pairs/s
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

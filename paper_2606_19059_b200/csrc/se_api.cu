@@ -150,6 +150,7 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
         const int zb = (M + SE_MMA_ZBIN - 1) / SE_MMA_ZBIN;
         if (se_mma_supported(P, (int)prec) && (double)M * zb * M < 5.0e8 && !want_tile && !want_sweep) {
             g.grid_mode = 2;
+            g.ring = se_mma_ring(P);
             g.nbin = zb;
             g.nbins_total = M * zb * M;
             const int BY = 4 * SE_MMA_NWY, BZ = 4 * SE_MMA_NWZ;
@@ -234,12 +235,12 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     A.get(&p->perm_grid, N * sizeof(int));
     A.get(&p->inv_grid, N * sizeof(int));
     A.get(&p->anchor, N * sizeof(short4));
-    A.get(&p->wtab, g.grid_mode == 2 ? (size_t)N * SE_MMA_RECS(P) * rb : (size_t)N * 3 * P * rb);
-    if (g.grid_mode == 2) A.get(&p->recg, (size_t)N * SE_MMA_RECG(P) * rb);
+    A.get(&p->wtab, g.grid_mode == 2 ? (size_t)N * SE_MMA_RECS(g.ring) * 8 : (size_t)N * 3 * P * rb);
+    if (g.grid_mode == 2) A.get(&p->recg, (size_t)N * SE_MMA_RECG(P) * 8);
     A.get(&p->fs_grid, N * 3 * rb);
     A.get(&p->uF, std::max((size_t)N * 3 * rb, (size_t)N * sizeof(int)));
     if (g.grid_mode == 1) A.get(&p->uFpart, (size_t)N * SE_NSLOT * 3 * rb);
-    if (g.grid_mode == 2) A.get(&p->uFpart, (size_t)N * se_mma_slots(P) * 3 * rb);
+    if (g.grid_mode == 2) A.get(&p->uFpart, (size_t)N * se_mma_slots(P) * 3 * 8);
     A.get(&p->grid, 3 * M3 * rb);
     A.get(&p->spec, 3 * nm * 2 * rb);
     A.get(&p->ktab, 2 * (size_t)M * rb);

@@ -29,8 +29,9 @@ constexpr int SE_NSLOT = SE_NSLOT_B * SE_NSLOT_C;
 constexpr int SE_GSTEPS_MAX = 16;
 // FP64 tensor-core gridding kernels (se_mma.cu): particles sorted by (anchor plane, anchor_z / ZBIN, anchor_y);
 // a block of NWY x NWZ consumer warps (+ the producer warpgroup) owns 4 NWY x 4 NWZ (y, z) columns.  K1 writes two
-// 16-byte aligned records per particle in sorted order (anchors as two int32 in one double slot):
-//   spread record, SE_MMA_RECS(P) doubles: c_w f_x Wx[P] | c_w f_y Wx[P] | c_w f_z Wx[P] | Wy[P] | Wz[P] | (a_y, a_z) | pad
+// 16-byte aligned records per particle in sorted order (always double, also for fp32 plans; anchors as two int32
+// in one double slot; R = P rounded up to a multiple of 8, rows zero beyond P):
+//   spread record, SE_MMA_RECS(R) doubles: c_w f_x Wx[R] | c_w f_y Wx[R] | c_w f_z Wx[R] | Wy[R] | Wz[R] | (a_y, a_z) | pad
 //   gather record, SE_MMA_RECG(P) doubles: Wx[P] | Wy[P] | Wz[P] | (a_y, a_z) | pad
 // (sizes = 24 mod 32 four-byte words, so that consecutive records start in different shared-memory bank octets)
 constexpr int SE_MMA_ZBIN = 8;
@@ -48,6 +49,7 @@ struct SeGeom {
     int nbins_total;    // nbin^3 (tile mode), M * nbin^2 (sweep mode), M * nbin * M (mma mode)
     int nchunk;         // sweep / mma mode: chunks along x (P2G)
     int nchunk_g2p;     // mma mode: chunks along x (G2P)
+    int ring;           // mma mode: row stride of the spread records = P rounded up to a multiple of 8
     int gsteps;         // sweep mode: planes whose candidates are enumerated together
     int rel_coords;     // 1: near-sorted positions are cell-relative (fp32 path)
     double L, xi, rc;
@@ -118,3 +120,4 @@ cudaError_t se_launch_mma_p2g(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_mma_g2p(se_plan *p, cudaStream_t s);
 bool se_mma_supported(int P, int precision);
 int se_mma_slots(int P);
+int se_mma_ring(int P);

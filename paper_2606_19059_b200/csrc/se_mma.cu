@@ -1,5 +1,6 @@
 // K3 P2G (eq. (2.5)) and K5 G2P (eq. (2.7)) in FP64 as an x-SWEEP whose inner
-// product runs on the FP64 tensor-core instruction (mma.sync m8n8k4 f64 -> DMMA), for P = 16 and 24.
+// product runs on the FP64 tensor-core instruction (mma.sync m8n8k4 f64 -> DMMA), for P = 16 and 24 in fp64
+// plans and P = 12 in fp32 plans (float grid, double records and accumulators; P2G on a ring of 16 planes).
 //
 // Why.  With a Gaussian window at P = 24 both gridding steps are FP64-arithmetic bound: 3 P^3 = 41,472
 // FMA per particle against ~1 KB of compulsory traffic.  On B200 DFMA and DMMA
@@ -106,7 +107,7 @@ struct Cfg {
     static constexpr int NST = SPREAD ? SE_EXP_NSTS : SE_EXP_NST;       // stages
     static constexpr int GRP = SPREAD ? 4 : 8;                 // candidates per K-group (P2G: k = 4; G2P: n = 8)
     static constexpr int NSB = (P + BY - 2) / BY + 2, NSC = (P + BZ - 2) / BZ + 2;   // block tiles a window can meet
-    static_assert(P % 8 == 0 && (REC % 2) == 0 && NCW % 4 == 0 && CAP % GRP == 0, "layout");
+    static_assert(P % 4 == 0 && (!SPREAD || P % 8 == 0) && (REC % 2) == 0 && NCW % 4 == 0 && CAP % GRP == 0, "layout");
 };
 // registers per thread after the warpgroups re-split the register file (setmaxnreg): per scheduler
 // 3 consumer warps + 1 producer-group warp share 512 registers per lane
@@ -141,11 +142,25 @@ __device__ __forceinline__ int modM(int v, int M) { v %= M; return v < 0 ? v + M
 // does the window [0, P) (indices mod M) meet columns T0 .. T0 + n - 1, given l0 = (T0 - anchor) mod M ?
 __device__ __forceinline__ bool meets(int l0, int n, int M, int P) { return n > 0 && (l0 < P || l0 + n - 1 >= M); }
 
-template <int P, bool SPREAD>
+// grid values <-> double pairs (the grid is stored in the plan's precision; all arithmetic here is double)
+template <typename GR> struct GV;
+template <> struct GV<double> {
+    static __device__ __forceinline__ void st2(double *p, double a, double b) { *reinterpret_cast<double2 *>(p) = make_double2(a, b); }
+    static __device__ __forceinline__ double2 ld2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
+};
+template <> struct GV<float> {
+    static __device__ __forceinline__ void st2(float *p, double a, double b) { *reinterpret_cast<float2 *>(p) = make_float2((float)a, (float)b); }
+    static __device__ __forceinline__ double2 ld2(const float *p) { const float2 v = *reinterpret_cast<const float2 *>(p); return make_double2((double)v.x, (double)v.y); }
+};
+
+// P: ring size = row stride of the records (a multiple of 8 for P2G, of 4 for G2P); W <= P: window support (the
+// record rows are zero beyond W); GR: grid storage type.
+template <int P, bool SPREAD, int W, typename GR>
 __global__ void __launch_bounds__((NWY * NWZ + 4) * 32, 1)
-k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_start, double *__restrict__ grid,
+k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_start, GR *__restrict__ grid,
       double *__restrict__ uFpart)
 {
+    static_assert(W <= P && (SPREAD || W == P), "window / ring");
     typedef Cfg<P, SPREAD> C;
     constexpr int NCW = C::NCW, BY = C::BY, BZ = C::BZ, MT = C::MT, REC = C::REC, NST = C::NST, GRP = C::GRP;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -165,7 +180,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
     // whole periodic axis: then the sweep starts at plane 0 and the P - 1 planes left in the ring at the end are the
     // wrapped contributions to planes 0 .. P - 2, which the same thread adds to what it wrote there (no warm-up).
     const bool wrap_add = SPREAD && nchunk == 1;
-    const int s_begin = (SPREAD && !wrap_add) ? X0 - (P - 1) : X0, s_end = X0 + CLen;
+    const int s_begin = (SPREAD && !wrap_add) ? X0 - (W - 1) : X0, s_end = X0 + CLen;
 
     for (int e = tid; e < NST * REC; e += C::NT) S.st[e / REC].rec[CAP][e % REC] = 0.0;
     if (tid == 0)
@@ -192,7 +207,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                     const int a = it / 3, c = it - 3 * a;
                     const int2 an = *reinterpret_cast<const int2 *>(&T.rec[a][C::OM]);
                     const int ly = modM(Y0 - an.x, M), lz = modM(Z0 - an.y, M);
-                    const bool hit = meets(ly, min(BY, M - Y0), M, P) && meets(lz, min(BZ, M - Z0), M, P);
+                    const bool hit = meets(ly, min(BY, M - Y0), M, W) && meets(lz, min(BZ, M - Z0), M, W);
                     const int rb = modM(ty - an.x / BY, ntY), rc = modM(tz - an.y / BZ, ntZ);
                     if (hit && rb < C::NSB && rc < C::NSC) {
                         double sum = 0.0;
@@ -207,14 +222,14 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
         }
         // =================================== PRODUCER ==========================================================
         // candidate rows / z-bins of this block tile (anchors): cyclic [Y0-(P-1), Y0+BY-1], [Z0-(P-1), Z0+BZ-1]
-        const int leny = min(BY + P - 1, M);
-        const int ylo = modM(Y0 - (P - 1), M);
+        const int leny = min(BY + W - 1, M);
+        const int ylo = modM(Y0 - (W - 1), M);
         int zb0, nzbins;
         {
-            const int len = BZ + P - 1;
+            const int len = BZ + W - 1;
             if (len + ZBW > M) { zb0 = 0; nzbins = nzb; }
             else {
-                const int lo = modM(Z0 - (P - 1), M), hi = modM(Z0 + BZ - 1, M);
+                const int lo = modM(Z0 - (W - 1), M), hi = modM(Z0 + BZ - 1, M);
                 zb0 = lo / ZBW;
                 nzbins = hi / ZBW - zb0; if (nzbins < 0) nzbins += nzb;
                 nzbins += 1;
@@ -328,7 +343,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                 const int2 an = *reinterpret_cast<const int2 *>(&T.rec[a][C::OM]);
                 ly = Yw - an.x; if (ly < 0) ly += M;
                 lz = Zw - an.y; if (lz < 0) lz += M;
-                hit = meets(ly, nyw, M, P) && meets(lz, nzw, M, P);
+                hit = meets(ly, nyw, M, W) && meets(lz, nzw, M, W);
                 if (!SPREAD) T.hit[a][warp] = (unsigned char)hit;
             }
             const unsigned m = __ballot_sync(0xffffffffu, hit);
@@ -343,7 +358,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
     // window value W[(l0 + i) mod M] of a staged record row, zero outside the support (l0 + i < 2 M)
     auto wrec = [&](const double *w, int l) -> double {
         if (l >= M) l -= M;
-        return l < P ? w[l] : 0.0;
+        return l < W ? w[l] : 0.0;
     };
 
     if constexpr (SPREAD) {
@@ -369,8 +384,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
                     if (valid && 2 * j + cyl < nyw)
-                        *reinterpret_cast<double2 *>(&grid[c * M3 + off + (size_t)(2 * j) * M]) =
-                            make_double2(acc[mt][c][j][0], acc[mt][c][j][1]);
+                        GV<GR>::st2(&grid[c * M3 + off + (size_t)(2 * j) * M], acc[mt][c][j][0], acc[mt][c][j][1]);
                     acc[mt][c][j][0] = acc[mt][c][j][1] = 0.0;
                 }
         };
@@ -405,9 +419,8 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                         for (int c = 0; c < 3; ++c)
 #pragma unroll
                             for (int j = 0; j < 2; ++j)
-                                if (cz_ok && t < P - 1 && 2 * j + cyl < nyw)
-                                    o[mt][c][j] = *reinterpret_cast<const double2 *>(
-                                        &grid[c * M3 + (size_t)t * MM + colS + (size_t)(2 * j) * M]);
+                                if (cz_ok && t < W - 1 && 2 * j + cyl < nyw)
+                                    o[mt][c][j] = GV<GR>::ld2(&grid[c * M3 + (size_t)t * MM + colS + (size_t)(2 * j) * M]);
                     }
 #pragma unroll
                     for (int mt = 0; mt < MT; ++mt)
@@ -415,10 +428,9 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                         for (int c = 0; c < 3; ++c)
 #pragma unroll
                             for (int j = 0; j < 2; ++j)
-                                if (cz_ok && tt[mt] < P - 1 && 2 * j + cyl < nyw)
-                                    *reinterpret_cast<double2 *>(
-                                        &grid[c * M3 + (size_t)tt[mt] * MM + colS + (size_t)(2 * j) * M]) =
-                                        make_double2(o[mt][c][j].x + acc[mt][c][j][0], o[mt][c][j].y + acc[mt][c][j][1]);
+                                if (cz_ok && tt[mt] < W - 1 && 2 * j + cyl < nyw)
+                                    GV<GR>::st2(&grid[c * M3 + (size_t)tt[mt] * MM + colS + (size_t)(2 * j) * M],
+                                                o[mt][c][j].x + acc[mt][c][j][0], o[mt][c][j].y + acc[mt][c][j][1]);
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&S.empty[sg]);
@@ -490,7 +502,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
 #ifdef SE_EXP_NORING
                     pre[c][j] = (double)(XM + c + j);
 #else
-                    pre[c][j] = (gz_ok && 2 * j + gyl < nyw) ? __ldg(&grid[c * M3 + off + (size_t)(2 * j) * M]) : 0.0;
+                    pre[c][j] = (gz_ok && 2 * j + gyl < nyw) ? (double)__ldg(&grid[c * M3 + off + (size_t)(2 * j) * M]) : 0.0;
 #endif
         };
         auto commit_ks = [&](auto ksc) {
@@ -578,9 +590,9 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
 }
 
 // u^F (grid-sorted order) = fixed-order sum of the slots the particle's window actually meets
-template <int P>
+template <int P, typename GR>
 __global__ void k_reduce_slots(SeGeom g, const short4 *__restrict__ anchor, const double *__restrict__ part,
-                               double *__restrict__ uF)
+                               GR *__restrict__ uF)
 {
     typedef Cfg<P, false> C;
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -599,10 +611,10 @@ __global__ void k_reduce_slots(SeGeom g, const short4 *__restrict__ anchor, cons
             s0 += q[0]; s1 += q[1]; s2 += q[2];
         }
     }
-    uF[3 * i + 0] = s0; uF[3 * i + 1] = s1; uF[3 * i + 2] = s2;
+    uF[3 * i + 0] = (GR)s0; uF[3 * i + 1] = (GR)s1; uF[3 * i + 2] = (GR)s2;
 }
 
-template <int P, bool SPREAD>
+template <int P, bool SPREAD, int W, typename GR>
 cudaError_t launch(se_plan *p, cudaStream_t s)
 {
     typedef Cfg<P, SPREAD> C;
@@ -610,7 +622,7 @@ cudaError_t launch(se_plan *p, cudaStream_t s)
     static bool attr_set = false;
     constexpr size_t smem = sizeof(Smem<P, SPREAD>);
     static_assert(smem <= 227 * 1024, "shared memory per block");
-    auto kern = k_mma<P, SPREAD>;
+    auto kern = k_mma<P, SPREAD, W, GR>;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -619,11 +631,11 @@ cudaError_t launch(se_plan *p, cudaStream_t s)
     const int ntY = (g.M + C::BY - 1) / C::BY, ntZ = (g.M + C::BZ - 1) / C::BZ;
     const int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
     kern<<<(unsigned)(nchunk * ntY * ntZ), C::NT, smem, s>>>(g, (const double *)(SPREAD ? p->wtab : p->recg), p->bin_start,
-                                                             (double *)p->grid, (double *)p->uFpart);
+                                                             (GR *)p->grid, (double *)p->uFpart);
     p->launches += 1;
     if (!SPREAD) {
-        k_reduce_slots<P><<<(unsigned)((g.N + 255) / 256), 256, 0, s>>>(g, p->anchor, (const double *)p->uFpart,
-                                                                        (double *)p->uF);
+        k_reduce_slots<P, GR><<<(unsigned)((g.N + 255) / 256), 256, 0, s>>>(g, p->anchor, (const double *)p->uFpart,
+                                                                            (GR *)p->uF);
         p->launches += 1;
     }
     return cudaGetLastError();
@@ -632,16 +644,32 @@ cudaError_t launch(se_plan *p, cudaStream_t s)
 template <bool SPREAD>
 cudaError_t dispatch(se_plan *p, cudaStream_t s)
 {
-    switch (p->g.P) {
-    case 24: return launch<24, SPREAD>(p, s);
-    case 16: return launch<16, SPREAD>(p, s);
-    default: return cudaErrorInvalidValue;
+    if (p->precision == SE_FP64) {
+        switch (p->g.P) {
+        case 24: return launch<24, SPREAD, 24, double>(p, s);
+        case 16: return launch<16, SPREAD, 16, double>(p, s);
+        default: return cudaErrorInvalidValue;
+        }
     }
+    // fp32 plans: float grid, double records and accumulation; P = 12 spreads on a ring of 16 planes
+    if (p->g.P == 12) return launch<SPREAD ? 16 : 12, SPREAD, 12, float>(p, s);
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace
 
-bool se_mma_supported(int P, int precision) { return precision == SE_FP64 && (P == 24 || P == 16); }
-int se_mma_slots(int P) { return P == 24 ? Cfg<24, false>::NSB * Cfg<24, false>::NSC : Cfg<16, false>::NSB * Cfg<16, false>::NSC; }
+bool se_mma_supported(int P, int precision)
+{
+    return precision == SE_FP64 ? (P == 24 || P == 16) : P == 12;
+}
+int se_mma_ring(int P) { return (P + 7) / 8 * 8; }     // row stride of the spread records
+int se_mma_slots(int P)
+{
+    switch (P) {
+    case 24: return Cfg<24, false>::NSB * Cfg<24, false>::NSC;
+    case 16: return Cfg<16, false>::NSB * Cfg<16, false>::NSC;
+    default: return Cfg<12, false>::NSB * Cfg<12, false>::NSC;
+    }
+}
 cudaError_t se_launch_mma_p2g(se_plan *p, cudaStream_t s) { return dispatch<true>(p, s); }
 cudaError_t se_launch_mma_g2p(se_plan *p, cudaStream_t s) { return dispatch<false>(p, s); }

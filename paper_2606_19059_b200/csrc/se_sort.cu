@@ -209,10 +209,10 @@ __global__ void k_gather_near(SeGeom g, const Real *__restrict__ x, const Real *
 // = exp(-a t_l^2), t_l = (anchor + l) h - x  (reading S11).  Always evaluated in
 // double and rounded once to Real.  In mma mode (fp64) the values go into the per-particle spread and
 // gather records of se_mma.cu (layout in se_common.cuh) instead of the plain [N][3][P] table.
-template <typename Real>
+template <typename Real, typename Rec>
 __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *__restrict__ f,
                               const int *__restrict__ perm, short4 *__restrict__ anchor,
-                              Real *__restrict__ wtab, Real *__restrict__ recg, Real *__restrict__ fs)
+                              Rec *__restrict__ wtab, Rec *__restrict__ recg, Real *__restrict__ fs)
 {
     int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int P = g.P, P3 = 3 * P;
@@ -224,16 +224,23 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
     double frac;
     int i0 = grid_base1(wrap1((double)x[3 * (int64_t)i + d], g.L), g, frac);
     double u = (double)(l - (P / 2 - 1)) - frac;
-    const Real w = (Real)exp(-g.beta * u * u);
+    const Rec w = (Rec)exp(-g.beta * u * u);
     const bool recs = g.grid_mode == 2;
-    Real *rs = wtab + p * SE_MMA_RECS(P), *rg = recg + p * SE_MMA_RECG(P);
+    const int R = g.ring;
+    Rec *rs = wtab + p * SE_MMA_RECS(R), *rg = recg + p * SE_MMA_RECG(P);
     if (recs) {
+        const bool padz = l < R - P;                             // this thread also clears row entry P + l
         rg[e] = w;
         if (d == 0) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) rs[c * P + l] = (Real)g.cw * f[3 * (int64_t)i + c] * w;   // c_w of eq. (2.5) folded in
-        } else
-            rs[(d + 2) * P + l] = w;
+            for (int c = 0; c < 3; ++c) {
+                rs[c * R + l] = (Rec)g.cw * (Rec)f[3 * (int64_t)i + c] * w;   // c_w of eq. (2.5) folded in
+                if (padz) rs[c * R + P + l] = (Rec)0;
+            }
+        } else {
+            rs[(d + 2) * R + l] = w;
+            if (padz) rs[(d + 2) * R + P + l] = (Rec)0;
+        }
     } else
         wtab[t] = w;
     if (l == 0) {
@@ -244,7 +251,7 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
         if (d == 0) ap[3] = 0;
         fs[3 * p + d] = f[3 * (int64_t)i + d];
         if (recs && d > 0) {
-            reinterpret_cast<int *>(&rs[5 * P])[d - 1] = a;
+            reinterpret_cast<int *>(&rs[5 * R])[d - 1] = a;
             reinterpret_cast<int *>(&rg[P3])[d - 1] = a;
         }
     }
@@ -290,8 +297,12 @@ cudaError_t sort_impl(se_plan *p, const void *xv, const void *fv, cudaStream_t s
     k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, p->perm_near, p->cell_of, (Real *)p->src_near,
                                            (float4 *)p->xq, p->cell_sorted);
     int64_t nt = g.N * 3 * g.P;
-    k_gather_grid<Real><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(g, x, f, p->perm_grid, p->anchor,
-                                                                  (Real *)p->wtab, (Real *)p->recg, (Real *)p->fs_grid);
+    if (g.grid_mode == 2)                                      // records are double for every plan precision
+        k_gather_grid<Real, double><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(
+            g, x, f, p->perm_grid, p->anchor, (double *)p->wtab, (double *)p->recg, (Real *)p->fs_grid);
+    else
+        k_gather_grid<Real, Real><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(
+            g, x, f, p->perm_grid, p->anchor, (Real *)p->wtab, (Real *)p->recg, (Real *)p->fs_grid);
     p->launches += 8;
     return cudaGetLastError();
 }
