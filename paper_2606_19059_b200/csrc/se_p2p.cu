@@ -41,6 +41,9 @@ constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV 
 #ifndef P2P_TWO
 #define P2P_TWO 2
 #endif
+#ifndef P2P_FU
+#define P2P_FU 8
+#endif
 #ifndef P2P_BLOCKS
 #define P2P_BLOCKS 4
 #endif
@@ -179,7 +182,7 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     const int64_t ic = valid ? i : g.N - 1;
     const float4 qi = xq[ic];
     const int pci = cellp[ic];
-    const int cx = pci >> 20, cy = (pci >> 10) & 1023, cz = pci & 1023;
+    const int cz = pci & 1023;
     const Real X0 = src[6 * ic + 0], X1 = src[6 * ic + 1], X2 = src[6 * ic + 2];
     Real a0 = 0, a1 = 0, a2 = 0;
     const Real czw = g.rel_coords ? (Real)cz * wc : (Real)0;    // z offset of this target's cell (cell-relative plans)
@@ -335,19 +338,27 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
 #pragma unroll 1
                     for (int j0 = v0; j0 < ve; j0 += P2P_CHUNK) {
                         const float4 cur = nxt;
+                        nxt = make_float4(FAR, FAR, FAR, 0.f);
                         if (j0 + P2P_CHUNK + lane < ve) nxt = __ldg(xq + j0 + P2P_CHUNK + lane);
                         while (__any_sync(0xffffffffu, queued() > P2P_QC - 1 - P2P_CHUNK)) round();
                         const int n = min(P2P_CHUNK, ve - j0);
-                        SB[lane] = cur;
+                        SB[lane] = cur;                          // entries past the cell's end are FAR: never in range
                         __syncwarp();
                         const int ebase = (vslot << P2P_VBITS) + (j0 - v0);
-#pragma unroll 8
-                        for (int jj = 0; jj < n; ++jj) {
-                            const float4 q = SB[jj];
-                            const float rx = tx - q.x, ry = ty - q.y, rz = tz - q.z;
-                            if (rx * rx + ry * ry + rz * rz <= rc2m) {
-                                *reinterpret_cast<unsigned short *>(Qb + woff) = (unsigned short)(ebase + jj);
-                                woff = (woff + QSTRIDE) & (QBYTES - 1);
+                        // groups of P2P_FU sources: all broadcast loads of a group first (the queue stores that
+                        // follow are shared-memory stores the compiler must order against later loads)
+#pragma unroll 1
+                        for (int jb = 0; jb < n; jb += P2P_FU) {
+                            float4 q[P2P_FU];
+#pragma unroll
+                            for (int u = 0; u < P2P_FU; ++u) q[u] = SB[jb + u];
+#pragma unroll
+                            for (int u = 0; u < P2P_FU; ++u) {
+                                const float rx = tx - q[u].x, ry = ty - q[u].y, rz = tz - q[u].z;
+                                if (rx * rx + ry * ry + rz * rz <= rc2m) {
+                                    *reinterpret_cast<unsigned short *>(Qb + woff) = (unsigned short)(ebase + jb + u);
+                                    woff = (woff + QSTRIDE) & (QBYTES - 1);
+                                }
                             }
                         }
                         __syncwarp();
