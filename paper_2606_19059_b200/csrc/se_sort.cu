@@ -214,45 +214,56 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
                               const int *__restrict__ perm, short4 *__restrict__ anchor,
                               Rec *__restrict__ wtab, Rec *__restrict__ recg, Real *__restrict__ fs)
 {
-    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // LP = 16 or 32 lanes per particle: lane d < 3 of the group wraps coordinate d and finds its base index once,
+    // the group shares them by shuffle, then lane l < P evaluates window value l of each dimension and the rows
+    // are written with consecutive lanes on consecutive addresses
     const int P = g.P, P3 = 3 * P;
-    int64_t p = t / P3;
-    if (p >= g.N) return;
-    int e = (int)(t - p * P3);
-    int d = e / P, l = e - d * P;
-    int i = perm[p];
-    double frac;
-    int i0 = grid_base1(wrap1((double)x[3 * (int64_t)i + d], g.L), g, frac);
-    double u = (double)(l - (P / 2 - 1)) - frac;
-    const Rec w = (Rec)exp(-g.beta * u * u);
+    const int LP = P <= 16 ? 16 : 32;
+    const int lane = threadIdx.x & 31, l = lane & (LP - 1), gbase = lane & ~(LP - 1);
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t p = warp * (32 / LP) + (lane / LP);
+    const bool live = p < g.N;
+    const int64_t pc = live ? p : g.N - 1;
+    const int i = perm[pc];
+    double frac = 0.0;
+    int i0 = 0;
+    Real fd = (Real)0;
+    if (l < 3) {
+        i0 = grid_base1(wrap1((double)x[3 * (int64_t)i + l], g.L), g, frac);
+        fd = f[3 * (int64_t)i + l];
+    }
     const bool recs = g.grid_mode == 2;
-    const int R = g.ring;
-    Rec *rs = wtab + p * SE_MMA_RECS(R), *rg = recg + p * SE_MMA_RECG(P);
-    if (recs) {
-        const bool padz = l < R - P;                             // this thread also clears row entry P + l
-        rg[e] = w;
-        if (d == 0) {
+    const int R = recs ? g.ring : P;
+    Rec *rs = wtab + pc * SE_MMA_RECS(R), *rg = recg + pc * SE_MMA_RECG(P);
+    Rec cf[3];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                rs[c * R + l] = (Rec)g.cw * (Rec)f[3 * (int64_t)i + c] * w;   // c_w of eq. (2.5) folded in
-                if (padz) rs[c * R + P + l] = (Rec)0;
-            }
-        } else {
-            rs[(d + 2) * R + l] = w;
-            if (padz) rs[(d + 2) * R + P + l] = (Rec)0;
-        }
-    } else
-        wtab[t] = w;
-    if (l == 0) {
+    for (int c = 0; c < 3; ++c) cf[c] = (Rec)g.cw * (Rec)__shfl_sync(0xffffffffu, fd, gbase + c);   // c_w of eq. (2.5) folded in
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const double fr = __shfl_sync(0xffffffffu, frac, gbase + d);
+        if (!live || l >= R) continue;
+        const double u = (double)(l - (P / 2 - 1)) - fr;
+        const Rec w = l < P ? (Rec)exp(-g.beta * u * u) : (Rec)0;       // rows are zero beyond the window
+        if (recs) {
+            if (l < P) rg[d * P + l] = w;
+            if (d == 0) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) rs[c * R + l] = cf[c] * w;
+            } else
+                rs[(d + 2) * R + l] = w;
+        } else if (l < P)
+            wtab[pc * P3 + d * P + l] = w;
+    }
+    if (live && l < 3) {
         int a = i0 - (P / 2 - 1);
         if (a < 0) a += g.M;
         short *ap = reinterpret_cast<short *>(&anchor[p]);
-        ap[d] = (short)a;
-        if (d == 0) ap[3] = 0;
-        fs[3 * p + d] = f[3 * (int64_t)i + d];
-        if (recs && d > 0) {
-            reinterpret_cast<int *>(&rs[5 * R])[d - 1] = a;
-            reinterpret_cast<int *>(&rg[P3])[d - 1] = a;
+        ap[l] = (short)a;
+        if (l == 0) ap[3] = 0;
+        fs[3 * p + l] = fd;
+        if (recs && l > 0) {
+            reinterpret_cast<int *>(&rs[5 * R])[l - 1] = a;
+            reinterpret_cast<int *>(&rg[P3])[l - 1] = a;
         }
     }
 }
@@ -296,7 +307,7 @@ cudaError_t sort_impl(se_plan *p, const void *xv, const void *fv, cudaStream_t s
     k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, p->bin_of, p->bin_start, tmp_grid, p->perm_grid, p->inv_grid);
     k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, p->perm_near, p->cell_of, (Real *)p->src_near,
                                            (float4 *)p->xq, p->cell_sorted);
-    int64_t nt = g.N * 3 * g.P;
+    int64_t nt = (g.N + (g.P <= 16 ? 1 : 0)) / (g.P <= 16 ? 2 : 1) * 32;   // 16 or 32 lanes per particle
     if (g.grid_mode == 2)                                      // records are double for every plan precision
         k_gather_grid<Real, double><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(
             g, x, f, p->perm_grid, p->anchor, (double *)p->wtab, (double *)p->recg, (Real *)p->fs_grid);
