@@ -38,6 +38,11 @@ void free_all(se_plan *p)
     if (p->fft_ok & 1) cufftDestroy(p->fft_fwd);
     if (p->fft_ok & 2) cufftDestroy(p->fft_inv);
     if (p->ev_ok) for (int i = 0; i <= SE_NSTAGES; ++i) cudaEventDestroy(p->ev[i]);
+    if (p->side_ok) {
+        cudaEventDestroy(p->ev_fork); cudaEventDestroy(p->ev_join);
+        cudaEventDestroy(p->ev_p2p[0]); cudaEventDestroy(p->ev_p2p[1]);
+        cudaStreamDestroy(p->side);
+    }
     delete p;
 }
 
@@ -271,6 +276,22 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     for (int i = 0; i <= SE_NSTAGES; ++i)
         if (cudaEventCreate(&p->ev[i]) != cudaSuccess) { free_all(p); return SE_ECUDA; }
     p->ev_ok = 1;
+    {
+        // side stream for K2 at the lowest priority: the grid chain on the caller's stream gets the SMs first
+        int lo = 0, hi = 0;
+        cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        const char *e = std::getenv("SE_OVERLAP");
+        p->overlap = e && std::atoi(e) != 0;             // off by default: measured gain <= 0.5 %
+        if (cudaStreamCreateWithPriority(&p->side, cudaStreamNonBlocking, lo) != cudaSuccess ||
+            cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreate(&p->ev_p2p[0]) != cudaSuccess || cudaEventCreate(&p->ev_p2p[1]) != cudaSuccess) {
+            cudaGetLastError();
+            free_all(p);
+            return SE_ECUDA;
+        }
+        p->side_ok = 1;
+    }
     *out = p;
     return SE_OK;
 }
@@ -307,10 +328,28 @@ se_status se_eval(se_plan *p, const void *x, const void *f, void *u, void *strea
     p->launches = 0;
     p->ev_recorded = 0;
     const bool prof = p->profiling != 0;
+    const bool fork = p->overlap != 0;
     if (prof && cudaEventRecord(p->ev[0], s) != cudaSuccess) return SE_ECUDA;
     for (int st = 0; st < SE_NSTAGES; ++st) {
-        se_status r = run_stage(p, st, x, f, u, s);
-        if (r != SE_OK) return r;
+        if (fork && st == SE_STAGE_P2P) {
+            // deferred: launched on the side stream once K3 has been queued (below)
+        } else if (fork && st == SE_STAGE_SUM) {
+            if (cudaStreamWaitEvent(s, p->ev_join, 0) != cudaSuccess) return SE_ECUDA;
+            se_status r = run_stage(p, st, x, f, u, s);
+            if (r != SE_OK) return r;
+        } else {
+            se_status r = run_stage(p, st, x, f, u, s);
+            if (r != SE_OK) return r;
+        }
+        if (fork && st == SE_STAGE_P2G) {
+            if (cudaEventRecord(p->ev_fork, s) != cudaSuccess) return SE_ECUDA;
+            if (cudaStreamWaitEvent(p->side, p->ev_fork, 0) != cudaSuccess) return SE_ECUDA;
+            if (prof && cudaEventRecord(p->ev_p2p[0], p->side) != cudaSuccess) return SE_ECUDA;
+            se_status r = run_stage(p, SE_STAGE_P2P, x, f, u, p->side);
+            if (r != SE_OK) return r;
+            if (prof && cudaEventRecord(p->ev_p2p[1], p->side) != cudaSuccess) return SE_ECUDA;
+            if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess) return SE_ECUDA;
+        }
         if (prof && cudaEventRecord(p->ev[st + 1], s) != cudaSuccess) return SE_ECUDA;
     }
     if (prof) p->ev_recorded = 1;
@@ -378,6 +417,10 @@ se_status se_stage_ms(se_plan *p, float ms[SE_NSTAGES])
     if (cudaEventSynchronize(p->ev[SE_NSTAGES]) != cudaSuccess) return SE_ECUDA;
     for (int st = 0; st < SE_NSTAGES; ++st)
         if (cudaEventElapsedTime(&ms[st], p->ev[st], p->ev[st + 1]) != cudaSuccess) return SE_ECUDA;
+    if (p->overlap) {                                   // K2 ran on the side stream, concurrently with stages 3..6
+        if (cudaEventSynchronize(p->ev_p2p[1]) != cudaSuccess) return SE_ECUDA;
+        if (cudaEventElapsedTime(&ms[SE_STAGE_P2P], p->ev_p2p[0], p->ev_p2p[1]) != cudaSuccess) return SE_ECUDA;
+    }
     return SE_OK;
 }
 

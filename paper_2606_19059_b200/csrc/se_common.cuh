@@ -102,6 +102,11 @@ struct se_plan {
     size_t workspace_bytes;
     cudaEvent_t ev[SE_NSTAGES + 1];
     int ev_ok, ev_recorded;
+    // SE_OVERLAP=1: se_eval runs K2 P2P (plain-ALU bound) on a side stream, forked after K3 and joined before K6,
+    // next to the HBM-bound FFT / scale / IFFT stages (PAPER.md:690 notes the two chains are independent)
+    cudaStream_t side;
+    cudaEvent_t ev_fork, ev_join, ev_p2p[2];
+    int overlap, side_ok;
 };
 
 // ---- launchers implemented in the .cu files -------------------------------------------------

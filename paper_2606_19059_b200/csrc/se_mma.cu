@@ -535,6 +535,24 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
             }
             // planes s .. s+P-1 must be in the ring; plane cur may be waiting in `pre`
             if (cur < s) { cur = s; curP = rs; curM = modM(s, M); pre_X = INT_MIN; }   // planes nobody gathers from
+            if (s + P - cur > 2) {
+                // (re)fill after a chunk start or a jump: all missing planes of this lane's k-columns at once (one
+                // memory latency instead of one per plane); residue 4 ks + tq holds plane s + ((4 ks + tq - rs) mod P)
+                const int sM = modM(s, M);
+#pragma unroll
+                for (int ks = 0; ks < KS; ++ks) {
+                    int l = 4 * ks + tq - rs; if (l < 0) l += P;
+                    if (s + l < cur) continue;                       // still valid in the ring
+                    int XM = sM + l; if (XM >= M) XM -= M;
+                    const size_t off = (size_t)XM * MM + colG;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c)
+#pragma unroll
+                        for (int j = 0; j < 2; ++j)
+                            rg[ks][c][j] = (gz_ok && 2 * j + gyl < nyw) ? (double)__ldg(&grid[c * M3 + off + (size_t)(2 * j) * M]) : 0.0;
+                }
+                cur = s + P; curP = rs; curM = modM(cur, M); pre_X = INT_MIN;
+            }
             while (cur < s + P) {
                 if (pre_X != cur) fetch_plane(cur, curP, curM);
                 commit_plane();
