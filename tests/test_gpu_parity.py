@@ -244,3 +244,39 @@ def test_plan_create_rejects_bad_arguments():
         assert ei.value.status == 1, b
     with pytest.raises(KeyError):
         se.Plan(**good, precision="fp16")
+
+
+def test_fp32_tensor_path_edges():
+    """fp32 plans with P = 12 grid on the DMMA sweep (float grid, double records): M not a multiple of the block
+    tile (8 x 24 columns), P == M / 2, particles on the faces, a cluster next to empty cells, ncell = 3."""
+    from dataclasses import replace
+    rng = np.random.default_rng(81)
+    x = rng.random((500, 3)).astype(np.float32)
+    x[:60] = (0.5 + 0.01 * rng.random((60, 3))).astype(np.float32)
+    x[60] = [0.0, 0.0, 0.0]
+    x[61] = [np.nextafter(np.float32(1.0), np.float32(0)), 0.5, 0.25]
+    f = rng.standard_normal((500, 3)).astype(np.float32)
+    for M in (26, 38, 24):
+        c = replace(W.CONFIGS[4], N=500, rc=0.3, xi=3.195 / 0.3, M=M, P=12, label=f"fp32 P=12 M={M}")
+        check_all(c, x, f)
+
+
+def test_side_stream_overlap_is_bit_identical(monkeypatch):
+    """SE_OVERLAP=1 runs K2 on the plan's side stream (fork after K3, join before K6): same bits."""
+    import torch
+    import paper_2606_19059_b200 as se
+    c, x, f = W.scaled(3, 4000)
+    xd = torch.as_tensor(x, device="cuda"); fd = torch.as_tensor(f, device="cuda")
+    out = []
+    for flag in ("0", "1"):
+        monkeypatch.setenv("SE_OVERLAP", flag)
+        with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P) as plan:
+            plan.set_profiling(flag == "1")
+            u = plan.eval(xd, fd).clone()
+            u2 = plan.eval(xd, fd).clone()
+            torch.cuda.synchronize()
+            assert torch.equal(u, u2)
+            if flag == "1":
+                assert plan.stage_ms()["p2p"] > 0
+            out.append(u)
+    assert torch.equal(out[0], out[1])
