@@ -182,7 +182,7 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
                 return best;
             };
             int nch = pick(M / (4 * P), true);
-            int nchg = pick(M / (2 * P), false);
+            int nchg = pick(2 * M / P, false);                  // G2P chunks may be as short as P / 2 planes
             const char *e = std::getenv("SE_NCHUNK");
             if (e && std::atoi(e) > 0) nch = std::min(std::atoi(e), M);
             e = std::getenv("SE_NCHUNK_G2P");
