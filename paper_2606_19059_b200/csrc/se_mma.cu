@@ -567,8 +567,11 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
             // epilogue weights of hit gq at this lane's D columns n = 2 tq, 2 tq + 1 of n-tile j:
             // row 2j + (tq >> 1), z-columns 2 (tq & 1), + 1
             const int ey = tq >> 1, ez = 2 * (tq & 1);
+            // the hit word of group q + 1 is read before the epilogue of group q (whose shared-memory stores would
+            // otherwise order the dependent chain hit word -> record loads behind it)
+            unsigned wn = padded > 0 ? WS.wl[gq] : (unsigned)CAP;
             for (int q = 0; q < padded; q += 8) {
-                const unsigned w = WS.wl[q + gq];
+                const unsigned w = wn;
                 const int a = (int)(w & 0xffu);
                 const double *rp = T.rec[a];
                 double wx[KS];
@@ -578,6 +581,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                 const double wy0 = wrec(rp + C::OY, ly), wy1 = wrec(rp + C::OY, ly + 2);
                 const double wz0 = wrec(rp + C::OZ, lz), wz1 = wrec(rp + C::OZ, lz + 1);
                 const double w00 = wy0 * wz0, w01 = wy0 * wz1, w10 = wy1 * wz0, w11 = wy1 * wz1;
+                if (q + 8 < padded) wn = WS.wl[q + 8 + gq];
                 double d[3][2][2];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) d[c][0][0] = d[c][0][1] = d[c][1][0] = d[c][1][1] = 0.0;
@@ -588,16 +592,11 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                 double pc[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-#ifdef SE_EXP_NOEPI
-                    long long z = __double_as_longlong(d[c][0][0]) ^ __double_as_longlong(d[c][0][1]) ^ __double_as_longlong(d[c][1][0]) ^ __double_as_longlong(d[c][1][1]) ^ __double_as_longlong(w00)^ __double_as_longlong(w01)^ __double_as_longlong(w10)^ __double_as_longlong(w11);
-                    pc[c] = __longlong_as_double(z);
-#else
                     double v = d[c][0][0] * w00;
                     v = fma(d[c][0][1], w01, v); v = fma(d[c][1][0], w10, v); v = fma(d[c][1][1], w11, v);
                     v += __shfl_xor_sync(0xffffffffu, v, 1);
                     v += __shfl_xor_sync(0xffffffffu, v, 2);
                     pc[c] = v;
-#endif
                 }
                 if (tq == 0 && a < CAP) { T.U[a][warp][0] = pc[0]; T.U[a][warp][1] = pc[1]; T.U[a][warp][2] = pc[2]; }
             }
