@@ -73,9 +73,9 @@ template <> struct NearMath<double> {
         for (int e = tid; e < TAB; e += nt) mt[e] = mtab[e];
     }
     // e^{-y}, y >= 0
-    static __device__ __forceinline__ double exp_neg(double y)
+    template <bool CLAMP> static __device__ __forceinline__ double exp_neg(double y)
     {
-        y = fmin(y, 700.0);
+        if (CLAMP) y = fmin(y, 700.0);
         const double SH = 6755399441055744.0;                    // 1.5 * 2^52: round-to-nearest integer shifter
         const double t = fma(y, -1.4426950408889634074, SH);
         const int n = __double2loint(t);                         // n = rint(-y log2 e) <= 0
@@ -87,10 +87,10 @@ template <> struct NearMath<double> {
         for (int k = MT_EXPDEG - 1; k >= 0; --k) p = fma(p, r, c_exp[k]);
         return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
     }
-    static __device__ __forceinline__ double erfcx_tab(double x, const double *mt)
+    template <bool CLAMP> static __device__ __forceinline__ double erfcx_tab(double x, const double *mt)
     {
         const double SH = 6755399441055744.0;
-        const double xm = fmin(x, 8.0);
+        const double xm = CLAMP ? fmin(x, 8.0) : x;
         const double t = fma(xm, 4.0, SH);                       // piece i = rint(4 x), v = x - i/4
         const double v = fma(t - SH, -0.25, xm);
         const double *c = mt + __double2loint(t) * MT_ROW;
@@ -107,11 +107,12 @@ template <> struct NearMath<double> {
         const double e = fma(-(x * y), y, 1.0);
         return fma(y * e, fma(0.375, e, 0.5), y);
     }
+    template <bool CLAMP>
     static __device__ __forceinline__ void coeffs(double r2, double xi, double c2, const double *mt, double &C1, double &C2)
     {
         const double rinv = rsq(r2);
-        const double e = exp_neg(xi * xi * r2);
-        const double A = e * erfcx_tab(xi * (r2 * rinv), mt) * rinv;
+        const double e = exp_neg<CLAMP>(xi * xi * r2);
+        const double A = e * erfcx_tab<CLAMP>(xi * (r2 * rinv), mt) * rinv;
         const double B = c2 * e;
         C1 = A - B;
         C2 = (A + B) * (rinv * rinv);
@@ -125,10 +126,10 @@ template <> struct NearMath<float> {
         const float *src = reinterpret_cast<const float *>(mtab + MT_F32);
         for (int e = tid; e < TAB; e += nt) mt[e] = src[e];
     }
-    static __device__ __forceinline__ float erfcx_tab(float x, const float *mt)
+    template <bool CLAMP> static __device__ __forceinline__ float erfcx_tab(float x, const float *mt)
     {
         const float SH = 12582912.0f;                            // 1.5 * 2^23
-        const float xm = fminf(x, 8.0f);
+        const float xm = CLAMP ? fminf(x, 8.0f) : x;
         const float t = fmaf(xm, 4.0f, SH);
         const float v = fmaf(t - SH, -0.25f, xm);
         const float *c = mt + (__float_as_int(t) - __float_as_int(SH)) * MT_ROWF;
@@ -137,19 +138,22 @@ template <> struct NearMath<float> {
         for (int k = MT_DEGF - 1; k >= 0; --k) p = fmaf(p, v, c[k]);
         return p;
     }
+    template <bool CLAMP>
     static __device__ __forceinline__ void coeffs(float r2, float xi, float c2, const float *mt, float &C1, float &C2)
     {
         float rinv = rsqrtf(r2);
         float x2 = xi * xi * r2;
         float e = expf(-x2);
-        float A = e * erfcx_tab(xi * (r2 * rinv), mt) * rinv;
+        float A = e * erfcx_tab<CLAMP>(xi * (r2 * rinv), mt) * rinv;
         float B = c2 * e;
         C1 = A - B;
         C2 = (A + B) * (rinv * rinv);
     }
 };
 
-template <typename Real>
+// CLAMP: xi rc is so large that the table argument must be clamped (plans with xi rc <= 7.8 never leave the tables:
+// every evaluated pair has r <= rc, a rejected one is evaluated at r = rc)
+template <typename Real, bool CLAMP>
 __global__ void __launch_bounds__(P2P_WARPS * 32, P2P_BLOCKS)
 k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, const int *__restrict__ cellp,
       const int *__restrict__ cell_start, const double *__restrict__ mtab, Real *__restrict__ uN, float rc2m)
@@ -194,7 +198,8 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     // pairs of the fullest queue together and a butterfly sum hands the result to its owner.  The choice is a pure
     // function of the queue lengths, so the summation order stays deterministic.
     // one pair: queue entry at byte offset qo of this lane's (or, mode B, the owner's) column -> contribution d
-    auto pair = [&](int qo, Real T0, Real T1, Real T2, Real tcz, Real &d0, Real &d1, Real &d2) {
+    // keep = false: evaluate but contribute nothing; d0..d2 are ADDED to (fused into the last FMAs)
+    auto pair = [&](int qo, bool keep, Real T0, Real T1, Real T2, Real tcz, Real &d0, Real &d1, Real &d2) {
         const int e = *reinterpret_cast<const unsigned short *>(Qb + qo);
         const int j = VT[e >> P2P_VBITS] + (e & ((1 << P2P_VBITS) - 1));
         const Real *sp = src + 6 * (int64_t)j;
@@ -216,15 +221,15 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
         const Real sx = vs[0], sy = vs[1], sz = vs[2] - tcz;
         const Real rx = T0 - (xj + sx), ry = T1 - (yj + sy), rz = T2 - (zj + sz);
         Real r2 = rx * rx + ry * ry + rz * rz;
-        const bool ok = (r2 <= rc2) && (r2 > (Real)0);
-        if (!ok) r2 = (Real)1;
+        const bool ok = keep && (r2 <= rc2) && (r2 > (Real)0);
+        if (!ok) r2 = rc2;                                       // stays inside the function tables
         Real C1, C2;
-        NearMath<Real>::coeffs(r2, xi, c2, mt, C1, C2);
+        NearMath<Real>::template coeffs<CLAMP>(r2, xi, c2, mt, C1, C2);
         if (!ok) { C1 = (Real)0; C2 = (Real)0; }
         const Real rf = C2 * (rx * f0 + ry * f1 + rz * f2);
-        d0 = C1 * f0 + rf * rx;
-        d1 = C1 * f1 + rf * ry;
-        d2 = C1 * f2 + rf * rz;
+        d0 = fma(rf, rx, fma(C1, f0, d0));
+        d1 = fma(rf, ry, fma(C1, f1, d1));
+        d2 = fma(rf, rz, fma(C1, f2, d2));
     };
     auto round = [&]() {
         const int c = queued();
@@ -237,7 +242,7 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
             const Real T2 = __shfl_sync(0xffffffffu, X2, o), tcz = __shfl_sync(0xffffffffu, czw, o);
             const int ro = (__shfl_sync(0xffffffffu, roff, o) + lane * QSTRIDE) & (QBYTES - 1);
             Real d0 = 0, d1 = 0, d2 = 0;
-            if (lane < cB) pair((o - lane) * 2 + ro, T0, T1, T2, tcz, d0, d1, d2);
+            if (lane < cB) pair((o - lane) * 2 + ro, true, T0, T1, T2, tcz, d0, d1, d2);
 #pragma unroll
             for (int sh = 16; sh > 0; sh >>= 1) {
                 d0 += __shfl_xor_sync(0xffffffffu, d0, sh);
@@ -249,22 +254,16 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
             // mode A2: most queues hold P2P_TWO pairs: every lane pops up to that many of its own, evaluated side
             // by side (independent dependency chains); a lane with fewer re-evaluates its last one and drops it
             if (c > 0) {
-                Real d[P2P_TWO][3];
                 int ro = roff;
 #pragma unroll
                 for (int k = 0; k < P2P_TWO; ++k) {
-                    pair(ro, X0, X1, X2, czw, d[k][0], d[k][1], d[k][2]);
+                    pair(ro, k < c, X0, X1, X2, czw, a0, a1, a2);
                     if (k + 1 < c) ro = (ro + QSTRIDE) & (QBYTES - 1);
                 }
-#pragma unroll
-                for (int k = 0; k < P2P_TWO; ++k)
-                    if (k < c) { a0 += d[k][0]; a1 += d[k][1]; a2 += d[k][2]; }
                 roff = (roff + min(c, P2P_TWO) * QSTRIDE) & (QBYTES - 1);
             }
         } else if (c > 0) {                                      // mode A: every lane pops one pair of its own
-            Real d0, d1, d2;
-            pair(roff, X0, X1, X2, czw, d0, d1, d2);
-            a0 += d0; a1 += d1; a2 += d2;
+            pair(roff, true, X0, X1, X2, czw, a0, a1, a2);
             roff = (roff + QSTRIDE) & (QBYTES - 1);
         }
     };
@@ -381,8 +380,12 @@ cudaError_t p2p_impl(se_plan *p, cudaStream_t s)
     // FP32 filter margin: the cell-relative coordinates are < 2 wcell in magnitude, each rounded to 6e-8
     // relative, so |dr| < 1e-6 wcell per component and |d r^2| < 2 sqrt(3) rc 1e-6 wcell
     const double rc2m = g.rc * g.rc * (1.0 + 1e-5) + 4e-6 * g.rc * g.wcell;
-    k_p2p<Real><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)p->xq, (const Real *)p->src_near, p->cell_sorted,
-                                               p->cell_start, p->mtab, (Real *)p->uN, (float)rc2m);
+    if (g.xi * g.rc > 7.8)
+        k_p2p<Real, true><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)p->xq, (const Real *)p->src_near, p->cell_sorted,
+                                                         p->cell_start, p->mtab, (Real *)p->uN, (float)rc2m);
+    else
+        k_p2p<Real, false><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)p->xq, (const Real *)p->src_near, p->cell_sorted,
+                                                          p->cell_start, p->mtab, (Real *)p->uN, (float)rc2m);
     p->launches += 1;
     return cudaGetLastError();
 }
