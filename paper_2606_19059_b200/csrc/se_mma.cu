@@ -98,13 +98,7 @@ struct Cfg {
     static constexpr int MT = P / 8;                           // m-tiles in the ring
     static constexpr int REC = SPREAD ? SE_MMA_RECS(P) : SE_MMA_RECG(P);   // doubles per record
     static constexpr int OY = SPREAD ? 3 * P : P, OZ = OY + P, OM = OZ + P; // offsets of Wy, Wz, (a_y, a_z)
-#ifndef SE_EXP_NST
-#define SE_EXP_NST 5
-#endif
-#ifndef SE_EXP_NSTS
-#define SE_EXP_NSTS 3
-#endif
-    static constexpr int NST = SPREAD ? SE_EXP_NSTS : SE_EXP_NST;       // stages
+    static constexpr int NST = SPREAD ? 3 : 5;                 // stages (measured: P2G 4 = 3, G2P 5 > 4)
     static constexpr int GRP = SPREAD ? 4 : 8;                 // candidates per K-group (P2G: k = 4; G2P: n = 8)
     static constexpr int NSB = (P + BY - 2) / BY + 2, NSC = (P + BZ - 2) / BZ + 2;   // block tiles a window can meet
     static_assert(P % 4 == 0 && (!SPREAD || P % 8 == 0) && (REC % 2) == 0 && NCW % 4 == 0 && CAP % GRP == 0, "layout");
@@ -499,11 +493,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
             for (int c = 0; c < 3; ++c)
 #pragma unroll
                 for (int j = 0; j < 2; ++j)
-#ifdef SE_EXP_NORING
-                    pre[c][j] = (double)(XM + c + j);
-#else
                     pre[c][j] = (gz_ok && 2 * j + gyl < nyw) ? (double)__ldg(&grid[c * M3 + off + (size_t)(2 * j) * M]) : 0.0;
-#endif
         };
         auto commit_ks = [&](auto ksc) {
             constexpr int ks = decltype(ksc)::value;
