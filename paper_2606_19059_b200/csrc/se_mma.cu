@@ -495,22 +495,18 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                 for (int j = 0; j < 2; ++j)
                     pre[c][j] = (gz_ok && 2 * j + gyl < nyw) ? (double)__ldg(&grid[c * M3 + off + (size_t)(2 * j) * M]) : 0.0;
         };
-        auto commit_ks = [&](auto ksc) {
-            constexpr int ks = decltype(ksc)::value;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) { rg[ks][c][0] = pre[c][0]; rg[ks][c][1] = pre[c][1]; }
-        };
         auto commit_plane = [&]() {                                  // move `pre` into its residue of the ring
-            if (tq != (preP & 3)) return;
-            switch (preP >> 2) {
-            case 0: commit_ks(std::integral_constant<int, 0>{}); break;
-            case 1: commit_ks(std::integral_constant<int, 1>{}); break;
-            case 2: commit_ks(std::integral_constant<int, 2>{}); break;
-            case 3: commit_ks(std::integral_constant<int, 3>{}); break;
-            case 4: if constexpr (KS > 4) commit_ks(std::integral_constant<int, 4>{}); break;
-            case 5: if constexpr (KS > 5) commit_ks(std::integral_constant<int, 5>{}); break;
-            case 6: if constexpr (KS > 6) commit_ks(std::integral_constant<int, 6>{}); break;
-            case 7: if constexpr (KS > 7) commit_ks(std::integral_constant<int, 7>{}); break;
+            // predicated moves over the k-steps (a switch makes the compiler shuffle the whole ring through moves)
+            const int ksel = preP >> 2;
+            const bool mine = tq == (preP & 3);
+#pragma unroll
+            for (int ks = 0; ks < KS; ++ks) {
+                const bool p = mine && ksel == ks;
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int j = 0; j < 2; ++j)
+                        if (p) rg[ks][c][j] = pre[c][j];
             }
         };
         for (int r = 0;; ++r) {
