@@ -496,18 +496,22 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                     pre[c][j] = (gz_ok && 2 * j + gyl < nyw) ? (double)__ldg(&grid[c * M3 + off + (size_t)(2 * j) * M]) : 0.0;
         };
         auto commit_plane = [&]() {                                  // move `pre` into its residue of the ring
-            // predicated moves over the k-steps (a switch makes the compiler shuffle the whole ring through moves)
-            const int ksel = preP >> 2;
+            // warp-uniform switch over the k-step, predicated moves inside (a divergent early-out in front of the
+            // switch made the compiler shuffle the whole ring through moves)
             const bool mine = tq == (preP & 3);
-#pragma unroll
-            for (int ks = 0; ks < KS; ++ks) {
-                const bool p = mine && ksel == ks;
-#pragma unroll
-                for (int c = 0; c < 3; ++c)
-#pragma unroll
-                    for (int j = 0; j < 2; ++j)
-                        if (p) rg[ks][c][j] = pre[c][j];
+            const int ksel = __shfl_sync(0xffffffffu, preP >> 2, 0);
+#define SE_COMMIT(ks)                                                                  \
+    case ks:                                                                           \
+        if constexpr (ks < KS) {                                                       \
+            _Pragma("unroll") for (int c = 0; c < 3; ++c) {                            \
+                if (mine) { rg[ks < KS ? ks : 0][c][0] = pre[c][0]; rg[ks < KS ? ks : 0][c][1] = pre[c][1]; } \
+            }                                                                          \
+        }                                                                              \
+        break;
+            switch (ksel) {
+                SE_COMMIT(0) SE_COMMIT(1) SE_COMMIT(2) SE_COMMIT(3) SE_COMMIT(4) SE_COMMIT(5) SE_COMMIT(6) SE_COMMIT(7)
             }
+#undef SE_COMMIT
         };
         for (int r = 0;; ++r) {
             const int sg = r % NST;
