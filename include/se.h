@@ -23,6 +23,10 @@
  *   - Every entry point returns a status; nothing aborts or throws.  NaN/Inf inputs give
  *     unspecified values but never out-of-bounds accesses.
  *   - There is no CPU fallback: without a CUDA device se_plan_create returns SE_ECUDA.
+ *   - Environment variables read at se_plan_create (experiments and tests only; results do not change beyond
+ *     rounding order): SE_GRID_MODE = tile | sweep | mma (gridding kernels; default: the FP64 tensor-core sweep
+ *     for fp64 plans with P = 16, 24 and fp32 plans with P = 12, else the generic tile kernel), SE_NCHUNK and
+ *     SE_NCHUNK_G2P (x-chunks of K3 / K5), SE_OVERLAP = 1 (K2 on a side stream next to the FFT stages).
  */
 #ifndef SE_B200_H
 #define SE_B200_H
