@@ -41,6 +41,9 @@ constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV 
 #ifndef P2P_TWO
 #define P2P_TWO 2
 #endif
+#ifndef P2P_TWO_F32
+#define P2P_TWO_F32 4
+#endif
 #ifndef P2P_FU
 #define P2P_FU 8
 #endif
@@ -231,6 +234,7 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
         d1 = fma(rf, ry, fma(C1, f1, d1));
         d2 = fma(rf, rz, fma(C1, f2, d2));
     };
+    constexpr int KP = sizeof(Real) == 8 ? P2P_TWO : P2P_TWO_F32;   // pairs per lane and round in mode A2
     auto round = [&]() {
         const int c = queued();
         const unsigned m1 = __ballot_sync(0xffffffffu, c > 0);
@@ -250,17 +254,17 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                 d2 += __shfl_xor_sync(0xffffffffu, d2, sh);
             }
             if (lane == o) { a0 += d0; a1 += d1; a2 += d2; roff = (roff + cB * QSTRIDE) & (QBYTES - 1); }
-        } else if (P2P_TWO > 1 && __popc(__ballot_sync(0xffffffffu, c >= P2P_TWO)) * 4 >= __popc(m1) * 3) {
-            // mode A2: most queues hold P2P_TWO pairs: every lane pops up to that many of its own, evaluated side
+        } else if (KP > 1 && __popc(__ballot_sync(0xffffffffu, c >= KP)) * 4 >= __popc(m1) * 3) {
+            // mode A2: most queues hold KP pairs: every lane pops up to that many of its own, evaluated side
             // by side (independent dependency chains); a lane with fewer re-evaluates its last one and drops it
             if (c > 0) {
                 int ro = roff;
 #pragma unroll
-                for (int k = 0; k < P2P_TWO; ++k) {
+                for (int k = 0; k < KP; ++k) {
                     pair(ro, k < c, X0, X1, X2, czw, a0, a1, a2);
                     if (k + 1 < c) ro = (ro + QSTRIDE) & (QBYTES - 1);
                 }
-                roff = (roff + min(c, P2P_TWO) * QSTRIDE) & (QBYTES - 1);
+                roff = (roff + min(c, KP) * QSTRIDE) & (QBYTES - 1);
             }
         } else if (c > 0) {                                      // mode A: every lane pops one pair of its own
             pair(roff, true, X0, X1, X2, czw, a0, a1, a2);
