@@ -39,13 +39,13 @@ constexpr int P2P_CHUNK = 32;       // sources scanned between two queue-room ch
 constexpr int P2P_VBITS = 9;        // a queue entry = (virtual cell << VBITS) | offset: virtual cells of <= 512 sources
 constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV << VBITS) = 2^15)
 #ifndef P2P_TWO
-#define P2P_TWO 2
+#define P2P_TWO 3
 #endif
 #ifndef P2P_TWO_F32
 #define P2P_TWO_F32 4
 #endif
 #ifndef P2P_FU
-#define P2P_FU 8
+#define P2P_FU 4            /* filter group (sources loaded ahead of the queue stores): fp64; fp32 uses twice as many */
 #endif
 #ifndef P2P_BLOCKS
 #define P2P_BLOCKS 4
@@ -351,12 +351,14 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                         // groups of P2P_FU sources: all broadcast loads of a group first (the queue stores that
                         // follow are shared-memory stores the compiler must order against later loads)
 #pragma unroll 1
-                        for (int jb = 0; jb < n; jb += P2P_FU) {
-                            float4 q[P2P_FU];
+                        constexpr int FU = sizeof(Real) == 8 ? P2P_FU : 2 * P2P_FU;
+#pragma unroll 1
+                        for (int jb = 0; jb < n; jb += FU) {
+                            float4 q[FU];
 #pragma unroll
-                            for (int u = 0; u < P2P_FU; ++u) q[u] = SB[jb + u];
+                            for (int u = 0; u < FU; ++u) q[u] = SB[jb + u];
 #pragma unroll
-                            for (int u = 0; u < P2P_FU; ++u) {
+                            for (int u = 0; u < FU; ++u) {
                                 const float rx = tx - q[u].x, ry = ty - q[u].y, rz = tz - q[u].z;
                                 if (rx * rx + ry * ry + rz * rz <= rc2m) {
                                     *reinterpret_cast<unsigned short *>(Qb + woff) = (unsigned short)(ebase + jb + u);
