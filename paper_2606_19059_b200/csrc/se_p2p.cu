@@ -350,7 +350,6 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                         const int ebase = (vslot << P2P_VBITS) + (j0 - v0);
                         // groups of P2P_FU sources: all broadcast loads of a group first (the queue stores that
                         // follow are shared-memory stores the compiler must order against later loads)
-#pragma unroll 1
                         constexpr int FU = sizeof(Real) == 8 ? P2P_FU : 2 * P2P_FU;
 #pragma unroll 1
                         for (int jb = 0; jb < n; jb += FU) {
