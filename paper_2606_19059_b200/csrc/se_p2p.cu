@@ -42,7 +42,7 @@ constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV 
 #define P2P_TWO 3
 #endif
 #ifndef P2P_TWO_F32
-#define P2P_TWO_F32 4
+#define P2P_TWO_F32 6
 #endif
 #ifndef P2P_FU
 #define P2P_FU 4            /* filter group (sources loaded ahead of the queue stores): fp64; fp32 uses twice as many */
