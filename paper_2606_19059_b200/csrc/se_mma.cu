@@ -572,18 +572,15 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                 const double wz0 = wrec(rp + C::OZ, lz), wz1 = wrec(rp + C::OZ, lz + 1);
                 const double w00 = wy0 * wz0, w01 = wy0 * wz1, w10 = wy1 * wz0, w11 = wy1 * wz1;
                 if (q + 8 < padded) wn = WS.wl[q + 8 + gq];
-                double d[3][2][2];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) d[c][0][0] = d[c][0][1] = d[c][1][0] = d[c][1][1] = 0.0;
-#pragma unroll
-                for (int ks = 0; ks < KS; ++ks)
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) { dmma(d[c][0], wx[ks], rg[ks][c][0]); dmma(d[c][1], wx[ks], rg[ks][c][1]); }
+                // one component at a time: 8 accumulator registers live instead of 24
                 double pc[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    double v = d[c][0][0] * w00;
-                    v = fma(d[c][0][1], w01, v); v = fma(d[c][1][0], w10, v); v = fma(d[c][1][1], w11, v);
+                    double d0[2] = {0.0, 0.0}, d1[2] = {0.0, 0.0};
+#pragma unroll
+                    for (int ks = 0; ks < KS; ++ks) { dmma(d0, wx[ks], rg[ks][c][0]); dmma(d1, wx[ks], rg[ks][c][1]); }
+                    double v = d0[0] * w00;
+                    v = fma(d0[1], w01, v); v = fma(d1[0], w10, v); v = fma(d1[1], w11, v);
                     v += __shfl_xor_sync(0xffffffffu, v, 1);
                     v += __shfl_xor_sync(0xffffffffu, v, 2);
                     pc[c] = v;
