@@ -572,18 +572,30 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                 const double wz0 = wrec(rp + C::OZ, lz), wz1 = wrec(rp + C::OZ, lz + 1);
                 const double w00 = wy0 * wz0, w01 = wy0 * wz1, w10 = wy1 * wz0, w11 = wy1 * wz1;
                 if (q + 8 < padded) wn = WS.wl[q + 8 + gq];
-                // one component at a time: 8 accumulator registers live instead of 24
+                // one component at a time (8 accumulator registers live instead of 24), the epilogue of component c
+                // placed behind the DMMAs of component c + 1 so that it does not wait for their results in line
                 double pc[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    double d0[2] = {0.0, 0.0}, d1[2] = {0.0, 0.0};
+                double e0[2], e1[2];
+                auto burst = [&](int c, double (&d0)[2], double (&d1)[2]) {
+                    d0[0] = d0[1] = d1[0] = d1[1] = 0.0;
 #pragma unroll
                     for (int ks = 0; ks < KS; ++ks) { dmma(d0, wx[ks], rg[ks][c][0]); dmma(d1, wx[ks], rg[ks][c][1]); }
+                };
+                auto fold = [&](const double (&d0)[2], const double (&d1)[2]) -> double {
                     double v = d0[0] * w00;
                     v = fma(d0[1], w01, v); v = fma(d1[0], w10, v); v = fma(d1[1], w11, v);
                     v += __shfl_xor_sync(0xffffffffu, v, 1);
                     v += __shfl_xor_sync(0xffffffffu, v, 2);
-                    pc[c] = v;
+                    return v;
+                };
+                {
+                    double f0[2], f1[2];
+                    burst(0, e0, e1);
+                    burst(1, f0, f1);
+                    pc[0] = fold(e0, e1);
+                    burst(2, e0, e1);
+                    pc[1] = fold(f0, f1);
+                    pc[2] = fold(e0, e1);
                 }
                 if (tq == 0 && a < CAP) { T.U[a][warp][0] = pc[0]; T.U[a][warp][1] = pc[1]; T.U[a][warp][2] = pc[2]; }
             }
