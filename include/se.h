@@ -24,8 +24,8 @@
  *     unspecified values but never out-of-bounds accesses.
  *   - There is no CPU fallback: without a CUDA device se_plan_create returns SE_ECUDA.
  *   - Environment variables read at se_plan_create (experiments and tests only; results do not change beyond
- *     rounding order): SE_GRID_MODE = tile | sweep | mma (gridding kernels; default: the FP64 tensor-core sweep
- *     for fp64 plans with P = 16, 24 and fp32 plans with P = 12, else the generic tile kernel), SE_NCHUNK and
+ *     rounding order): SE_GRID_MODE = tile (force the generic gridding kernel; default: the FP64 tensor-core
+ *     sweep for fp64 plans with P = 16, 24 and fp32 plans with P = 12, else the generic tile kernel), SE_NCHUNK and
  *     SE_NCHUNK_G2P (x-chunks of K3 / K5), SE_OVERLAP = 1 (K2 on a side stream next to the FFT stages).
  */
 #ifndef SE_B200_H
@@ -87,10 +87,10 @@ typedef struct {
     double a;            /* window exponent 2 xi^2 / eta : w(r) = c_w exp(-a r^2)        */
     double cw;           /* (a/pi)^{3/2}                                                 */
     int ncell;           /* near cells per dimension, floor(L/rc)          (reading S7)  */
-    int nbin;            /* grid bins per dimension: ceil(M/8) (tile mode), ceil(M/4) (sweep mode) */
-    int grid_mode;       /* gridding kernels: 0 = tile-stationary (any even P), 1 = z-sweep (P = 12, 16, 24) */
+    int nbin;            /* grid bins per dimension: ceil(M/8)                          */
+    int grid_mode;       /* gridding kernels: 0 = tile-stationary (any even P), 2 = FP64 tensor-core sweep */
     int nbins_total;     /* entries of SE_BUF_BIN_START minus 1: nbin^3 (mode 0), M * nbin^2 (mode 1)      */
-    int nchunk;          /* sweep mode: chunks along x                                   */
+    int nchunk;          /* tensor-core sweep: chunks along x (P2G)                      */
     int64_t nmodes;      /* M * M * (M/2+1) stored modes per component                   */
     size_t workspace_bytes; /* device memory owned by the plan (incl. cuFFT work area)   */
 } se_info;

@@ -145,15 +145,14 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     g.ncell = ncell;
     g.nbin = (M + SE_BIN - 1) / SE_BIN;
     g.nbins_total = g.nbin * g.nbin * g.nbin;
-    g.grid_mode = 0; g.nchunk = 1; g.nchunk_g2p = 1; g.gsteps = 1;
+    g.grid_mode = 0; g.nchunk = 1; g.nchunk_g2p = 1;
     {
         // Gridding kernels: FP64 tensor-core sweep where it applies, else the generic tile kernel.
-        // SE_GRID_MODE = tile | sweep | mma overrides (tests and experiments).
+        // SE_GRID_MODE = tile forces the generic kernel (tests and experiments).
         const char *force = std::getenv("SE_GRID_MODE");
         const bool want_tile = force && std::strcmp(force, "tile") == 0;
-        const bool want_sweep = force && std::strcmp(force, "sweep") == 0;
         const int zb = (M + SE_MMA_ZBIN - 1) / SE_MMA_ZBIN;
-        if (se_mma_supported(P, (int)prec) && (double)M * zb * M < 5.0e8 && !want_tile && !want_sweep) {
+        if (se_mma_supported(P, (int)prec) && (double)M * zb * M < 5.0e8 && !want_tile) {
             g.grid_mode = 2;
             g.ring = se_mma_ring(P);
             g.nbin = zb;
@@ -189,25 +188,6 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
             if (e && std::atoi(e) > 0) nchg = std::min(std::atoi(e), M);
             g.nchunk = std::max(nch, 1);
             g.nchunk_g2p = std::max(nchg, 1);
-        } else if (want_sweep && se_sweep_supported(P) &&
-                   (double)M * ((M + SE_SBIN - 1) / SE_SBIN) * ((M + SE_SBIN - 1) / SE_SBIN) < 1.0e9) {
-            const int sb = (M + SE_SBIN - 1) / SE_SBIN;
-            g.grid_mode = 1;
-            g.nbin = sb;
-            g.nbins_total = M * sb * sb;
-            // candidates per plane seen by one block: density x (bins covering tile + support)
-            double dens = (double)N / ((double)M * M * M);
-            double cand = dens * (SE_SWEEP_TB + P + 2 * SE_SBIN) * (16 + P + 2 * SE_SBIN);
-            int gs = (int)std::ceil(512.0 / std::max(cand, 1e-3));
-            g.gsteps = std::min(std::max(gs, 1), SE_GSTEPS_MAX);
-            int tiles = ((M + SE_SWEEP_TB - 1) / SE_SWEEP_TB) * ((M + 15) / 16);
-            int nch = (148 * 6 + tiles - 1) / tiles;
-            nch = std::min(nch, std::max(1, M / (2 * P)));
-            const char *e = std::getenv("SE_NCHUNK");
-            if (e && std::atoi(e) > 0) nch = std::min(std::atoi(e), M);
-            g.nchunk = std::max(nch, 1);
-            e = std::getenv("SE_GSTEPS");
-            if (e && std::atoi(e) > 0) g.gsteps = std::min(std::atoi(e), SE_GSTEPS_MAX);
         }
     }
     g.rel_coords = prec == SE_FP32;
@@ -244,7 +224,6 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     if (g.grid_mode == 2) A.get(&p->recg, (size_t)N * SE_MMA_RECG(P) * 8);
     A.get(&p->fs_grid, N * 3 * rb);
     A.get(&p->uF, std::max((size_t)N * 3 * rb, (size_t)N * sizeof(int)));
-    if (g.grid_mode == 1) A.get(&p->uFpart, (size_t)N * SE_NSLOT * 3 * rb);
     if (g.grid_mode == 2) A.get(&p->uFpart, (size_t)N * se_mma_slots(P) * 3 * 8);
     A.get(&p->grid, 3 * M3 * rb);
     A.get(&p->spec, 3 * nm * 2 * rb);

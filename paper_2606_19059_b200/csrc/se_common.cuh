@@ -21,12 +21,6 @@ constexpr int SE_BIN = 8;
 constexpr int SE_GRID_THREADS = SE_TX * SE_TY;      // 256
 constexpr int SE_ROUND = 128;                        // candidates examined per staging round
 constexpr int SE_PMAX = 32;                          // largest window support
-// z-sweep gridding kernels (se_sweep.cu): particles sorted by (base plane, 4x4 bins in y,z)
-constexpr int SE_SBIN = 4;
-constexpr int SE_SWEEP_TB = 8;                       // block tile in y
-constexpr int SE_NSLOT_B = 5, SE_NSLOT_C = 3;        // G2P partial-sum slots per particle (tiles touched)
-constexpr int SE_NSLOT = SE_NSLOT_B * SE_NSLOT_C;
-constexpr int SE_GSTEPS_MAX = 16;
 // FP64 tensor-core gridding kernels (se_mma.cu): particles sorted by (anchor plane, anchor_z / ZBIN, anchor_y);
 // a block of NWY x NWZ consumer warps (+ the producer warpgroup) owns 4 NWY x 4 NWZ (y, z) columns.  K1 writes two
 // 16-byte aligned records per particle in sorted order (always double, also for fp32 plans; anchors as two int32
@@ -43,14 +37,13 @@ struct SeGeom {
     int64_t N;
     int M, P;
     int ncell;          // near cells per dimension
-    int nbin;           // grid bins per dimension = ceil(M / SE_BIN) (tile mode) or ceil(M / SE_SBIN) (sweep)
-    int grid_mode;      // 0: tile-stationary k_grid (any even P), 1: z-sweep kernels (P = 12, 16, 24),
-                        // 2: FP64 tensor-core sweep (se_mma.cu; P = 16, 24)
-    int nbins_total;    // nbin^3 (tile mode), M * nbin^2 (sweep mode), M * nbin * M (mma mode)
-    int nchunk;         // sweep / mma mode: chunks along x (P2G)
+    int nbin;           // grid bins per dimension = ceil(M / SE_BIN) (tile mode) or z-bins ceil(M / 8) (mma mode)
+    int grid_mode;      // 0: tile-stationary k_grid (any even P),
+                        // 2: FP64 tensor-core sweep (se_mma.cu; fp64 P = 16, 24; fp32 P = 12)
+    int nbins_total;    // nbin^3 (tile mode), M * nbin * M (mma mode)
+    int nchunk;         // mma mode: chunks along x (P2G)
     int nchunk_g2p;     // mma mode: chunks along x (G2P)
     int ring;           // mma mode: row stride of the spread records = P rounded up to a multiple of 8
-    int gsteps;         // sweep mode: planes whose candidates are enumerated together
     int rel_coords;     // 1: near-sorted positions are cell-relative (fp32 path)
     double L, xi, rc;
     double h;           // L / M
@@ -88,7 +81,7 @@ struct se_plan {
     void *recg;                    // mma mode: gather records
     void *fs_grid;                 // [N][3] Real
     void *uF;                      // [N][3] Real, grid-sorted order (unscaled sum)
-    void *uFpart;                  // sweep mode: [N][SE_NSLOT][3] Real per-(particle, tile) partial sums
+    void *uFpart;                  // mma mode: [slots][N][3] double per-(particle, block tile) partial sums
     // grids
     void *grid;                    // [3][M][M][M] Real
     void *spec;                    // [3][M][M][M/2+1] complex Real
@@ -118,9 +111,6 @@ cudaError_t se_launch_g2p(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_sum(se_plan *p, const void *f, void *u, cudaStream_t s);
 cudaError_t se_build_ktab(se_plan *p);
 cudaError_t se_build_mtab(se_plan *p);      // allocates and fills p->mtab
-cudaError_t se_launch_sweep_p2g(se_plan *p, cudaStream_t s);
-cudaError_t se_launch_sweep_g2p(se_plan *p, cudaStream_t s);
-bool se_sweep_supported(int P);
 cudaError_t se_launch_mma_p2g(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_mma_g2p(se_plan *p, cudaStream_t s);
 bool se_mma_supported(int P, int precision);

@@ -282,13 +282,11 @@ cudaError_t grid_impl(se_plan *p, cudaStream_t s)
 cudaError_t se_launch_p2g(se_plan *p, cudaStream_t s)
 {
     if (p->g.grid_mode == 2) return se_launch_mma_p2g(p, s);
-    if (p->g.grid_mode == 1) return se_launch_sweep_p2g(p, s);
     return p->precision == SE_FP64 ? grid_impl<double, true>(p, s) : grid_impl<float, true>(p, s);
 }
 
 cudaError_t se_launch_g2p(se_plan *p, cudaStream_t s)
 {
     if (p->g.grid_mode == 2) return se_launch_mma_g2p(p, s);
-    if (p->g.grid_mode == 1) return se_launch_sweep_g2p(p, s);
     return p->precision == SE_FP64 ? grid_impl<double, false>(p, s) : grid_impl<float, false>(p, s);
 }

@@ -53,9 +53,7 @@ __global__ void k_bin(SeGeom g, const Real *__restrict__ x, int *__restrict__ ce
 #pragma unroll
         for (int d = 0; d < 3; ++d) { a[d] = b[d] - (g.P / 2 - 1); if (a[d] < 0) a[d] += g.M; }
         bi = (a[0] * g.nbin + a[2] / SE_MMA_ZBIN) * g.M + a[1];
-    } else if (g.grid_mode == 1)
-        bi = (b[0] * g.nbin + b[1] / SE_SBIN) * g.nbin + b[2] / SE_SBIN;
-    else
+    } else
         bi = ((b[0] / SE_BIN) * g.nbin + b[1] / SE_BIN) * g.nbin + b[2] / SE_BIN;
     cell_of[i] = ci;
     bin_of[i] = bi;

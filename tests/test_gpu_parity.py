@@ -45,8 +45,6 @@ def check_all(c, x, f, tol_override=None):
     if g["info"]["grid_mode"] == 2:      # FP64 tensor-core sweep: key (anchor plane, anchor_z / 8, anchor_y)
         an = (i0 - (c.P // 2 - 1)) % c.M
         linb = (an[:, 0] * nb + an[:, 2] // 8) * c.M + an[:, 1]
-    elif g["info"]["grid_mode"] == 1:    # z-sweep kernels: key (base plane, y-bin, z-bin), 4-wide bins
-        linb = (i0[:, 0] * nb + i0[:, 1] // 4) * nb + i0[:, 2] // 4
     else:                                # tile kernels: 8^3 bins
         linb = ((i0[:, 0] // 8) * nb + i0[:, 1] // 8) * nb + i0[:, 2] // 8
     assert bs.shape[0] == g["info"]["nbins_total"] + 1
