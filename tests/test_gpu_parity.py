@@ -278,3 +278,19 @@ def test_side_stream_overlap_is_bit_identical(monkeypatch):
                 assert plan.stage_ms()["p2p"] > 0
             out.append(u)
     assert torch.equal(out[0], out[1])
+
+
+def test_large_xi_rc_clamp_path_and_tiny_N():
+    """xi rc = 9 > 7.8 selects the K2 instantiation that clamps the function-table arguments; N = 2 and N = 33
+    exercise warps with a single live lane and a ragged last warp."""
+    from dataclasses import replace
+    rng = np.random.default_rng(82)
+    for N in (2, 33, 700):
+        c = replace(W.CONFIGS[1], N=N, rc=0.3, xi=30.0, M=96, P=24, label=f"clamp N={N}")
+        x = rng.random((N, 3)); f = rng.standard_normal((N, 3))
+        if N == 2:
+            x[1] = x[0] + [0.01, -0.02, 0.015]          # one close pair inside rc
+        check_all(c, x, f)
+    c = replace(W.CONFIGS[4], N=700, rc=0.3, xi=30.0, M=96, P=12, label="clamp fp32")
+    x = rng.random((700, 3)).astype(np.float32); f = rng.standard_normal((700, 3)).astype(np.float32)
+    check_all(c, x, f)
