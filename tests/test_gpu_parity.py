@@ -294,3 +294,14 @@ def test_large_xi_rc_clamp_path_and_tiny_N():
     c = replace(W.CONFIGS[4], N=700, rc=0.3, xi=30.0, M=96, P=12, label="clamp fp32")
     x = rng.random((700, 3)).astype(np.float32); f = rng.standard_normal((700, 3)).astype(np.float32)
     check_all(c, x, f)
+
+
+@pytest.mark.parametrize("P,M", [(16, 48), (32, 64), (8, 40), (2, 24)])
+def test_other_window_sizes_fp64(P, M):
+    """P = 16 is the second tensor-core instantiation; P = 32 (the largest support), 8 and 2 run the generic tile
+    kernel.  Small P make the method inaccurate, not the parity: the oracle uses the same discretisation."""
+    from dataclasses import replace
+    rng = np.random.default_rng(83 + P)
+    c = replace(W.CONFIGS[1], N=900, rc=0.2, xi=12.0, M=M, P=P, label=f"P={P} M={M}")
+    x = rng.random((900, 3)); f = rng.standard_normal((900, 3))
+    check_all(c, x, f)
