@@ -294,6 +294,9 @@ def run_b200(args):
         "data": "synthetic",
         "config": {"workload": c.label, "N": c.N, "L": c.L, "xi": c.xi, "rc": c.rc, "M": c.M, "P": c.P,
                    "precision": c.precision, "eta": info.eta, "ncell": info.ncell,
+                   "gridding": ("FP64 tensor-core sweep (double records and accumulators%s)" %
+                                (", float grid" if c.precision == "fp32" else "")) if info.grid_mode == 2
+                   else "generic tile kernel in the plan's precision",
                    "parallelism": "replicas x%d" % world,
                    "l2": "no explicit flush: every step streams the %.2f GB plan workspace (grid %.2f GB + "
                          "spectrum %.2f GB), far larger than the 126 MB L2" %
