@@ -6,7 +6,11 @@ def rel(a, b):
     a, b = np.asarray(a), np.asarray(b)
     dt = np.complex128 if (np.iscomplexobj(a) or np.iscomplexobj(b)) else np.float64
     a, b = a.astype(dt), b.astype(dt)
-    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+    den = float(np.linalg.norm(b))
+    num = float(np.linalg.norm(a - b))
+    if den == 0.0:                       # e.g. u^N of a single particle: both sides must be exactly zero
+        return 0.0 if num == 0.0 else float("inf")
+    return num / den
 
 
 def run_stages(c, x, f):

@@ -305,3 +305,28 @@ def test_other_window_sizes_fp64(P, M):
     c = replace(W.CONFIGS[1], N=900, rc=0.2, xi=12.0, M=M, P=P, label=f"P={P} M={M}")
     x = rng.random((900, 3)); f = rng.standard_normal((900, 3))
     check_all(c, x, f)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_small_plans(seed):
+    """Seeded random plans on the tensor-core path: grid sizes around the block-tile multiples (8 x 24 columns),
+    M close to P, few and many particles per tile, non-unit box, positions outside the box."""
+    from dataclasses import replace
+    rng = np.random.default_rng(9000 + seed)
+    prec = "fp32" if seed % 3 == 2 else "fp64"
+    P = 12 if prec == "fp32" else (16 if seed % 2 else 24)
+    M = int(rng.choice([P, P + 2, 26, 30, 34, 46, 50, 58, 72, 74]))
+    M = max(M, P)
+    L = float(rng.choice([1.0, 2.5, 0.37]))
+    N = int(rng.choice([1, 3, 40, 333, 1500]))
+    ncell = int(rng.integers(3, 7))
+    rc = L / ncell * float(rng.uniform(0.8, 1.0))
+    h = L / M
+    m = 0.95 * np.sqrt(np.pi * P)
+    xi = float(rng.uniform(0.55, 0.95)) * m / (P * h)          # eta = (P h xi / m)^2 < 1
+    base = W.CONFIGS[4] if prec == "fp32" else W.CONFIGS[1]
+    c = replace(base, N=N, L=L, rc=rc, xi=xi, M=M, P=P, label=f"random {seed}: {prec} N={N} L={L} M={M} P={P}")
+    dt = np.float32 if prec == "fp32" else np.float64
+    x = (rng.random((N, 3)) * L * 1.6 - 0.3 * L).astype(dt)    # some outside [0, L)
+    f = rng.standard_normal((N, 3)).astype(dt)
+    check_all(c, x, f)
