@@ -188,6 +188,17 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
             if (e && std::atoi(e) > 0) nchg = std::min(std::atoi(e), M);
             g.nchunk = std::max(nch, 1);
             g.nchunk_g2p = std::max(nchg, 1);
+            // P2G with whole sweeps: if the last wave is partly filled, split only its tiles along x (each piece pays
+            // P - 1 warm-up planes) when that shortens the tail
+            g.nfull = tiles; g.nsplit = 1;
+            const int R = tiles % nsm;
+            if (g.nchunk == 1 && R > 0 && tiles > nsm && !std::getenv("SE_NCHUNK")) {
+                double best = 0.95;
+                for (int k = 2; k <= 4 && M / k >= P; ++k) {
+                    const double cost = std::ceil((double)R * k / nsm) * ((double)M / k + P - 1) / M;
+                    if (cost < best) { best = cost; g.nsplit = k; g.nfull = tiles - R; }
+                }
+            }
         }
     }
     g.rel_coords = prec == SE_FP32;

@@ -43,6 +43,8 @@ struct SeGeom {
     int nbins_total;    // nbin^3 (tile mode), M * nbin * M (mma mode)
     int nchunk;         // mma mode: chunks along x (P2G)
     int nchunk_g2p;     // mma mode: chunks along x (G2P)
+    int nfull, nsplit;  // mma mode, P2G with nchunk = 1: the last `tiles - nfull` block tiles (those of the partly filled
+                        // last wave) are split into nsplit x-chunks each (nsplit = 1: no split)
     int ring;           // mma mode: row stride of the spread records = P rounded up to a multiple of 8
     int rel_coords;     // 1: near-sorted positions are cell-relative (fp32 path)
     double L, xi, rc;

@@ -163,8 +163,14 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int M = g.M, nzb = g.nbin;
     const int ntY = (M + BY - 1) / BY, ntZ = (M + BZ - 1) / BZ;
-    const int tz = blockIdx.x % ntZ, ty = (blockIdx.x / ntZ) % ntY, chunk = blockIdx.x / (ntZ * ntY);
-    const int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
+    int tile = blockIdx.x % (ntZ * ntY), chunk = blockIdx.x / (ntZ * ntY);
+    int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
+    if (SPREAD && g.nsplit > 1) {
+        // whole sweeps first (one block per tile), then the tiles of the last wave in nsplit pieces each
+        if ((int)blockIdx.x < g.nfull) { tile = blockIdx.x; chunk = 0; nchunk = 1; }
+        else { const int bb = blockIdx.x - g.nfull; tile = g.nfull + bb / g.nsplit; chunk = bb % g.nsplit; nchunk = g.nsplit; }
+    }
+    const int tz = tile % ntZ, ty = tile / ntZ;
     const int CL = (M + nchunk - 1) / nchunk;
     const int X0 = chunk * CL;
     const int CLen = min(CL, M - X0);
@@ -646,7 +652,8 @@ cudaError_t launch(se_plan *p, cudaStream_t s)
     }
     const int ntY = (g.M + C::BY - 1) / C::BY, ntZ = (g.M + C::BZ - 1) / C::BZ;
     const int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
-    kern<<<(unsigned)(nchunk * ntY * ntZ), C::NT, smem, s>>>(g, (const double *)(SPREAD ? p->wtab : p->recg), p->bin_start,
+    const int nblocks = (SPREAD && g.nsplit > 1) ? g.nfull + g.nsplit * (ntY * ntZ - g.nfull) : nchunk * ntY * ntZ;
+    kern<<<(unsigned)nblocks, C::NT, smem, s>>>(g, (const double *)(SPREAD ? p->wtab : p->recg), p->bin_start,
                                                              (GR *)p->grid, (double *)p->uFpart);
     p->launches += 1;
     if (!SPREAD) {
