@@ -9,7 +9,7 @@
  * Follows Algorithm 2.1 step by step; every stage is a separate
  * function so each intermediate (u^N, H, H~hat, H~, u^F) can be compared on its own.
  * The two FFTs are NOT here: the Python wrapper
- * (oracle/__init__.py) calls numpy.fft.fftn / ifftn (a library primitive) between
+ * (oracle/__init__.py) calls scipy.fft.fftn / ifftn (pocketfft, a library primitive) between
  * se_p2g and se_scale and between se_scale and se_g2p.
  *
  * Discretisation (readings S4, S5, S8, S11 in DESIGN.md):
@@ -18,6 +18,15 @@
  *   dimension around the particle: anchor a_d = floor(x_d/h) - (P/2 - 1),
  *   offsets t_l = (a_d + l) h - x_d, l = 0..P-1, grid index (a_d + l) mod M.
  *   w_hat(k) = e^{-eta k^2/(8 xi^2)}.
+ *
+ * Second window (the paper's own, eq. (2.8)): truncated
+ * Kaiser-Bessel  w0(r) = I0(beta sqrt(1 - r^2/a_w^2)) / I0(beta) for |r| < a_w, else 0, with
+ * beta = 2.5 P, a_w = P h / 2, w(r) = w0(r1) w0(r2) w0(r3), same anchor and support points;
+ * either evaluated exactly (WIN_KB, own power series of I0) or by the piecewise polynomial
+ * of degree nu, one polynomial per bin of width h, Horner's rule (WIN_KBPOLY; the
+ * coefficients are made by oracle/__init__.py:kb_poly_coeffs).  The deconvolution uses the
+ * window's own transform w_hat0(k) (computed by quadrature in oracle/__init__.py:kb_what),
+ * c_w = 1.  Readings S18-S20 in DESIGN.md.
  */
 #include <math.h>
 #include <stdint.h>
@@ -153,17 +162,62 @@ int se_near_cells(int64_t N, const double *xw, const double *f, double L, double
     return 0;
 }
 
+/* window kinds; wpar = {a} (Gaussian), {beta, a_w} (KB), {nu, c[P][nu+1]} (KB polynomial) */
+#define WIN_GAUSS 0
+#define WIN_KB 1
+#define WIN_KBPOLY 2
+
+/* modified Bessel function I0(x) = sum_k (x^2/4)^k / (k!)^2  (all terms positive: no cancellation) */
+double se_bessel_i0(double x)
+{
+    double q = 0.25 * x * x, term = 1.0, sum = 1.0;
+    for (int k = 1; k < 500; ++k) {
+        term *= q / ((double)k * (double)k);
+        sum += term;
+        if (term < 1e-17 * sum) break;
+    }
+    return sum;
+}
+
+/* truncated Kaiser-Bessel window, eq. (2.8) */
+double se_kb_window(double r, double beta, double aw)
+{
+    double z = r / aw;
+    if (!(fabs(z) < 1.0)) return 0.0;
+    return se_bessel_i0(beta * sqrt(1.0 - z * z)) / se_bessel_i0(beta);
+}
+
+/* one window value at the physical offset t of support point l (reading S11) */
+static inline double window_value(double t, int l, double h, int P, int wkind, const double *wpar)
+{
+    if (wkind == WIN_GAUSS) return exp(-wpar[0] * t * t);
+    if (wkind == WIN_KB) return se_kb_window(t, wpar[0], wpar[1]);
+    /* WIN_KBPOLY: bin l is r in [(l - P/2) h, (l - P/2 + 1) h]; local variable s in [-1, 1] */
+    int nu = (int)wpar[0];
+    const double *c = wpar + 1 + (size_t)l * (nu + 1);
+    double s = 2.0 * (t / h - (double)(l - P / 2)) - 1.0;
+    double v = c[nu];
+    for (int k = nu - 1; k >= 0; --k) v = v * s + c[k];       /* Horner: nu multiply-adds */
+    return v;
+}
+
 /* 1-D window table of one particle along one dimension (step 4 of the O2 definition) */
-static inline void window_1d(double xd, double h, int M, int P, double a, double *W, int *idx)
+static inline void window_1d(double xd, double h, int M, int P, int wkind, const double *wpar, double *W, int *idx)
 {
     long anchor = (long)floor(xd / h) - (P / 2 - 1);
     for (int l = 0; l < P; ++l) {
         double t = (double)(anchor + l) * h - xd;
-        W[l] = exp(-a * t * t);
+        W[l] = window_value(t, l, h, P, wkind, wpar);
         long g = (anchor + l) % M;
         if (g < 0) g += M;
         idx[l] = (int)g;
     }
+}
+
+/* the P window values of one coordinate (tests) */
+void se_window_1d(double xd, double L, int M, int P, int wkind, const double *wpar, double *W, int *idx)
+{
+    window_1d(xd, L / M, M, P, wkind, wpar, W, idx);
 }
 
 /* ---- step 4: P2G, eq. (2.5) PAPER.md:80 ------------------------------------------
@@ -173,7 +227,7 @@ static inline void window_1d(double xd, double h, int M, int P, double a, double
  */
 #define PMAX 64
 void se_p2g(int64_t N, const double *xw, const double *f, double L, int M, int P,
-            double a, double cw, double *H)
+            int wkind, const double *wpar, double cw, double *H)
 {
     double h = L / M;
     size_t M3 = (size_t)M * M * M;
@@ -189,9 +243,9 @@ void se_p2g(int64_t N, const double *xw, const double *f, double L, int M, int P
             if (lq < 0) lq += M;
             if (lq >= P) continue;
             int hit = (int)lq;
-            window_1d(xw[3*n+0], h, M, P, a, W1, I1);
-            window_1d(xw[3*n+1], h, M, P, a, W2, I2);
-            window_1d(xw[3*n+2], h, M, P, a, W3, I3);
+            window_1d(xw[3*n+0], h, M, P, wkind, wpar, W1, I1);
+            window_1d(xw[3*n+1], h, M, P, wkind, wpar, W2, I2);
+            window_1d(xw[3*n+2], h, M, P, wkind, wpar, W3, I3);
             for (int l2 = 0; l2 < P; ++l2)
                 for (int l3 = 0; l3 < P; ++l3) {
                     double w = cw * W1[hit] * W2[l2] * W3[l3];
@@ -207,7 +261,7 @@ void se_p2g(int64_t N, const double *xw, const double *f, double L, int M, int P
 /* P2G evaluated one grid point at a time (gather form of the same sum): for sampled
  * grid indices gi (ns x 3) returns Hs (ns x 3 comps).  O(N) per sample. */
 void se_p2g_points(int64_t N, const double *xw, const double *f, double L, int M, int P,
-                   double a, double cw, int64_t ns, const int32_t *gi, double *Hs)
+                   int wkind, const double *wpar, double cw, int64_t ns, const int32_t *gi, double *Hs)
 {
     double h = L / M;
     #pragma omp parallel for schedule(dynamic, 1)
@@ -222,7 +276,7 @@ void se_p2g_points(int64_t N, const double *xw, const double *f, double L, int M
                 if (lq < 0) lq += M;
                 if (lq >= P) { ok = 0; break; }
                 double t = (double)(anchor + lq) * h - xw[3*n+d];
-                w *= exp(-a * t * t);
+                w *= window_value(t, (int)lq, h, P, wkind, wpar);
             }
             if (!ok) continue;
             acc[0] += w * f[3*n+0]; acc[1] += w * f[3*n+1]; acc[2] += w * f[3*n+2];
@@ -236,9 +290,12 @@ void se_p2g_points(int64_t N, const double *xw, const double *f, double L, int M
  * (G^F_hat / w_hat^2 with w_hat = e^{-eta k^2/8xi^2};  h^3 = P2G quadrature weight folded
  * in here, 1/V = Fourier-series normalisation, reading S1).  Zero for k = 0 (S2) and on
  * every Nyquist plane idx_d = M/2 when M is even (S8).
+ * what == NULL: the Gaussian window as above.  what != NULL (Kaiser-Bessel): what[i] is the 1-D window
+ * transform w_hat0 at the wavenumber of index i, w_hat(k) = w_hat0(k1) w_hat0(k2) w_hat0(k3), and the
+ * factor is e^{-k^2/4xi^2} / w_hat(k)^2, eq. (2.6) as printed.
  * in/out: 3 complex numbers as {re,im} pairs.
  */
-void se_scale_mode(int M, double L, double xi, double eta, const int *idx,
+void se_scale_mode(int M, double L, double xi, double eta, const double *what, const int *idx,
                    const double *in, double *out)
 {
     double k[3];
@@ -254,7 +311,13 @@ void se_scale_mode(int M, double L, double xi, double eta, const int *idx,
     double k2 = k[0]*k[0] + k[1]*k[1] + k[2]*k[2];
     double q4 = k2 / (4.0 * xi * xi);
     double h = L / M;
-    double s = (h*h*h / (L*L*L)) * 8.0 * PI / (k2*k2) * (1.0 + q4) * exp(-(1.0 - eta) * q4);
+    double dec;
+    if (what) {
+        double wh = what[idx[0]] * what[idx[1]] * what[idx[2]];
+        dec = exp(-q4) / (wh * wh);
+    } else
+        dec = exp(-(1.0 - eta) * q4);
+    double s = (h*h*h / (L*L*L)) * 8.0 * PI / (k2*k2) * (1.0 + q4) * dec;
     double kHr = k[0]*in[0] + k[1]*in[2] + k[2]*in[4];
     double kHi = k[0]*in[1] + k[1]*in[3] + k[2]*in[5];
     for (int c = 0; c < 3; ++c) {
@@ -264,7 +327,7 @@ void se_scale_mode(int M, double L, double xi, double eta, const int *idx,
 }
 
 /* whole spectrum, full complex-to-complex layout (3, M, M, M) of {re,im}, in place */
-void se_scale(int M, double L, double xi, double eta, double *Hhat)
+void se_scale(int M, double L, double xi, double eta, const double *what, double *Hhat)
 {
     size_t M3 = (size_t)M * M * M;
     #pragma omp parallel for schedule(static)
@@ -275,7 +338,7 @@ void se_scale(int M, double L, double xi, double eta, double *Hhat)
                 int idx[3] = {i, j, k};
                 double in[6], out[6];
                 for (int c = 0; c < 3; ++c) { in[2*c] = Hhat[2*(c*M3+g)]; in[2*c+1] = Hhat[2*(c*M3+g)+1]; }
-                se_scale_mode(M, L, xi, eta, idx, in, out);
+                se_scale_mode(M, L, xi, eta, what, idx, in, out);
                 for (int c = 0; c < 3; ++c) { Hhat[2*(c*M3+g)] = out[2*c]; Hhat[2*(c*M3+g)+1] = out[2*c+1]; }
             }
 }
@@ -284,7 +347,7 @@ void se_scale(int M, double L, double xi, double eta, double *Hhat)
  * u^F_{i,c} = h^3 c_w sum_{l1 l2 l3} W1 W2 W3 H~_c[i1,i2,i3]; same W, idx as P2G.
  * Ht is (3, M, M, M); targets are the nt positions in xt (wrapped).
  */
-void se_g2p(int64_t nt, const double *xt, double L, int M, int P, double a, double cw,
+void se_g2p(int64_t nt, const double *xt, double L, int M, int P, int wkind, const double *wpar, double cw,
             const double *Ht, double *uF)
 {
     double h = L / M;
@@ -293,9 +356,9 @@ void se_g2p(int64_t nt, const double *xt, double L, int M, int P, double a, doub
     for (int64_t n = 0; n < nt; ++n) {
         double W1[PMAX], W2[PMAX], W3[PMAX];
         int I1[PMAX], I2[PMAX], I3[PMAX];
-        window_1d(xt[3*n+0], h, M, P, a, W1, I1);
-        window_1d(xt[3*n+1], h, M, P, a, W2, I2);
-        window_1d(xt[3*n+2], h, M, P, a, W3, I3);
+        window_1d(xt[3*n+0], h, M, P, wkind, wpar, W1, I1);
+        window_1d(xt[3*n+1], h, M, P, wkind, wpar, W2, I2);
+        window_1d(xt[3*n+2], h, M, P, wkind, wpar, W3, I3);
         double acc[3] = {0, 0, 0};
         for (int l1 = 0; l1 < P; ++l1)
             for (int l2 = 0; l2 < P; ++l2)

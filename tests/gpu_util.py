@@ -13,6 +13,30 @@ def rel(a, b):
     return num / den
 
 
+def maxabs(a, b):
+    """max |a - b| over max |b|: the worst single element, next to the rel-L2 gate."""
+    a, b = np.asarray(a), np.asarray(b)
+    dt = np.complex128 if (np.iscomplexobj(a) or np.iscomplexobj(b)) else np.float64
+    den = float(np.max(np.abs(b.astype(dt)))) if b.size else 0.0
+    num = float(np.max(np.abs(a.astype(dt) - b.astype(dt)))) if b.size else 0.0
+    if den == 0.0:
+        return 0.0 if num == 0.0 else float("inf")
+    return num / den
+
+
+# gate on the worst element: MAXABS_FACTOR x the rel-L2 tolerance of the same array (a single element may sit
+# above the root-mean-square error; a wrong element is orders of magnitude above either)
+MAXABS_FACTOR = 10.0
+
+
+def gate(name, got, ref, tol):
+    """Assert rel-L2 <= tol and max-abs / max|ref| <= MAXABS_FACTOR tol; returns (rel, maxabs)."""
+    e, m = rel(got, ref), maxabs(got, ref)
+    assert e <= tol, (name, "rel-L2", e, tol)
+    assert m <= MAXABS_FACTOR * tol, (name, "max-abs", m, MAXABS_FACTOR * tol)
+    return e, m
+
+
 def run_stages(c, x, f):
     """Run every stage through se_eval_stage and return the intermediates as numpy (user order)."""
     import torch
