@@ -9,7 +9,10 @@ configs[2] (N = 1,048,576 uniform, fp64, 9 digits), the configuration SURVEY.md 
 fp64 headline that fits one GPU comfortably; `--config` selects another (1..5).
 Multi-GPU (`--gpus N` under torchrun): N independent replicas, no data-path collective
 (replicas only); value = particles all ranks processed / max-over-ranks time.
-`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample instead.
+The default run (config 3, one GPU) also carries `configs`: sub-results for config 5, config 4 and the same workloads with
+the paper's Kaiser-Bessel window, each with its own stage times and rooflines, and `peaks`: the FP64 / FP32 / HBM
+figures se_measure_peak measured on this device before the timed region.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the bench workload itself, one evaluation per step.
 """
 from __future__ import annotations
 
@@ -29,11 +32,16 @@ sys.path.insert(0, ROOT)
 
 METRIC = "particles/s, full Stokes SE sum"
 UNIT = "particles/s"
-# FP64 / FP32 FMA peak of one B200 from unit counts and clocks:
-# 148 SMs x 64 (128) FMA lanes x 2 flop x 1.965 GHz.  A register-only DFMA/FFMA chain measured
-# 36.7 / 72.0 TFLOP/s on this pool (profiles/r01b_mma_ws.md).
-ALU_PEAK_TFLOPS = {"fp64": 148 * 64 * 2 * 1.965e9 / 1e12, "fp32": 148 * 128 * 2 * 1.965e9 / 1e12}
-SAMPLE_CFG = 2          # the oracle's bounded sample: config 2 in full
+# Nominal FP64 / FP32 FMA peaks of one B200 from unit counts and clocks (148 SMs x 64 / 128 FMA lanes x 2 flop x
+# 1.965 GHz) and the fallback HBM figure of /opt/skills/guides/B200_PROFILING.md; used only when the measured ones
+# (se_measure_peak: register-only DFMA / DMMA / FFMA chains, run before the timed region) are unavailable.
+NOMINAL_TFLOPS = {"fp64": 148 * 64 * 2 * 1.965e9 / 1e12, "fp32": 148 * 128 * 2 * 1.965e9 / 1e12}
+# FP64 (FP32) arithmetic instructions K2 spends per in-range pair (DESIGN.md section 6 "K2"): the "alu" work of P2P
+P2P_INSTR_PER_PAIR = 64
+# sub-results of the default run (world size 1): (key, config, steps, plan overrides)
+SUB_RESULTS = [("cfg5", 5, 3, {}), ("cfg4", 4, 5, {}),
+               ("cfg3_kb_P12", 3, 5, {"window": "kb", "P": 12}), ("cfg5_kb_P12", 5, 3, {"window": "kb", "P": 12}),
+               ("cfg4_kb_P8", 4, 5, {"window": "kb", "P": 8})]
 
 
 def env_int(name, default):
@@ -92,59 +100,104 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def stage_flops_bytes(c, stage):
-    """Algorithmic work of one launch of a stage (DESIGN.md "Kernels": per-unit figure x units)."""
+def stage_work(c, P, stage, pairs):
+    """Algorithmic work of one launch of a stage (DESIGN.md section 6: per-unit figure x units)."""
     B = 8 if c.precision == "fp64" else 4
-    N, M, P = c.N, c.M, c.P
+    N, M = c.N, c.M
     nk = M * M * (M // 2 + 1)
     if stage in ("p2g", "g2p"):
         return {"bound": "alu", "work": 2.0 * 3 * P ** 3 * N, "unit": "TFLOP/s"}
+    if stage == "p2p" and pairs:
+        return {"bound": "alu", "work": 2.0 * P2P_INSTR_PER_PAIR * pairs, "unit": "TFLOP/s"}
     if stage == "scale":
         return {"bound": "hbm", "work": 12.0 * B * nk, "unit": "GB/s"}
     if stage in ("fft", "ifft"):
         return {"bound": "hbm", "work": 3.0 * (B * M ** 3 + 2 * B * nk), "unit": "GB/s"}
     if stage == "sort":
-        return {"bound": "hbm", "work": N * (6.0 * B * 3 + 3 * P * B + 40), "unit": "GB/s"}
+        # x, f read twice (binning; gather), two sorted copies and the FP32 filter copy written, index arrays,
+        # and the per-particle window records of the tensor-core sweep (8 bytes per entry in every precision)
+        return {"bound": "hbm", "work": N * (4.0 * 3 * B + 6.0 * B + 16 + 3 * B + 40 + 8.0 * (8 * P + 8)), "unit": "GB/s"}
     if stage == "sum":
         return {"bound": "hbm", "work": N * (12.0 * B + 8), "unit": "GB/s"}
     return None
 
 
-def oracle_sample():
-    """The bounded sample the CPU oracle is timed on (same dimensionless parameters as the workload)."""
-    from paper_2606_19059_b200 import workloads as W
-    c, x, f = W.make(SAMPLE_CFG)
-    desc = (f"config {SAMPLE_CFG} in full (N={c.N}, M={c.M}, P={c.P}: same xi*rc, pi*M/(2 xi L), P and "
-            f"neighbours per particle as config 3, 1/16 of its particles)")
-    return c, x, f, desc
+def gridding_hbm_bytes(c, P):
+    """Compulsory DRAM bytes of one gridding launch: the grid once plus the particles' records once."""
+    B = 8 if c.precision == "fp64" else 4
+    return 3.0 * B * c.M ** 3 + c.N * 8.0 * (4 * P + 4)
 
 
-def time_oracle_once(c, x, f):
+def load_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh_:
+            return json.load(fh_)
+    except (OSError, ValueError):
+        return {}
+
+
+def load_traffic():
+    """profiles/dram_traffic.csv: cfg, stage, dram bytes per launch (ncu --set full), source."""
+    out = {}
+    try:
+        with open(os.path.join(ROOT, "profiles", "dram_traffic.csv")) as fh_:
+            for ln in fh_:
+                p = ln.strip().split(",")
+                if len(p) >= 3 and not p[0].startswith("#"):
+                    try:
+                        out[(p[0], p[1])] = float(p[2])
+                    except ValueError:
+                        pass
+    except OSError:
+        pass
+    return out
+
+
+def measure_peaks(se):
+    """Register-only chains and a read+write stream on this device (se_measure_peak), before any timed region."""
+    out = {}
+    for key, which in (("fp64_tflops_measured", "fp64"), ("fp64_tensor_tflops_measured", "fp64_tensor"),
+                       ("fp32_tflops_measured", "fp32"), ("hbm_stream_tbs_measured", "hbm")):
+        try:
+            out[key] = se.measure_peak(which, 5)
+        except Exception as ex:                          # reported, never fatal
+            out[key] = None
+            out.setdefault("errors", []).append(f"{which}: {ex}")
+    return out
+
+
+def oracle_step(c, x, f):
+    """One evaluation of the CPU oracle, as it stands, on the workload itself; seconds and per-step timings."""
     import oracle
+    tm = {}
     t = time.perf_counter()
-    oracle.se_eval(x, f, c.L, c.xi, c.rc, c.M, c.P)
-    return time.perf_counter() - t
+    oracle.se_eval(x, f, c.L, c.xi, c.rc, c.M, c.P, timings=tm)
+    return time.perf_counter() - t, tm
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    """--impl reference: the CPU oracle on the host cores, one full evaluation of the bench workload per step
+    (rank 0 only).  At most one warm-up evaluation is made (an evaluation of config 3 takes ~12 s on 16 cores)."""
     if env_int("RANK", 0) != 0:
         return 0
     import oracle
     from paper_2606_19059_b200 import workloads as W
     oracle.build()
-    c, x, f, desc = oracle_sample()
-    wl = W.CONFIGS[args.config]
-    for _ in range(args.warmup):
-        time_oracle_once(c, x, f)
-    ts = [time_oracle_once(c, x, f) for _ in range(args.steps)]
+    c, x, f = W.make(args.config)
+    warm = min(args.warmup, 1)
+    for _ in range(warm):
+        oracle_step(c, x, f)
+    ts = [oracle_step(c, x, f)[0] for _ in range(args.steps)]
     total = sum(ts)
     val = c.N * args.steps / total
+    desc = (f"the bench workload itself, in full ({c.label}: every step is one oracle.se_eval over all N = {c.N} "
+            f"particles; {warm} warm-up evaluation(s) instead of {args.warmup})")
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "steps": args.steps, "warmup": warm, "ms_per_step": 1e3 * total / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": wl.label, "timed_on": desc},
+        "config": {"workload": c.label, "N": c.N, "L": c.L, "xi": c.xi, "rc": c.rc, "M": c.M, "P": c.P,
+                   "precision": c.precision},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle", "sample": desc},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -153,25 +206,20 @@ def run_reference(args):
     return 0
 
 
-def run_b200(args):
-    import torch
-    import torch.distributed as dist
-    import paper_2606_19059_b200 as se
-    from paper_2606_19059_b200 import replicas, workloads as W
+class Ctx:
+    """Process-wide state of one bench run: torch, ranks, peaks."""
+    pass
 
-    rank, world, local = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
-    se.lib()                                          # fail loudly if libse_b200.so is missing
-    torch.cuda.set_device(local)
-    distributed = world > 1
-    if distributed:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    c, x, f = W.make(args.config)
-    if rank > 0 and c.kind == "uniform":              # replicas: every rank its own seeded batch
+def bench_plan(ctx, cfg, steps, warmup, over, headline):
+    """Time one plan on config `cfg` (plan overrides `over`: window, P).  Returns the result dict; for the headline
+    also samples clocks around the timed regions."""
+    torch, se, W, replicas = ctx.torch, ctx.se, ctx.W, ctx.replicas
+    c, x, f = W.make(cfg)
+    if ctx.rank > 0 and c.kind == "uniform":              # replicas: every rank its own seeded batch
         x, f = (a.astype(W.np_dtype(c.precision))
-                for a in W.uniform_cloud(replicas.replica_seed(W.SEED_BASE + args.config, rank), c.N, c.L))
+                for a in W.uniform_cloud(replicas.replica_seed(W.SEED_BASE + cfg, ctx.rank), c.N, c.L))
+    window, P = over.get("window", "gaussian"), over.get("P", c.P)
     dt = torch.float64 if c.precision == "fp64" else torch.float32
     xh = torch.as_tensor(np.ascontiguousarray(x), dtype=dt).pin_memory()
     fh = torch.as_tensor(np.ascontiguousarray(f), dtype=dt).pin_memory()
@@ -180,150 +228,196 @@ def run_b200(args):
     ud = torch.empty_like(xd)
     stream = torch.cuda.current_stream()
 
+    plan = se.Plan(c.N, c.L, c.xi, c.rc, c.M, P, c.precision, window=window)
+    info = plan.info()
+    plan.set_profiling(True)                          # CUDA events around each stage, no host sync
+    for _ in range(max(warmup, 3)):
+        plan.eval(xd, fd, ud)
+    ctx.barrier()
+    cand, pairs = plan.count_pairs()                  # K2's work, counted once outside every timed region
+
+    sampler = None
+    if headline and ctx.rank == 0:
+        props = torch.cuda.get_device_properties(ctx.local)
+        sampler = ClockSampler("GPU-" + str(props.uuid))
+        time.sleep(0.3)
+    ctx.barrier()
+
+    # ---- device-resident timed region: exactly `steps` evaluations ----------------------------------------
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_wall0 = time.perf_counter()
+    ctx.barrier()
+    e0.record(stream)
+    for _ in range(steps):
+        plan.eval(xd, fd, ud)
+    e1.record(stream)
+    ctx.barrier()
+    ms_dev = ctx.max_over_ranks(e0.elapsed_time(e1))
+    # stage times: the events se_eval records on the same stream, averaged over `steps` more evaluations (outside the
+    # headline timing, same launches)
+    stage_acc = {k: 0.0 for k in se.STAGES}
+    for _ in range(steps):
+        plan.eval(xd, fd, ud)
+        for k, v in plan.stage_ms().items():
+            stage_acc[k] += v
+    launches = plan.launch_count() * steps
+    stage_ms = {k: v / steps for k, v in stage_acc.items()}
+
+    # ---- end to end through the host-buffer entry point ------------------------------------------------------
+    for _ in range(2):
+        plan.eval_host(xh, fh, uh)
+    ctx.barrier()
+    e0.record(stream)
+    for _ in range(steps):
+        plan.eval_host(xh, fh, uh)
+    e1.record(stream)
+    ctx.barrier()
+    t_wall1 = time.perf_counter()
+    ms_e2e = ctx.max_over_ranks(e0.elapsed_time(e1))
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    ok = bool(torch.isfinite(ud).all().item()) and bool(torch.isfinite(uh).all().item())
+    plan.destroy()
+    del xd, fd, ud, xh, fh, uh
+    torch.cuda.empty_cache()
+
+    B = 8 if c.precision == "fp64" else 4
+    world = ctx.world
+    pk = ctx.peaks
+    hbm_peak = float(ctx.file_peaks.get("hbm_gbs", 6650.0))
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs (copy)" if "hbm_gbs" in ctx.file_peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    # the FP64 datapath serves DFMA and DMMA alike: the measured peak is the better of the two chains
+    f64 = max([v for v in (pk.get("fp64_tflops_measured"), pk.get("fp64_tensor_tflops_measured")) if v] or [0.0])
+    f32 = pk.get("fp32_tflops_measured") or 0.0
+    alu = {"fp64": (f64, "measured: register-only DFMA / DMMA chain (se_measure_peak)") if f64 else
+           (NOMINAL_TFLOPS["fp64"], "nominal: 148 SM x 64 FMA/clk x 2 x 1.965 GHz"),
+           "fp32": (f32, "measured: register-only FFMA chain (se_measure_peak)") if f32 else
+           (NOMINAL_TFLOPS["fp32"], "nominal: 148 SM x 128 FMA/clk x 2 x 1.965 GHz")}
+    tag = "%d%s" % (cfg, "" if not over else "_" + window + str(P))
+    per_stage = {}
+    for st, ms in stage_ms.items():
+        w = stage_work(c, P, st, pairs)
+        if w is None or ms <= 0:
+            continue
+        r = {"bound": w["bound"], "unit": w["unit"], "ms": ms}
+        if w["bound"] == "alu":
+            r["achieved"] = w["work"] / (ms * 1e-3) / 1e12
+            # the survey's bound for a plan is the ALU pipe of its own precision; fp32 plans grid on
+            # the FP64 datapath (double records and accumulators), so that figure is given beside it
+            r["peak"], r["peak_source"] = alu[c.precision]
+            if st in ("p2g", "g2p"):
+                if c.precision == "fp32" and info.grid_mode == 2:
+                    r["frac_of_fp64_datapath"] = r["achieved"] / alu["fp64"][0]
+                r["hbm_gbs_on_compulsory_bytes"] = gridding_hbm_bytes(c, P) / (ms * 1e-3) / 1e9
+                r["hbm_frac_on_compulsory_bytes"] = r["hbm_gbs_on_compulsory_bytes"] / hbm_peak
+        else:
+            r["achieved"] = w["work"] / (ms * 1e-3) / 1e9
+            r["peak"], r["peak_source"] = hbm_peak, hbm_src
+        r["frac"] = r["achieved"] / r["peak"]
+        if r["bound"] == "hbm" and r["frac"] > 1.0:
+            r["note"] = ("above the copy figure of MEASURED_PEAKS.json; this device's read+write stream measured "
+                         "%.0f GB/s (se_measure_peak)" % (1e3 * (pk.get("hbm_stream_tbs_measured") or 0.0)))
+        r["traffic"] = ctx.traffic.get((tag, st))
+        per_stage[st] = r
+    own = [s_ for s_ in ("p2p", "p2g", "g2p", "scale", "sort", "sum") if s_ in per_stage]
+    dom = max(own, key=lambda s_: stage_ms[s_])
+    roof = dict(per_stage[dom])
+    roof["kernel"] = {"p2p": "k_p2p (K2)", "p2g": "k_mma<spread> (K3)", "g2p": "k_mma<gather> (K5)",
+                      "scale": "k_scale (K4)", "sort": "K1", "sum": "K6"}[dom]
+    total_stage = sum(stage_ms.values())
+    res = {
+        "workload": c.label + ("" if not over else f" [{window} window, P={P}]"),
+        "value": world * c.N * steps / (ms_dev * 1e-3), "unit": UNIT, "steps": steps,
+        "ms_per_step": ms_dev / steps,
+        "e2e": {"value": world * c.N * steps / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e / steps,
+                "h2d_bytes_per_step": 2 * 3 * c.N * B, "d2h_bytes_per_step": 3 * c.N * B},
+        "gpu_launches": launches, "roofline": roof,
+        "stages_ms": {k: round(v, 4) for k, v in stage_ms.items()},
+        "stages_roofline": {k: {kk: (round(vv, 4) if isinstance(vv, float) else vv) for kk, vv in v.items()
+                                if kk not in ("ms", "peak_source")} for k, v in per_stage.items()},
+        "p2p_pairs": {"in_range": pairs, "candidates": cand, "in_range_per_s": pairs / (stage_ms["p2p"] * 1e-3)
+                      if stage_ms["p2p"] > 0 else None},
+        "value_excluding_fft": world * c.N / ((total_stage - stage_ms["fft"] - stage_ms["ifft"]) * 1e-3),
+        "finite": ok,
+    }
+    cfgd = {"workload": res["workload"], "N": c.N, "L": c.L, "xi": c.xi, "rc": c.rc, "M": c.M, "P": P,
+            "precision": c.precision, "window": window, "eta": info.eta, "ncell": info.ncell,
+            "gridding": ("FP64 tensor-core sweep (double records and accumulators%s)" %
+                         (", float grid" if c.precision == "fp32" else "")) if info.grid_mode == 2
+            else "generic tile kernel in the plan's precision",
+            "parallelism": "replicas x%d" % world,
+            "l2": "no explicit flush: every step streams the %.2f GB plan workspace (grid %.2f GB + spectrum %.2f GB), "
+                  "far larger than the 126 MB L2" % (info.workspace_bytes / 1e9, 3 * B * c.M ** 3 / 1e9,
+                                                      6 * B * info.nmodes / 1e9)}
+    return res, cfgd, clocks, c
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_19059_b200 as se
+    from paper_2606_19059_b200 import replicas, workloads as W
+
+    ctx = Ctx()
+    ctx.torch, ctx.se, ctx.W, ctx.replicas = torch, se, W, replicas
+    ctx.rank, ctx.world, ctx.local = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    se.lib()                                          # fail loudly if libse_b200.so is missing
+    torch.cuda.set_device(ctx.local)
+    distributed = ctx.world > 1
+    if distributed:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", ctx.local))
+
     def barrier():
         if distributed:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(v):
-        return replicas.aggregate(0.0, v, device="cuda")[1]
-
-    plan = se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P, c.precision)
-    info = plan.info()
-    plan.set_profiling(True)                          # CUDA events around each stage, no host sync
-    for _ in range(max(args.warmup, 3)):
-        plan.eval(xd, fd, ud)
+    ctx.barrier = barrier
+    ctx.max_over_ranks = lambda v: replicas.aggregate(0.0, v, device="cuda")[1]
+    ctx.file_peaks, ctx.traffic = load_peaks(), load_traffic()
+    ctx.peaks = measure_peaks(se)
     barrier()
 
-    props = torch.cuda.get_device_properties(local)
-    sampler = ClockSampler("GPU-" + str(props.uuid)) if rank == 0 else None
-    time.sleep(0.3 if rank == 0 else 0.0)
-    barrier()
-
-    # ---- device-resident timed region: exactly K steps ---------------------------------
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    stage_acc = {k: 0.0 for k in se.STAGES}
-    launches = 0
-    t_wall0 = time.perf_counter()
-    barrier()
-    e0.record(stream)
-    for _ in range(args.steps):
-        plan.eval(xd, fd, ud)
-    e1.record(stream)
-    barrier()
-    ms_dev = max_over_ranks(e0.elapsed_time(e1))
-    # stage times of the LAST timed step come from the events se_eval recorded on the same stream;
-    # re-run K profiled steps to average them (outside the headline timing, same launches).
-    for _ in range(args.steps):
-        plan.eval(xd, fd, ud)
-        sm = plan.stage_ms()
-        for k, v in sm.items():
-            stage_acc[k] += v
-    launches = plan.launch_count() * args.steps
-    stage_ms = {k: v / args.steps for k, v in stage_acc.items()}
-
-    # ---- end to end through the host-buffer entry point ------------------------------------
-    for _ in range(2):
-        plan.eval_host(xh, fh, uh)
-    barrier()
-    e0.record(stream)
-    for _ in range(args.steps):
-        plan.eval_host(xh, fh, uh)
-    e1.record(stream)
-    barrier()
-    t_wall1 = time.perf_counter()
-    ms_e2e = max_over_ranks(e0.elapsed_time(e1))
-    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
-
-    ok = bool(torch.isfinite(ud).all().item()) and bool(torch.isfinite(uh).all().item())
+    steps, warmup = args.steps, max(args.warmup, 3)
+    res, cfgd, clocks, c = bench_plan(ctx, args.config, steps, warmup, {}, headline=True)
+    subs = {}
+    if ctx.world == 1 and not args.no_sub and args.config == 3:
+        for key, cfg, k, over in SUB_RESULTS:
+            try:
+                r, cd, _, _ = bench_plan(ctx, cfg, k, 3, over, headline=False)
+                r["config"] = {kk: cd[kk] for kk in ("N", "xi", "rc", "M", "P", "precision", "window", "gridding")}
+                subs[key] = r
+            except Exception as ex:                      # a sub-result must never cost the headline
+                subs[key] = {"error": repr(ex)}
     if distributed:
         dist.barrier()
-    if rank != 0:
-        plan.destroy()
+    if ctx.rank != 0:
         if distributed:
             dist.destroy_process_group()
         return 0
 
-    B = 8 if c.precision == "fp64" else 4
-    value = world * c.N * args.steps / (ms_dev * 1e-3)
-    e2e = world * c.N * args.steps / (ms_e2e * 1e-3)
-
-    # ---- roofline of every stage; the headline object is the dominant kernel of ours -------
-    peaks = {}
-    try:
-        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh_:
-            peaks = json.load(fh_)
-    except OSError:
-        pass
-    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-    hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s"
-    traffic = {}
-    try:
-        with open(os.path.join(ROOT, "profiles", "dram_traffic.csv")) as fh_:
-            for ln in fh_:
-                p = ln.strip().split(",")
-                if len(p) >= 3 and p[0] == str(args.config):
-                    traffic[p[1]] = float(p[2])
-    except OSError:
-        pass
-    per_stage = {}
-    for st, ms in stage_ms.items():
-        w = stage_flops_bytes(c, st)
-        if w is None or ms <= 0:
-            continue
-        if w["bound"] == "alu":
-            ach = w["work"] / (ms * 1e-3) / 1e12
-            # fp32 plans grid on the FP64 tensor path too (double records and accumulators, float grid)
-            peak = ALU_PEAK_TFLOPS["fp64" if info.grid_mode == 2 else c.precision]
-        else:
-            ach = w["work"] / (ms * 1e-3) / 1e9
-            peak = hbm_peak
-        per_stage[st] = {"bound": w["bound"], "achieved": ach, "peak": peak, "unit": w["unit"],
-                         "frac": ach / peak, "ms": ms, "traffic": traffic.get(st)}
-    own = [s for s in ("p2g", "g2p", "scale", "sort", "sum") if s in per_stage]
-    dom = max(own, key=lambda s: stage_ms[s])
-    roof = dict(per_stage[dom])
-    roof["kernel"] = {"p2g": "k_p2g (K3)", "g2p": "k_g2p (K5)", "scale": "k_scale (K4)", "sort": "K1", "sum": "K6"}[dom]
-    roof["peak_source"] = ("unit counts x clock: 148 SM x %d FMA/clk x 2 x 1.965 GHz (DESIGN.md)" %
-                           (64 if (c.precision == "fp64" or info.grid_mode == 2) else 128)) if roof["bound"] == "alu" else hbm_src
-    # P2P: plain-ALU kernel whose work is data dependent -- reported as in-range pairs/s
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms_dev / args.steps, "higher_is_better": True,
+        "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": ctx.world, "steps": steps,
+        "warmup": warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64" if c.precision == "fp64" else "f32",
-        "data": "synthetic",
-        "config": {"workload": c.label, "N": c.N, "L": c.L, "xi": c.xi, "rc": c.rc, "M": c.M, "P": c.P,
-                   "precision": c.precision, "eta": info.eta, "ncell": info.ncell,
-                   "gridding": ("FP64 tensor-core sweep (double records and accumulators%s)" %
-                                (", float grid" if c.precision == "fp32" else "")) if info.grid_mode == 2
-                   else "generic tile kernel in the plan's precision",
-                   "parallelism": "replicas x%d" % world,
-                   "l2": "no explicit flush: every step streams the %.2f GB plan workspace (grid %.2f GB + "
-                         "spectrum %.2f GB), far larger than the 126 MB L2" %
-                         (info.workspace_bytes / 1e9, 3 * B * c.M ** 3 / 1e9, 6 * B * info.nmodes / 1e9)},
-        "e2e": {"value": e2e, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
-                "h2d_bytes_per_step": 2 * 3 * c.N * B, "d2h_bytes_per_step": 3 * c.N * B},
-        "gpu_launches": launches,
-        "clocks": clocks,
-        "roofline": roof,
-        "stages_ms": {k: round(v, 4) for k, v in stage_ms.items()},
-        "stages_roofline": {k: {"bound": v["bound"], "frac": round(v["frac"], 4), "achieved": round(v["achieved"], 2),
-                                "unit": v["unit"]} for k, v in per_stage.items()},
-        "value_excluding_fft": world * c.N / ((sum(stage_ms.values()) - stage_ms["fft"] - stage_ms["ifft"]) * 1e-3),
-        "finite": ok,
+        "data": "synthetic", "config": cfgd, "e2e": res["e2e"], "gpu_launches": res["gpu_launches"],
+        "clocks": clocks, "roofline": res["roofline"], "stages_ms": res["stages_ms"],
+        "stages_roofline": res["stages_roofline"], "p2p_pairs": res["p2p_pairs"],
+        "value_excluding_fft": res["value_excluding_fft"], "finite": res["finite"],
+        "peaks": dict(ctx.peaks, hbm_gbs_file=ctx.file_peaks.get("hbm_gbs"),
+                      fp64_tflops_nominal=NOMINAL_TFLOPS["fp64"], fp32_tflops_nominal=NOMINAL_TFLOPS["fp32"]),
+        "configs": subs,
     }
-    plan.destroy()
-    if world == 1 and not args.no_cpu_baseline:
+    if ctx.world == 1 and not args.no_cpu_baseline:
         import oracle
+        from paper_2606_19059_b200 import workloads as W2
         oracle.build()
-        sc, sx, sf, desc = oracle_sample()
-        t = time_oracle_once(sc, sx, sf)
-        reps = 1
-        while t < 8.0 and reps < 8:                    # aim at ~10-30 s of CPU work in total
-            t += time_oracle_once(sc, sx, sf)
-            reps += 1
-        line["cpu_baseline"] = {"value": sc.N * reps / t, "unit": UNIT, "cores": oracle.n_threads(),
-                                "kind": "oracle", "sample": desc + f", {reps} run(s), {t:.1f} s"}
+        oc, ox, of = W2.make(args.config)
+        t, tm = oracle_step(oc, ox, of)
+        line["cpu_baseline"] = {"value": oc.N / t, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
+                                "sample": f"the bench workload itself, in full ({oc.label}), one evaluation, {t:.1f} s",
+                                "stages_s": {k: round(v, 2) for k, v in tm.items()}}
     else:
         line["cpu_baseline"] = None
     print(json.dumps(line), flush=True)
@@ -340,15 +434,13 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sub", action="store_true", help="skip the sub-results (configs 4, 5, Kaiser-Bessel variants)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     world = env_int("WORLD_SIZE", 1)
-    if world != args.gpus:
-        if args.gpus == 1 and world > 1:
-            pass
-        elif world == 1 and args.gpus > 1:
-            raise SystemExit("bench.py: --gpus %d needs torchrun with --nproc-per-node %d" % (args.gpus, args.gpus))
+    if world == 1 and args.gpus > 1:
+        raise SystemExit("bench.py: --gpus %d needs torchrun with --nproc-per-node %d" % (args.gpus, args.gpus))
     return run_b200(args)
 
 

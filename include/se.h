@@ -6,9 +6,12 @@
  * (eq. (2.1)) with the Hasimoto split G = G^N + G^F
  * (eq. (2.3), eq. (2.4b)) by the spectral Ewald method
  * (Algorithm 2.1): P2P + P2G + FFT + CNV + IFFT + G2P + SUM, with a
- * Gaussian window over P^3 grid points (reading S4).  Targets = sources; the
- * i = j, p = 0 pair is excluded and the self term -(4 xi/sqrt(pi)) f_i is added
- * (reading S3); the k = 0 mode is dropped (reading S2); G carries no 1/(8 pi mu).
+ * Gaussian window over P^3 grid points (reading S4) or the paper's truncated
+ * Kaiser-Bessel window in piecewise-polynomial form (eq. (2.8),
+ * PAPER.md:421-427; readings S18-S20).  Targets = sources by default: the i = j, p = 0 pair
+ * is excluded and the self term -(4 xi/sqrt(pi)) f_i is added (reading S3); a plan may
+ * instead carry its own N_t target points (eq. (1.1)/(2.1)).
+ * The k = 0 mode is dropped (reading S2); G carries no 1/(8 pi mu).
  *
  * Conventions
  *   - All x, f, u arrays are N x 3, row-major (AoS), in the plan's precision
@@ -19,14 +22,16 @@
  *     OVERWRITES u.  A plan may be evaluated any number of times with new x, f.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
  *   - A plan is bound to the CUDA device current at se_plan_create and is not
- *     thread-safe.
+ *     thread-safe; every later call on it must be made with that device current
+ *     (SE_EINVAL otherwise).
  *   - Every entry point returns a status; nothing aborts or throws.  NaN/Inf inputs give
  *     unspecified values but never out-of-bounds accesses.
  *   - There is no CPU fallback: without a CUDA device se_plan_create returns SE_ECUDA.
  *   - Environment variables read at se_plan_create (experiments and tests only; results do not change beyond
  *     rounding order): SE_GRID_MODE = tile (force the generic gridding kernel; default: the FP64 tensor-core
- *     sweep for fp64 plans with P = 16, 24 and fp32 plans with P = 12, else the generic tile kernel), SE_NCHUNK and
- *     SE_NCHUNK_G2P (x-chunks of K3 / K5), SE_OVERLAP = 1 (K2 on a side stream next to the FFT stages).
+ *     sweep for fp64 plans with P = 8, 12, 16, 24 and fp32 plans with P = 8, 12, else the generic tile kernel),
+ *     SE_NCHUNK and SE_NCHUNK_G2P (x-chunks of K3 / K5), SE_OVERLAP = 1 (K2 on a side stream next to the FFT
+ *     stages).
  */
 #ifndef SE_B200_H
 #define SE_B200_H
@@ -41,6 +46,16 @@ extern "C" {
 typedef struct se_plan se_plan;                      /* opaque, owned by the library */
 
 typedef enum { SE_FP64 = 0, SE_FP32 = 1 } se_precision;
+
+/* Window of the P2G / G2P steps.
+ *   SE_WINDOW_GAUSSIAN       w(r) = (a/pi)^{3/2} e^{-a r^2}, a = 2 xi^2/eta, eta = (P h xi/m)^2, m = 0.95 sqrt(pi P)
+ *                            (the "classic" window the paper names at PAPER.md:103; reading S4); deconvolved with
+ *                            w_hat(k) = e^{-eta k^2/8 xi^2}.
+ *   SE_WINDOW_KAISER_BESSEL  w0(r) = I0(beta sqrt(1 - r^2/a_w^2))/I0(beta), |r| < a_w, beta = 2.5 P, a_w = P h/2
+ *                            (eq. (2.8)), evaluated as one polynomial of degree nu = min(P + 3, 13) per
+ *                            bin of width h by Horner's rule (reading S19), deconvolved with its
+ *                            closed-form transform (reading S20). */
+typedef enum { SE_WINDOW_GAUSSIAN = 0, SE_WINDOW_KAISER_BESSEL = 1 } se_window;
 
 typedef enum {
     SE_OK = 0,
@@ -72,10 +87,14 @@ enum {
     SE_BUF_PERM_NEAR = 4, /* int32[N]: sorted position -> user index, near-cell order              */
     SE_BUF_PERM_GRID = 5, /* int32[N]: sorted position -> user index, grid-bin order               */
     SE_BUF_CELL_START = 6,/* int32[ncell^3 + 1]: CSR offsets of the near cells                     */
-    SE_BUF_BIN_START = 7, /* int32[nbins_total + 1]: CSR offsets of the grid bins.  Mode 0: bins of 8^3 grid
-                             cells, key (bx, by, bz); mode 1: key (base plane ix, by/4, bz/4)               */
+    SE_BUF_BIN_START = 7, /* int32[nbins_total + 1]: CSR offsets of the grid bins.  grid_mode 0: bins of 8^3 grid
+                             cells, key (bx, by, bz); grid_mode 2: key (anchor plane a_x, a_z / 8, a_y)     */
     SE_NBUFS = 8
 };
+/* For plans with their own targets (Nt > 0) SE_BUF_UN / SE_BUF_UF hold Nt x 3 reals in the TARGETS' near / grid
+ * order and SE_BUF_PERM_* / SE_BUF_*_START describe the SOURCES; add SE_BUF_TARGETS to a PERM / START id to read
+ * the target set's array instead. */
+enum { SE_BUF_TARGETS = 16 };
 
 typedef struct {
     int64_t N;
@@ -89,11 +108,26 @@ typedef struct {
     int ncell;           /* near cells per dimension, floor(L/rc)          (reading S7)  */
     int nbin;            /* grid bins per dimension: ceil(M/8)                          */
     int grid_mode;       /* gridding kernels: 0 = tile-stationary (any even P), 2 = FP64 tensor-core sweep */
-    int nbins_total;     /* entries of SE_BUF_BIN_START minus 1: nbin^3 (mode 0), M * nbin^2 (mode 1)      */
+    int nbins_total;     /* entries of SE_BUF_BIN_START minus 1: nbin^3 (mode 0), M * nbin * M (mode 2)    */
     int nchunk;          /* tensor-core sweep: chunks along x (P2G)                      */
     int64_t nmodes;      /* M * M * (M/2+1) stored modes per component                   */
     size_t workspace_bytes; /* device memory owned by the plan (incl. cuFFT work area)   */
+    int64_t Nt;          /* targets (0: the targets are the sources)                     */
+    int window;          /* se_window                                                    */
+    int nu;              /* Kaiser-Bessel: degree of the piecewise polynomial            */
+    double kb_beta;      /* Kaiser-Bessel: beta = 2.5 P ; a_w = P h / 2                  */
 } se_info;
+
+/* Everything se_plan_create takes, plus the window and an optional separate target count. */
+typedef struct {
+    int64_t N;           /* source points                                                */
+    int64_t Nt;          /* target points; 0 = the targets are the sources (self term added, se_eval);
+                            > 0 = own targets (no self term, se_eval_targets)            */
+    double L, xi, rc;
+    int M, P;
+    int precision;       /* se_precision */
+    int window;          /* se_window    */
+} se_plan_desc;
 
 /*
  * Create a plan.  N particles in the periodic cube [0,L)^3, split parameter xi,
@@ -105,13 +139,26 @@ typedef struct {
 se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double rc,
                          int M, int P, se_precision prec);
 
-/* Full evaluation, all stages; x, f, u are device pointers (N x 3). */
+/* Same with a descriptor: Gaussian or Kaiser-Bessel window (for which cw = 1 and eta, m, a are reported as 0),
+ * optional separate targets.  Kaiser-Bessel needs 2 <= P <= 16 as well. */
+se_status se_plan_create_ex(se_plan **out, const se_plan_desc *desc);
+
+/* Full evaluation, all stages; x, f, u are device pointers (N x 3).  Plans with Nt = 0 only. */
 se_status se_eval(se_plan *p, const void *x, const void *f, void *u, void *stream);
 
 /*
+ * Plans with Nt > 0: u_t(x_i) = sum_j sum_p G(x_i - y_j + p) f_j at the Nt targets xt (Nt x 3, device) from the
+ * N sources xs, f (N x 3, device); ut is Nt x 3 (eq. (1.1)).  No self term.  A target that coincides
+ * with a source skips that pair in the near sum only (r = 0 is never evaluated); its smooth far part
+ * stays.  The per-stage hook se_eval_stage takes xt through se_set_targets.
+ */
+se_status se_eval_targets(se_plan *p, const void *xs, const void *f, const void *xt, void *ut, void *stream);
+
+/*
  * Same, with HOST buffers (pinned or pageable): copies x, f host->device into plan-owned
- * staging buffers, runs se_eval, copies u device->host, all asynchronously on `stream`
- * (the caller synchronises the stream before reading u_host).
+ * staging buffers (allocated at plan creation like all other workspace), runs se_eval, copies u
+ * device->host, all asynchronously on `stream` (the caller synchronises the stream before
+ * reading u_host).  Plans with Nt = 0 only.
  */
 se_status se_eval_host(se_plan *p, const void *x_host, const void *f_host, void *u_host,
                        void *stream);
@@ -132,6 +179,9 @@ se_status se_plan_info(const se_plan *p, se_info *out);
 se_status se_eval_stage(se_plan *p, int stage, const void *x, const void *f, void *u,
                         void *stream);
 
+/* Plans with Nt > 0: the target positions (Nt x 3, device) the next se_eval_stage(SE_STAGE_SORT) bins. */
+se_status se_set_targets(se_plan *p, const void *xt);
+
 /* Copy an internal buffer to / from caller DEVICE memory (`bytes` must equal its size,
  * obtainable with dst == NULL: *size_out is set and nothing is copied). */
 se_status se_buffer_read(se_plan *p, int which, void *dst, size_t bytes, size_t *size_out,
@@ -149,6 +199,47 @@ se_status se_stage_ms(se_plan *p, float ms[SE_NSTAGES]);
 /* Number of this library's own kernel launches issued by the last se_eval (cuFFT's are
  * not counted). */
 se_status se_last_launch_count(const se_plan *p, int *count);
+
+/* Benchmark diagnostics, not on the evaluation path: over the point sets of the last se_eval / SE_STAGE_SORT, the number
+ * of (target, source) candidates in the 27 colleague cells and of pairs with 0 < r <= rc, counted in FP32
+ * cell-relative coordinates (a pair within ~1e-6 rc of the cutoff may fall on either side).  bench.py rates K2 by
+ * in-range pairs per second with them.  Synchronises the device. */
+se_status se_count_pairs(se_plan *p, int64_t *candidates, int64_t *in_range);
+
+/* ---- parameter selection from a tolerance (section 2.4, eq. (2.9)) ------- */
+
+typedef struct {
+    double rc, xi;       /* cutoff and split parameter                                    */
+    int M, P;            /* grid points per dimension (even, 2^a 3^b 5^c 7^d), window support */
+    double EN, EF, Ew;   /* the three terms of eq. (2.9) at the chosen parameters          */
+    double s;            /* mean points per near cell, N rc^3 / L^3                        */
+    double model_ms;     /* the stage-time model's estimate for one evaluation on a B200   */
+} se_params;
+
+/*
+ * HOST ONLY, no CUDA call: choose (rc, xi, M, P) for N points in [0,L)^3 so that each term of the error
+ * estimate (2.9) is below eps/3 and the modelled time of Algorithm 2.1 is least
+ * (min over rc of T(rc) subject to E_rms <= eps).  eps is the absolute RMS error for
+ * sum_j |f_j|^2 = 1 in the unit box, as in the paper; E^N and E^F are (2.9)'s; E^w, whose constant C(xi) the paper
+ * does not print, is the window's aliasing + truncation error at the chosen h and xi (reading S21).  P is rounded up
+ * to a support the tensor-core gridding kernels are built for.  SE_EINVAL if N < 1, L <= 0, eps outside
+ * (1e-15, 1e-1), or no admissible choice exists.
+ */
+se_status se_select_params(int64_t N, double L, double eps, se_window window, se_precision prec, se_params *out);
+
+/* se_select_params followed by se_plan_create_ex (Nt as in se_plan_desc); *chosen (optional) receives the choice. */
+se_status se_plan_create_tol(se_plan **out, int64_t N, int64_t Nt, double L, double eps, se_window window,
+                             se_precision prec, se_params *chosen);
+
+/* ---- measured arithmetic peaks (bench.py's roofline denominators) ------------------------------- */
+
+/*
+ * Time register-only dependent chains on the current device: which = 0 FP64 DFMA, 1 FP64 tensor op
+ * (mma.sync m8n8k4 f64), 2 FP32 FFMA: *tflops receives 2 x FMA / s (in TFLOP/s) of the best of `reps` launches.
+ * which = 3: an in-place streaming pass over 2 GiB, every 16 bytes read and written once (the access pattern of K4):
+ * *tflops receives (bytes read + written) / s in TB/s.  Allocates and frees its own buffers; synchronises the device.
+ */
+se_status se_measure_peak(int which, int reps, double *tflops);
 
 #ifdef __cplusplus
 }

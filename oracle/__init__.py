@@ -139,6 +139,18 @@ def near_brute(xw, f, L, xi, rc, targets=None):
     return u
 
 
+def near_targets(xw, f, xt, L, xi, rc):
+    """u^N at separate (wrapped) target positions xt from the sources (xw, f): plain loop, 27 images."""
+    lib = _load()
+    xw, xp = _d(xw)
+    f, fp = _d(f)
+    xt, tp = _d(xt)
+    u = np.zeros_like(xt)
+    lib.se_near_targets(C.c_int64(xw.shape[0]), xp, fp, C.c_int64(xt.shape[0]), tp, C.c_double(L), C.c_double(xi),
+                        C.c_double(rc), u.ctypes.data_as(C.POINTER(C.c_double)))
+    return u
+
+
 def near_cells(xw, f, L, xi, rc):
     lib = _load()
     xw, xp = _d(xw)
@@ -363,4 +375,22 @@ def se_eval(x, f, L, xi, rc, M, P, keep=False, near="auto", timings=None, window
     out["uN"] = uN
     out["xw"] = xw
     out["u"] = se_sum(uN, out["uF"], f, xi)
+    return out
+
+
+def se_eval_targets(xs, f, xt, L, xi, rc, M, P, keep=False, window="gaussian"):
+    """SE oracle with separate targets (eq. (1.1)): u(x_i) = sum_j sum_p G(x_i - y_j + p) f_j at the
+    targets xt; no self term.  Near: plain loop; far: the sources' grid (steps 4-7) gathered at the targets (step 8)."""
+    xs = np.asarray(xs, dtype=np.float64)
+    f = np.asarray(f, dtype=np.float64)
+    xt = np.asarray(xt, dtype=np.float64)
+    xw, tw = wrap(xs, L), wrap(xt, L)
+    uN = near_targets(xw, f, tw, L, xi, rc)
+    H = p2g(xw, f, L, xi, M, P, window)
+    Hs = scale(_fft.fftn(H, axes=(1, 2, 3), workers=n_threads()), L, xi, M, P, window)
+    Ht = np.ascontiguousarray(_fft.ifftn(Hs, axes=(1, 2, 3), workers=n_threads()).real) * float(M) ** 3
+    uF = g2p(tw, Ht, L, xi, M, P, window)
+    out = dict(u=uN + uF, uN=uN, uF=uF, xw=xw, tw=tw)
+    if keep:
+        out.update(H=H, Hs=Hs, Ht=Ht)
     return out

@@ -104,6 +104,30 @@ void se_near_brute(int64_t N, const double *xw, const double *f, double L, doubl
     }
 }
 
+/* ---- step 3 for separate targets (eq. (1.1)/(2.2)): nt target positions xt (wrapped),
+ * N sources xw, plain loop over all sources and the 27 nearest images; r = 0 is skipped.
+ */
+void se_near_targets(int64_t N, const double *xw, const double *f, int64_t nt, const double *xt,
+                     double L, double xi, double rc, double *uN)
+{
+    double rc2 = rc * rc;
+    #pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t t = 0; t < nt; ++t) {
+        double acc[3] = {0, 0, 0};
+        for (int64_t j = 0; j < N; ++j)
+            for (int px = -1; px <= 1; ++px)
+            for (int py = -1; py <= 1; ++py)
+            for (int pz = -1; pz <= 1; ++pz) {
+                double rx = xt[3*t+0] - xw[3*j+0] + px * L;
+                double ry = xt[3*t+1] - xw[3*j+1] + py * L;
+                double rz = xt[3*t+2] - xw[3*j+2] + pz * L;
+                double r2 = rx*rx + ry*ry + rz*rz;
+                if (r2 > 0.0 && r2 <= rc2) near_pair(rx, ry, rz, r2, xi, f + 3*j, acc);
+            }
+        uN[3*t+0] = acc[0]; uN[3*t+1] = acc[1]; uN[3*t+2] = acc[2];
+    }
+}
+
 /* ---- step 3 (variant B): near field with a cell list: cells of width
  * L/ncell >= rc, ncell = floor(L/rc) (reading S7), 27 colleague cells with periodic
  * shifts.  Needs ncell >= 3.  Same pair arithmetic as variant A; cross-checked in tests.

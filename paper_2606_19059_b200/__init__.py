@@ -14,6 +14,9 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libse_b200.so"
 
 SE_FP64, SE_FP32 = 0, 1
+SE_WINDOW_GAUSSIAN, SE_WINDOW_KAISER_BESSEL = 0, 1
+WINDOWS = {"gaussian": SE_WINDOW_GAUSSIAN, "kb": SE_WINDOW_KAISER_BESSEL}
+SE_BUF_TARGETS = 16
 STAGES = ("sort", "p2p", "p2g", "fft", "scale", "ifft", "g2p", "sum")
 (SE_STAGE_SORT, SE_STAGE_P2P, SE_STAGE_P2G, SE_STAGE_FFT, SE_STAGE_SCALE, SE_STAGE_IFFT,
  SE_STAGE_G2P, SE_STAGE_SUM) = range(8)
@@ -21,9 +24,10 @@ SE_NSTAGES = 8
 (SE_BUF_UN, SE_BUF_UF, SE_BUF_GRID, SE_BUF_SPEC, SE_BUF_PERM_NEAR, SE_BUF_PERM_GRID,
  SE_BUF_CELL_START, SE_BUF_BIN_START) = range(8)
 
-EXPORTS = ("se_plan_create", "se_eval", "se_eval_host", "se_plan_destroy", "se_strerror",
+EXPORTS = ("se_plan_create", "se_plan_create_ex", "se_plan_create_tol", "se_select_params", "se_eval",
+           "se_eval_targets", "se_set_targets", "se_eval_host", "se_plan_destroy", "se_strerror",
            "se_plan_info", "se_eval_stage", "se_buffer_read", "se_buffer_write",
-           "se_set_profiling", "se_stage_ms", "se_last_launch_count")
+           "se_set_profiling", "se_stage_ms", "se_last_launch_count", "se_measure_peak", "se_count_pairs")
 
 
 class SeInfo(C.Structure):
@@ -32,7 +36,19 @@ class SeInfo(C.Structure):
                 ("m", C.c_double), ("eta", C.c_double), ("a", C.c_double), ("cw", C.c_double),
                 ("ncell", C.c_int), ("nbin", C.c_int), ("grid_mode", C.c_int), ("nbins_total", C.c_int),
                 ("nchunk", C.c_int), ("nmodes", C.c_int64),
-                ("workspace_bytes", C.c_size_t)]
+                ("workspace_bytes", C.c_size_t), ("Nt", C.c_int64), ("window", C.c_int), ("nu", C.c_int),
+                ("kb_beta", C.c_double)]
+
+
+class SePlanDesc(C.Structure):
+    _fields_ = [("N", C.c_int64), ("Nt", C.c_int64), ("L", C.c_double), ("xi", C.c_double), ("rc", C.c_double),
+                ("M", C.c_int), ("P", C.c_int), ("precision", C.c_int), ("window", C.c_int)]
+
+
+class SeParams(C.Structure):
+    _fields_ = [("rc", C.c_double), ("xi", C.c_double), ("M", C.c_int), ("P", C.c_int),
+                ("EN", C.c_double), ("EF", C.c_double), ("Ew", C.c_double), ("s", C.c_double),
+                ("model_ms", C.c_double)]
 
 
 class SeError(RuntimeError):
@@ -56,7 +72,14 @@ def lib() -> C.CDLL:
         L = C.CDLL(str(LIB_PATH))
         vp, i64, dbl, i32 = C.c_void_p, C.c_int64, C.c_double, C.c_int
         L.se_plan_create.argtypes = [C.POINTER(vp), i64, dbl, dbl, dbl, i32, i32, i32]
+        L.se_plan_create_ex.argtypes = [C.POINTER(vp), C.POINTER(SePlanDesc)]
+        L.se_plan_create_tol.argtypes = [C.POINTER(vp), i64, i64, dbl, dbl, i32, i32, C.POINTER(SeParams)]
+        L.se_select_params.argtypes = [i64, dbl, dbl, i32, i32, C.POINTER(SeParams)]
         L.se_eval.argtypes = [vp, vp, vp, vp, vp]
+        L.se_eval_targets.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.se_set_targets.argtypes = [vp, vp]
+        L.se_measure_peak.argtypes = [i32, i32, C.POINTER(dbl)]
+        L.se_count_pairs.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
         L.se_eval_host.argtypes = [vp, vp, vp, vp, vp]
         L.se_plan_destroy.argtypes = [vp]
         L.se_strerror.argtypes = [i32]
@@ -86,10 +109,27 @@ def _stream_ptr(stream):
     return C.c_void_p(s.cuda_stream)
 
 
-class Plan:
-    """se_plan_create / se_eval / se_plan_destroy with torch tensors for memory."""
+def select_params(N, L, eps, window="gaussian", precision="fp64") -> SeParams:
+    """se_select_params: (rc, xi, M, P) from a tolerance (host arithmetic only, no GPU needed)."""
+    out = SeParams()
+    _check(lib().se_select_params(int(N), float(L), float(eps), WINDOWS[window],
+                                  {"fp64": SE_FP64, "fp32": SE_FP32}[precision], C.byref(out)), "se_select_params")
+    return out
 
-    def __init__(self, N, L, xi, rc, M, P, precision="fp64"):
+
+def measure_peak(which, reps=5) -> float:
+    """se_measure_peak: TFLOP/s of a register-only chain, which = "fp64" | "fp64_tensor" | "fp32"; TB/s of a read + write
+    stream for which = "hbm"."""
+    v = C.c_double()
+    _check(lib().se_measure_peak({"fp64": 0, "fp64_tensor": 1, "fp32": 2, "hbm": 3}[which], int(reps), C.byref(v)),
+           "se_measure_peak")
+    return v.value
+
+
+class Plan:
+    """se_plan_create[_ex|_tol] / se_eval / se_plan_destroy with torch tensors for memory."""
+
+    def __init__(self, N, L, xi=None, rc=None, M=None, P=None, precision="fp64", window="gaussian", Nt=0, eps=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_19059_b200 needs a CUDA device (no CPU fallback)")
@@ -97,9 +137,20 @@ class Plan:
         self.precision = precision
         self.dtype = torch.float64 if precision == "fp64" else torch.float32
         prec = {"fp64": SE_FP64, "fp32": SE_FP32}[precision]
-        _check(lib().se_plan_create(C.byref(self._h), int(N), float(L), float(xi), float(rc), int(M), int(P), prec),
-               "se_plan_create")
-        self.N, self.M, self.P = int(N), int(M), int(P)
+        win = WINDOWS[window]
+        self.chosen = None
+        if eps is not None:                                   # parameters from a tolerance
+            self.chosen = SeParams()
+            _check(lib().se_plan_create_tol(C.byref(self._h), int(N), int(Nt), float(L), float(eps), win, prec,
+                                            C.byref(self.chosen)), "se_plan_create_tol")
+            M, P = self.chosen.M, self.chosen.P
+        elif win == SE_WINDOW_GAUSSIAN and not Nt:
+            _check(lib().se_plan_create(C.byref(self._h), int(N), float(L), float(xi), float(rc), int(M), int(P), prec),
+                   "se_plan_create")
+        else:
+            d = SePlanDesc(int(N), int(Nt), float(L), float(xi), float(rc), int(M), int(P), prec, win)
+            _check(lib().se_plan_create_ex(C.byref(self._h), C.byref(d)), "se_plan_create_ex")
+        self.N, self.M, self.P, self.Nt = int(N), int(M), int(P), int(Nt)
 
     # -- lifetime -----------------------------------------------------------------------
     def destroy(self):
@@ -120,13 +171,14 @@ class Plan:
         self.destroy()
 
     # -- helpers --------------------------------------------------------------------------
-    def _dev(self, t, name):
+    def _dev(self, t, name, n=None):
         if t is None:
             return C.c_void_p()
+        n = self.N if n is None else n
         if not (t.is_cuda and t.is_contiguous() and t.dtype == self.dtype):
             raise ValueError(f"{name}: need a contiguous CUDA tensor of dtype {self.dtype}")
-        if t.numel() != 3 * self.N:
-            raise ValueError(f"{name}: need N x 3 = {3 * self.N} elements, got {t.numel()}")
+        if t.numel() != 3 * n:
+            raise ValueError(f"{name}: need {n} x 3 = {3 * n} elements, got {t.numel()}")
         return C.c_void_p(t.data_ptr())
 
     def info(self) -> SeInfo:
@@ -143,6 +195,18 @@ class Plan:
                "se_eval")
         return u
 
+    def eval_targets(self, xs, f, xt, ut=None, stream=None):
+        """Plans with Nt > 0: u at the Nt targets xt from the N sources (xs, f)."""
+        import torch
+        if ut is None:
+            ut = torch.empty((self.Nt, 3), dtype=self.dtype, device=xs.device)
+        _check(lib().se_eval_targets(self._h, self._dev(xs, "xs"), self._dev(f, "f"), self._dev(xt, "xt", self.Nt),
+                                     self._dev(ut, "ut", self.Nt), _stream_ptr(stream)), "se_eval_targets")
+        return ut
+
+    def set_targets(self, xt):
+        _check(lib().se_set_targets(self._h, self._dev(xt, "xt", self.Nt)), "se_set_targets")
+
     def eval_host(self, x_host, f_host, u_host, stream=None):
         """x_host, f_host, u_host: CPU tensors (ideally pinned); async on the stream."""
         for t in (x_host, f_host, u_host):
@@ -155,16 +219,18 @@ class Plan:
     def stage(self, stage, x=None, f=None, u=None, stream=None):
         if isinstance(stage, str):
             stage = STAGES.index(stage)
-        _check(lib().se_eval_stage(self._h, int(stage), self._dev(x, "x"), self._dev(f, "f"), self._dev(u, "u"),
-                                   _stream_ptr(stream)), f"se_eval_stage({stage})")
+        _check(lib().se_eval_stage(self._h, int(stage), self._dev(x, "x"), self._dev(f, "f"),
+                                   self._dev(u, "u", self.Nt or self.N), _stream_ptr(stream)), f"se_eval_stage({stage})")
 
     # -- buffers ------------------------------------------------------------------------------
     def _buf_shape(self, which):
         import torch
-        N, M = self.N, self.M
+        tg = bool(which & SE_BUF_TARGETS)
+        which &= ~SE_BUF_TARGETS
+        N, M = (self.Nt if tg else self.N), self.M
         i = self.info()
         if which in (SE_BUF_UN, SE_BUF_UF):
-            return (N, 3), self.dtype
+            return (self.Nt or self.N, 3), self.dtype
         if which == SE_BUF_GRID:
             return (3, M, M, M), self.dtype
         if which == SE_BUF_SPEC:
@@ -202,6 +268,12 @@ class Plan:
         arr = (C.c_float * SE_NSTAGES)()
         _check(lib().se_stage_ms(self._h, arr), "se_stage_ms")
         return dict(zip(STAGES, [float(v) for v in arr]))
+
+    def count_pairs(self):
+        """se_count_pairs: (candidates, in-range pairs) of the last sorted point sets."""
+        a, b = C.c_int64(), C.c_int64()
+        _check(lib().se_count_pairs(self._h, C.byref(a), C.byref(b)), "se_count_pairs")
+        return a.value, b.value
 
     def launch_count(self) -> int:
         n = C.c_int()

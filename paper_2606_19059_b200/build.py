@@ -9,7 +9,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libse_b200.so"
-SOURCES = ["se_api.cu", "se_sort.cu", "se_p2p.cu", "se_grid.cu", "se_mma.cu", "se_scale.cu"]
+SOURCES = ["se_api.cu", "se_sort.cu", "se_p2p.cu", "se_grid.cu", "se_mma.cu", "se_scale.cu", "se_window.cu", "se_peak.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
     "-O3", "-std=c++17", "-lineinfo",

@@ -30,10 +30,14 @@ struct Alloc {
 void free_all(se_plan *p)
 {
     if (!p) return;
-    void *ptrs[] = {p->cell_of, p->cell_start, p->cell_cursor, p->perm_near, p->inv_near, p->cell_sorted,
-                    p->src_near, p->xq, p->uN, p->bin_of, p->bin_start, p->bin_cursor, p->perm_grid,
-                    p->inv_grid, p->anchor, p->wtab, p->recg, p->fs_grid, p->uF, p->uFpart, p->grid, p->spec, p->ktab, p->mtab,
-                    p->hx, p->hf, p->hu};
+    auto free_set = [](SeSet &Q) {
+        void *ptrs[] = {Q.cell_of, Q.cell_start, Q.cell_cursor, Q.perm_near, Q.inv_near, Q.cell_sorted, Q.src_near, Q.xq,
+                        Q.bin_of, Q.bin_start, Q.bin_cursor, Q.perm_grid, Q.inv_grid, Q.anchor, Q.wtab, Q.recg, Q.fs_grid};
+        for (void *q : ptrs) if (q) cudaFree(q);
+    };
+    free_set(p->S);
+    if (p->own_targets) free_set(p->T);
+    void *ptrs[] = {p->uN, p->uF, p->uFpart, p->grid, p->spec, p->ktab, p->mtab, p->wcoef, p->hx, p->hf, p->hu};
     for (void *q : ptrs) if (q) cudaFree(q);
     if (p->fft_ok & 1) cufftDestroy(p->fft_fwd);
     if (p->fft_ok & 2) cufftDestroy(p->fft_inv);
@@ -65,8 +69,8 @@ se_status run_stage(se_plan *p, int stage, const void *x, const void *f, void *u
     cudaError_t e = cudaSuccess;
     switch (stage) {
     case SE_STAGE_SORT:
-        if (!x || !f) return SE_EINVAL;
-        e = se_launch_sort(p, x, f, s);
+        if (!x || !f || (p->own_targets && !p->xt_stage)) return SE_EINVAL;
+        e = se_launch_sort(p, x, f, p->xt_stage, s);
         break;
     case SE_STAGE_P2P: e = se_launch_p2p(p, s); break;
     case SE_STAGE_P2G: e = se_launch_p2g(p, s); break;
@@ -75,7 +79,7 @@ se_status run_stage(se_plan *p, int stage, const void *x, const void *f, void *u
     case SE_STAGE_IFFT: return run_fft(p, false, s);
     case SE_STAGE_G2P: e = se_launch_g2p(p, s); break;
     case SE_STAGE_SUM:
-        if (!f || !u) return SE_EINVAL;
+        if ((!f && !p->own_targets) || !u) return SE_EINVAL;
         e = se_launch_sum(p, f, u, s);
         break;
     default: return SE_EINVAL;
@@ -88,15 +92,16 @@ size_t buffer_bytes(const se_plan *p, int which, void **ptr)
     const SeGeom &g = p->g;
     size_t rb = p->real_bytes;
     size_t M3 = (size_t)g.M * g.M * g.M, nm = (size_t)g.M * g.M * (g.M / 2 + 1);
-    switch (which) {
-    case SE_BUF_UN: *ptr = p->uN; return (size_t)g.N * 3 * rb;
-    case SE_BUF_UF: *ptr = p->uF; return (size_t)g.N * 3 * rb;
+    const SeSet &Q = (which & SE_BUF_TARGETS) ? p->T : p->S;       // PERM / START ids: which point set
+    switch (which & ~SE_BUF_TARGETS) {
+    case SE_BUF_UN: *ptr = p->uN; return (size_t)p->T.n * 3 * rb;
+    case SE_BUF_UF: *ptr = p->uF; return (size_t)p->T.n * 3 * rb;
     case SE_BUF_GRID: *ptr = p->grid; return 3 * M3 * rb;
     case SE_BUF_SPEC: *ptr = p->spec; return 3 * nm * 2 * rb;
-    case SE_BUF_PERM_NEAR: *ptr = p->perm_near; return (size_t)g.N * sizeof(int);
-    case SE_BUF_PERM_GRID: *ptr = p->perm_grid; return (size_t)g.N * sizeof(int);
-    case SE_BUF_CELL_START: *ptr = p->cell_start; return ((size_t)g.ncell * g.ncell * g.ncell + 1) * sizeof(int);
-    case SE_BUF_BIN_START: *ptr = p->bin_start; return ((size_t)g.nbins_total + 1) * sizeof(int);
+    case SE_BUF_PERM_NEAR: *ptr = Q.perm_near; return (size_t)Q.n * sizeof(int);
+    case SE_BUF_PERM_GRID: *ptr = Q.perm_grid; return (size_t)Q.n * sizeof(int);
+    case SE_BUF_CELL_START: *ptr = Q.cell_start; return ((size_t)g.ncell * g.ncell * g.ncell + 1) * sizeof(int);
+    case SE_BUF_BIN_START: *ptr = Q.bin_start; return ((size_t)g.nbins_total + 1) * sizeof(int);
     default: *ptr = nullptr; return 0;
     }
 }
@@ -120,16 +125,33 @@ const char *se_strerror(se_status s)
 se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double rc, int M, int P,
                          se_precision prec)
 {
+    se_plan_desc d{};
+    d.N = N; d.Nt = 0; d.L = L; d.xi = xi; d.rc = rc; d.M = M; d.P = P;
+    d.precision = (int)prec; d.window = SE_WINDOW_GAUSSIAN;
+    return se_plan_create_ex(out, &d);
+}
+
+se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
+{
     if (!out) return SE_EINVAL;
     *out = nullptr;
-    if (!(N >= 1) || N >= ((int64_t)1 << 31) || !(L > 0) || !(xi > 0) || !(rc > 0) || !std::isfinite(L) ||
-        !std::isfinite(xi) || !std::isfinite(rc))
+    if (!d) return SE_EINVAL;
+    const int64_t N = d->N, Nt = d->Nt;
+    const double L = d->L, xi = d->xi, rc = d->rc;
+    const int M = d->M, P = d->P, prec = d->precision, window = d->window;
+    if (!(N >= 1) || N >= ((int64_t)1 << 31) || Nt < 0 || Nt >= ((int64_t)1 << 31) || !(L > 0) || !(xi > 0) || !(rc > 0) ||
+        !std::isfinite(L) || !std::isfinite(xi) || !std::isfinite(rc))
         return SE_EINVAL;
     if (M < 2 || (M & 1) || M > 4096 || P < 2 || (P & 1) || P > SE_PMAX || P > M) return SE_EINVAL;
     if (prec != SE_FP64 && prec != SE_FP32) return SE_EINVAL;
+    if (window != SE_WINDOW_GAUSSIAN && window != SE_WINDOW_KAISER_BESSEL) return SE_EINVAL;
+    if (window == SE_WINDOW_KAISER_BESSEL && P > 16) return SE_EINVAL;
     double ncd = std::floor(L / rc);
     if (!(ncd >= 3)) return SE_EINVAL;
-    int ncell = ncd > 1024 ? 1024 : (int)ncd;          // more cells than this only wastes memory
+    // near cells: floor(L / rc) per dimension (reading S7), but no more than ~8 cells per point (wider cells stay
+    // correct -- the 27-cell stencil only needs a width >= rc -- and keep the per-evaluation histogram and scan O(N))
+    const double ncap = std::max(3.0, std::ceil(std::cbrt(8.0 * (double)std::max(N, Nt))));
+    int ncell = (int)std::min(std::min(ncd, ncap), 1024.0);
 
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return SE_ECUDA; }
@@ -138,10 +160,13 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     if (!p) return SE_ENOMEM;
     std::memset(p, 0, sizeof(*p));
     p->device = dev;
-    p->precision = (int)prec;
+    p->precision = prec;
     p->real_bytes = prec == SE_FP64 ? 8 : 4;
+    p->own_targets = Nt > 0;
     SeGeom &g = p->g;
     g.N = N; g.M = M; g.P = P; g.L = L; g.xi = xi; g.rc = rc;
+    g.window = window;
+    g.nu = window == SE_WINDOW_KAISER_BESSEL ? se_kb_degree(P) : 0;
     g.ncell = ncell;
     g.nbin = (M + SE_BIN - 1) / SE_BIN;
     g.nbins_total = g.nbin * g.nbin * g.nbin;
@@ -152,7 +177,10 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
         const char *force = std::getenv("SE_GRID_MODE");
         const bool want_tile = force && std::strcmp(force, "tile") == 0;
         const int zb = (M + SE_MMA_ZBIN - 1) / SE_MMA_ZBIN;
-        if (se_mma_supported(P, (int)prec) && (double)M * zb * M < 5.0e8 && !want_tile) {
+        // the sort key has M * zb * M bins: beyond ~64 bins per point the per-evaluation scan would dominate
+        const double nbins_mma = (double)M * zb * M;
+        if (se_mma_supported(P, prec) && se_mma_ring(P) <= M && nbins_mma < 5.0e8 &&
+            nbins_mma <= 64.0 * (double)std::max(N, Nt) + 4.0e6 && !want_tile) {
             g.grid_mode = 2;
             g.ring = se_mma_ring(P);
             g.nbin = zb;
@@ -204,11 +232,15 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     g.rel_coords = prec == SE_FP32;
     g.h = L / M;
     g.wcell = L / ncell;
-    double m = 0.95 * std::sqrt(SE_PI * P);             // reading S4
-    g.eta = (P * g.h * xi / m) * (P * g.h * xi / m);
-    double a = 2.0 * xi * xi / g.eta;
-    g.beta = a * g.h * g.h;
-    g.cw = std::pow(a / SE_PI, 1.5);
+    if (window == SE_WINDOW_GAUSSIAN) {
+        double m = 0.95 * std::sqrt(SE_PI * P);             // reading S4
+        g.eta = (P * g.h * xi / m) * (P * g.h * xi / m);
+        double a = 2.0 * xi * xi / g.eta;
+        g.beta = a * g.h * g.h;
+        g.cw = std::pow(a / SE_PI, 1.5);
+    } else {                                                // Kaiser-Bessel: w0(0) = 1, no prefactor (eq. (2.8))
+        g.eta = 0.0; g.beta = 0.0; g.cw = 1.0;
+    }
 
     size_t rb = p->real_bytes;
     size_t nc3 = (size_t)ncell * ncell * ncell, nb3 = (size_t)g.nbins_total;
@@ -216,29 +248,42 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     size_t scan_tiles = (std::max(nc3, nb3) + 2047) / 2048 + 1;
 
     Alloc A{p};
-    A.get(&p->cell_of, N * sizeof(int));
-    A.get(&p->cell_start, (nc3 + 1 + scan_tiles) * sizeof(int));
-    A.get(&p->cell_cursor, (nc3 + 1) * sizeof(int));
-    A.get(&p->perm_near, N * sizeof(int));
-    A.get(&p->inv_near, N * sizeof(int));
-    A.get(&p->cell_sorted, N * sizeof(int));
-    A.get(&p->src_near, N * 6 * rb);
-    A.get(&p->xq, N * sizeof(float4));
-    A.get(&p->uN, N * 3 * rb);
-    A.get(&p->bin_of, N * sizeof(int));
-    A.get(&p->bin_start, (nb3 + 1 + scan_tiles) * sizeof(int));
-    A.get(&p->bin_cursor, (nb3 + 1) * sizeof(int));
-    A.get(&p->perm_grid, N * sizeof(int));
-    A.get(&p->inv_grid, N * sizeof(int));
-    A.get(&p->anchor, N * sizeof(short4));
-    A.get(&p->wtab, g.grid_mode == 2 ? (size_t)N * SE_MMA_RECS(g.ring) * 8 : (size_t)N * 3 * P * rb);
-    if (g.grid_mode == 2) A.get(&p->recg, (size_t)N * SE_MMA_RECG(P) * 8);
-    A.get(&p->fs_grid, N * 3 * rb);
-    A.get(&p->uF, std::max((size_t)N * 3 * rb, (size_t)N * sizeof(int)));
-    if (g.grid_mode == 2) A.get(&p->uFpart, (size_t)N * se_mma_slots(P) * 3 * 8);
+    auto alloc_set = [&](SeSet &Q, int64_t n, bool spread, bool gather) {
+        Q.n = n;
+        A.get(&Q.cell_of, n * sizeof(int));
+        A.get(&Q.cell_start, (nc3 + 1 + scan_tiles) * sizeof(int));
+        A.get(&Q.cell_cursor, (nc3 + 1) * sizeof(int));
+        A.get(&Q.perm_near, n * sizeof(int));
+        A.get(&Q.inv_near, n * sizeof(int));
+        A.get(&Q.cell_sorted, n * sizeof(int));
+        A.get(&Q.src_near, n * 6 * rb);
+        A.get(&Q.xq, n * sizeof(float4));
+        A.get(&Q.bin_of, n * sizeof(int));
+        A.get(&Q.bin_start, (nb3 + 1 + scan_tiles) * sizeof(int));
+        A.get(&Q.bin_cursor, (nb3 + 1) * sizeof(int));
+        A.get(&Q.perm_grid, n * sizeof(int));
+        A.get(&Q.inv_grid, n * sizeof(int));
+        A.get(&Q.anchor, n * sizeof(short4));
+        if (g.grid_mode == 2) {
+            if (spread) A.get(&Q.wtab, (size_t)n * SE_MMA_RECS(g.ring) * 8);
+            if (gather) A.get(&Q.recg, (size_t)n * SE_MMA_RECG(P) * 8);
+        } else
+            A.get(&Q.wtab, (size_t)n * 3 * P * rb);
+        A.get(&Q.fs_grid, std::max((size_t)n * 3 * rb, (size_t)n * sizeof(int)));
+    };
+    alloc_set(p->S, N, true, !p->own_targets);
+    if (p->own_targets) alloc_set(p->T, Nt, false, true);
+    else p->T = p->S;
+    const int64_t NT = p->T.n;
+    A.get(&p->uN, NT * 3 * rb);
+    A.get(&p->uF, NT * 3 * rb);
+    if (g.grid_mode == 2) A.get(&p->uFpart, (size_t)NT * se_mma_slots(P) * 3 * 8);
     A.get(&p->grid, 3 * M3 * rb);
     A.get(&p->spec, 3 * nm * 2 * rb);
     A.get(&p->ktab, 2 * (size_t)M * rb);
+    if (!p->own_targets) {                                  // staging of se_eval_host
+        A.get(&p->hx, N * 3 * rb); A.get(&p->hf, N * 3 * rb); A.get(&p->hu, N * 3 * rb);
+    }
     if (!A.ok) { free_all(p); return SE_ENOMEM; }
 
     // cuFFT: batch of 3 out-of-place 3-D transforms, contiguous, z fastest, halved axis last
@@ -261,8 +306,12 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     }
     p->workspace_bytes += p->fft_work_bytes;
 
-    if (se_build_ktab(p) != cudaSuccess) { cudaGetLastError(); free_all(p); return SE_ECUDA; }
-    if (se_build_mtab(p) != cudaSuccess) { cudaGetLastError(); free_all(p); return SE_ECUDA; }
+    if (se_build_ktab(p) != cudaSuccess || se_build_wcoef(p) != cudaSuccess || se_build_mtab(p) != cudaSuccess ||
+        se_prepare_grid(p) != cudaSuccess) {
+        cudaGetLastError();
+        free_all(p);
+        return SE_ECUDA;
+    }
     for (int i = 0; i <= SE_NSTAGES; ++i)
         if (cudaEventCreate(&p->ev[i]) != cudaSuccess) { free_all(p); return SE_ECUDA; }
     p->ev_ok = 1;
@@ -286,9 +335,18 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
     return SE_OK;
 }
 
+// every call on a plan must be made with the plan's device current
+static bool on_device(const se_plan *p)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return false; }
+    return dev == p->device;
+}
+
 se_status se_plan_destroy(se_plan *p)
 {
     if (!p) return SE_OK;
+    if (!on_device(p)) return SE_EINVAL;
     cudaDeviceSynchronize();
     free_all(p);
     return SE_OK;
@@ -298,11 +356,14 @@ se_status se_plan_info(const se_plan *p, se_info *o)
 {
     if (!p || !o) return SE_EINVAL;
     const SeGeom &g = p->g;
-    o->N = g.N; o->M = g.M; o->P = g.P; o->precision = p->precision;
+    o->N = p->S.n; o->M = g.M; o->P = g.P; o->precision = p->precision;
     o->L = g.L; o->xi = g.xi; o->rc = g.rc; o->h = g.h;
-    o->m = 0.95 * std::sqrt(SE_PI * g.P);
+    o->m = g.window == SE_WINDOW_GAUSSIAN ? 0.95 * std::sqrt(SE_PI * g.P) : 0.0;
     o->eta = g.eta;
     o->a = g.beta / (g.h * g.h);
+    o->Nt = p->own_targets ? p->T.n : 0;
+    o->window = g.window; o->nu = g.nu;
+    o->kb_beta = g.window == SE_WINDOW_KAISER_BESSEL ? 2.5 * g.P : 0.0;
     o->cw = g.cw;
     o->ncell = g.ncell; o->nbin = g.nbin;
     o->grid_mode = g.grid_mode; o->nbins_total = g.nbins_total; o->nchunk = g.nchunk;
@@ -311,9 +372,8 @@ se_status se_plan_info(const se_plan *p, se_info *o)
     return SE_OK;
 }
 
-se_status se_eval(se_plan *p, const void *x, const void *f, void *u, void *stream)
+static se_status run_all(se_plan *p, const void *x, const void *f, void *u, void *stream)
 {
-    if (!p || !x || !f || !u) return SE_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     p->launches = 0;
     p->ev_recorded = 0;
@@ -346,16 +406,31 @@ se_status se_eval(se_plan *p, const void *x, const void *f, void *u, void *strea
     return SE_OK;
 }
 
+se_status se_eval(se_plan *p, const void *x, const void *f, void *u, void *stream)
+{
+    if (!p || !x || !f || !u || p->own_targets || !on_device(p)) return SE_EINVAL;
+    return run_all(p, x, f, u, stream);
+}
+
+se_status se_eval_targets(se_plan *p, const void *xs, const void *f, const void *xt, void *ut, void *stream)
+{
+    if (!p || !xs || !f || !xt || !ut || !p->own_targets || !on_device(p)) return SE_EINVAL;
+    p->xt_stage = xt;
+    return run_all(p, xs, f, ut, stream);
+}
+
+se_status se_set_targets(se_plan *p, const void *xt)
+{
+    if (!p || !xt || !p->own_targets) return SE_EINVAL;
+    p->xt_stage = xt;
+    return SE_OK;
+}
+
 se_status se_eval_host(se_plan *p, const void *xh, const void *fh, void *uh, void *stream)
 {
-    if (!p || !xh || !fh || !uh) return SE_EINVAL;
+    if (!p || !xh || !fh || !uh || p->own_targets || !on_device(p)) return SE_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
-    size_t bytes = (size_t)p->g.N * 3 * p->real_bytes;
-    if (!p->hx) {
-        Alloc A{p};
-        A.get(&p->hx, bytes); A.get(&p->hf, bytes); A.get(&p->hu, bytes);
-        if (!A.ok) return SE_ENOMEM;
-    }
+    size_t bytes = (size_t)p->S.n * 3 * p->real_bytes;
     if (cudaMemcpyAsync(p->hx, xh, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) return SE_ECUDA;
     if (cudaMemcpyAsync(p->hf, fh, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) return SE_ECUDA;
     se_status r = se_eval(p, p->hx, p->hf, p->hu, stream);
@@ -366,13 +441,13 @@ se_status se_eval_host(se_plan *p, const void *xh, const void *fh, void *uh, voi
 
 se_status se_eval_stage(se_plan *p, int stage, const void *x, const void *f, void *u, void *stream)
 {
-    if (!p) return SE_EINVAL;
+    if (!p || !on_device(p)) return SE_EINVAL;
     return run_stage(p, stage, x, f, u, (cudaStream_t)stream);
 }
 
 se_status se_buffer_read(se_plan *p, int which, void *dst, size_t bytes, size_t *size_out, void *stream)
 {
-    if (!p) return SE_EINVAL;
+    if (!p || !on_device(p)) return SE_EINVAL;
     void *src = nullptr;
     size_t n = buffer_bytes(p, which, &src);
     if (!src) return SE_EINVAL;
@@ -385,7 +460,7 @@ se_status se_buffer_read(se_plan *p, int which, void *dst, size_t bytes, size_t 
 
 se_status se_buffer_write(se_plan *p, int which, const void *srcv, size_t bytes, void *stream)
 {
-    if (!p || !srcv) return SE_EINVAL;
+    if (!p || !srcv || !on_device(p)) return SE_EINVAL;
     void *dst = nullptr;
     size_t n = buffer_bytes(p, which, &dst);
     if (!dst || bytes != n) return SE_EINVAL;

@@ -34,8 +34,10 @@ constexpr int SE_MMA_NWY = 2, SE_MMA_NWZ = 6;
 #define SE_MMA_RECG(P) (3 * (P) + 4)
 
 struct SeGeom {
-    int64_t N;
+    int64_t N;          // points of the set a launch works on (sources or targets; the launchers set it)
     int M, P;
+    int window;         // se_window
+    int nu;             // Kaiser-Bessel: polynomial degree per bin
     int ncell;          // near cells per dimension
     int nbin;           // grid bins per dimension = ceil(M / SE_BIN) (tile mode) or z-bins ceil(M / 8) (mma mode)
     int grid_mode;      // 0: tile-stationary k_grid (any even P),
@@ -55,6 +57,30 @@ struct SeGeom {
     double eta;
 };
 
+// One point set (the sources, or a plan's own targets) in its two sorted orders.
+struct SeSet {
+    int64_t n;
+    // near field (K1a, K2)
+    int *cell_of;                  // [n]  near cell of user particle i
+    int *cell_start;               // [ncell^3 + 1]
+    int *cell_cursor;              // [ncell^3 + 1] scatter cursors
+    int *perm_near;                // [n] sorted pos -> user index
+    int *inv_near;                 // [n] user index -> sorted pos
+    int *cell_sorted;              // [n] packed cell coordinates (cx << 20 | cy << 10 | cz) of sorted particle
+    void *src_near;                // [n][6] Real: x, y, z (absolute fp64 / cell-relative fp32), f_x, f_y, f_z (0 for targets)
+    void *xq;                      // [n] float4: cell-relative x, y, z and absolute z in FP32 (K2 candidate filter)
+    // grid path (K1b, K3, K5)
+    int *bin_of;                   // [n]
+    int *bin_start;                // [nbins_total + 1]
+    int *bin_cursor;               // [nbins_total + 1]
+    int *perm_grid;                // [n]
+    int *inv_grid;                 // [n]
+    short4 *anchor;                // [n] (a_x, a_y, a_z, 0): anchor grid index in [0, M)
+    void *wtab;                    // [n][3][P] Real: 1-D window values of every particle (mma mode: spread records)
+    void *recg;                    // mma mode: gather records
+    void *fs_grid;                 // [n][3] Real
+};
+
 struct se_plan {
     SeGeom g;
     int precision;
@@ -62,28 +88,14 @@ struct se_plan {
     int profiling;
     int launches;
     size_t real_bytes;             // sizeof(Real)
-    // near field (K1a, K2)
-    int *cell_of;                  // [N]  near cell of user particle i
-    int *cell_start;               // [ncell^3 + 1]
-    int *cell_cursor;              // [ncell^3 + 1] scatter cursors
-    int *perm_near;                // [N] sorted pos -> user index
-    int *inv_near;                 // [N] user index -> sorted pos
-    int *cell_sorted;              // [N] packed cell coordinates (cx << 20 | cy << 10 | cz) of sorted particle
-    void *src_near;                // [N][6] Real: x, y, z (absolute fp64 / cell-relative fp32), f_x, f_y, f_z
-    void *xq;                      // [N] float4: cell-relative x, y, z and absolute z in FP32 (K2 candidate filter)
-    void *uN;                      // [N][3] Real, near-sorted order
-    // grid path (K1b, K3, K5)
-    int *bin_of;                   // [N]
-    int *bin_start;                // [nbin^3 + 1]
-    int *bin_cursor;               // [nbin^3 + 1]
-    int *perm_grid;                // [N]
-    int *inv_grid;                 // [N]
-    short4 *anchor;                // [N] (a_x, a_y, a_z, 0): anchor grid index in [0, M)
-    void *wtab;                    // [N][3][P] Real: 1-D window values of every particle (mma mode: spread records)
-    void *recg;                    // mma mode: gather records
-    void *fs_grid;                 // [N][3] Real
-    void *uF;                      // [N][3] Real, grid-sorted order (unscaled sum)
-    void *uFpart;                  // mma mode: [slots][N][3] double per-(particle, block tile) partial sums
+    SeSet S;                       // sources
+    SeSet T;                       // targets: a copy of S (same pointers) unless the plan has its own targets
+    int own_targets;               // 1: T has its own arrays (se_eval_targets)
+    const void *xt_stage;          // se_set_targets: target positions for se_eval_stage(SE_STAGE_SORT)
+    double *wcoef;                 // Kaiser-Bessel: [P][nu + 1] polynomial coefficients (always double)
+    void *uN;                      // [Nt][3] Real, the targets' near-sorted order
+    void *uF;                      // [Nt][3] Real, the targets' grid-sorted order (unscaled sum)
+    void *uFpart;                  // mma mode: [slots][Nt][3] double per-(particle, block tile) partial sums
     // grids
     void *grid;                    // [3][M][M][M] Real
     void *spec;                    // [3][M][M][M/2+1] complex Real
@@ -105,14 +117,21 @@ struct se_plan {
 };
 
 // ---- launchers implemented in the .cu files -------------------------------------------------
-cudaError_t se_launch_sort(se_plan *p, const void *x, const void *f, cudaStream_t s);
+cudaError_t se_launch_sort(se_plan *p, const void *x, const void *f, const void *xt, cudaStream_t s);
 cudaError_t se_launch_p2p(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_p2g(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_scale(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_g2p(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_sum(se_plan *p, const void *f, void *u, cudaStream_t s);
-cudaError_t se_build_ktab(se_plan *p);
+cudaError_t se_build_ktab(se_plan *p);      // se_window.cu: k values and the deconvolution factor per 1-D index
+cudaError_t se_build_wcoef(se_plan *p);     // se_window.cu: allocates and fills p->wcoef (Kaiser-Bessel plans)
 cudaError_t se_build_mtab(se_plan *p);      // allocates and fills p->mtab
+cudaError_t se_prepare_mma(se_plan *p);     // per-plan kernel attributes (dynamic shared memory opt-in) on the plan's device
+cudaError_t se_prepare_grid(se_plan *p);
+int se_kb_degree(int P);                    // reading S19
+// Chebyshev-node interpolant of fn on [c - hw, c + hw], degree deg <= 23, as monomials in (x - c)/hw (host, long double)
+void se_cheb_fit(long double (*fn)(long double, const void *), const void *ctx, long double c, long double hw, int deg,
+                 double *out);
 cudaError_t se_launch_mma_p2g(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_mma_g2p(se_plan *p, cudaStream_t s);
 bool se_mma_supported(int P, int precision);

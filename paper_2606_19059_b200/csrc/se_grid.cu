@@ -254,24 +254,21 @@ k_grid(SeGeom g, const short4 *__restrict__ anchor, const Real *__restrict__ wta
 }
 
 template <typename Real, bool SPREAD>
-cudaError_t grid_impl(se_plan *p, cudaStream_t s)
+cudaError_t grid_impl(se_plan *p, cudaStream_t s, bool prepare = false)
 {
-    const SeGeom &g = p->g;
-    static bool attr_set[2] = {false, false};
+    SeGeom g = p->g;
+    const SeSet &Q = SPREAD ? p->S : p->T;                     // P2G spreads the sources, G2P gathers at the targets
+    g.N = Q.n;
     size_t smem = sizeof(GridSmem<Real>);
     auto kern = k_grid<Real, SPREAD>;
-    if (!attr_set[SPREAD]) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set[SPREAD] = true;
-    }
+    if (prepare) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     int ntz = (g.M + SE_TZ - 1) / SE_TZ, nty = (g.M + SE_TY - 1) / SE_TY, ntx = (g.M + SE_TX - 1) / SE_TX;
     if (!SPREAD) {
         cudaError_t e = cudaMemsetAsync(p->uF, 0, (size_t)g.N * 3 * sizeof(Real), s);
         if (e != cudaSuccess) return e;
     }
     kern<<<(unsigned)(ntx * nty * ntz), SE_GRID_THREADS, smem, s>>>(
-        g, p->anchor, (const Real *)p->wtab, (const Real *)p->fs_grid, p->bin_start, (Real *)p->grid,
+        g, Q.anchor, (const Real *)Q.wtab, (const Real *)Q.fs_grid, Q.bin_start, (Real *)p->grid,
         (Real *)p->uF);
     p->launches += 1;
     return cudaGetLastError();
@@ -289,4 +286,12 @@ cudaError_t se_launch_g2p(se_plan *p, cudaStream_t s)
 {
     if (p->g.grid_mode == 2) return se_launch_mma_g2p(p, s);
     return p->precision == SE_FP64 ? grid_impl<double, false>(p, s) : grid_impl<float, false>(p, s);
+}
+
+cudaError_t se_prepare_grid(se_plan *p)
+{
+    if (p->g.grid_mode == 2) return se_prepare_mma(p);
+    cudaError_t e = p->precision == SE_FP64 ? grid_impl<double, true>(p, nullptr, true) : grid_impl<float, true>(p, nullptr, true);
+    if (e != cudaSuccess) return e;
+    return p->precision == SE_FP64 ? grid_impl<double, false>(p, nullptr, true) : grid_impl<float, false>(p, nullptr, true);
 }

@@ -636,28 +636,26 @@ __global__ void k_reduce_slots(SeGeom g, const short4 *__restrict__ anchor, cons
     uF[3 * i + 0] = (GR)s0; uF[3 * i + 1] = (GR)s1; uF[3 * i + 2] = (GR)s2;
 }
 
+// prepare == true: only opt this plan's device in to the kernel's dynamic shared memory (once per plan, at creation)
 template <int P, bool SPREAD, int W, typename GR>
-cudaError_t launch(se_plan *p, cudaStream_t s)
+cudaError_t launch(se_plan *p, cudaStream_t s, bool prepare)
 {
     typedef Cfg<P, SPREAD> C;
-    const SeGeom &g = p->g;
-    static bool attr_set = false;
+    SeGeom g = p->g;
+    const SeSet &Q = SPREAD ? p->S : p->T;                     // P2G spreads the sources, G2P gathers at the targets
+    g.N = Q.n;
     constexpr size_t smem = sizeof(Smem<P, SPREAD>);
     static_assert(smem <= 227 * 1024, "shared memory per block");
     auto kern = k_mma<P, SPREAD, W, GR>;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    if (prepare) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int ntY = (g.M + C::BY - 1) / C::BY, ntZ = (g.M + C::BZ - 1) / C::BZ;
     const int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
     const int nblocks = (SPREAD && g.nsplit > 1) ? g.nfull + g.nsplit * (ntY * ntZ - g.nfull) : nchunk * ntY * ntZ;
-    kern<<<(unsigned)nblocks, C::NT, smem, s>>>(g, (const double *)(SPREAD ? p->wtab : p->recg), p->bin_start,
+    kern<<<(unsigned)nblocks, C::NT, smem, s>>>(g, (const double *)(SPREAD ? Q.wtab : Q.recg), Q.bin_start,
                                                              (GR *)p->grid, (double *)p->uFpart);
     p->launches += 1;
     if (!SPREAD) {
-        k_reduce_slots<P, GR><<<(unsigned)((g.N + 255) / 256), 256, 0, s>>>(g, p->anchor, (const double *)p->uFpart,
+        k_reduce_slots<P, GR><<<(unsigned)((g.N + 255) / 256), 256, 0, s>>>(g, Q.anchor, (const double *)p->uFpart,
                                                                             (GR *)p->uF);
         p->launches += 1;
     }
@@ -665,25 +663,30 @@ cudaError_t launch(se_plan *p, cudaStream_t s)
 }
 
 template <bool SPREAD>
-cudaError_t dispatch(se_plan *p, cudaStream_t s)
+cudaError_t dispatch(se_plan *p, cudaStream_t s, bool prepare = false)
 {
+    // ring (row stride of the records) P rounded up to 8 for P2G; fp32 plans: float grid, double records / accumulators
     if (p->precision == SE_FP64) {
         switch (p->g.P) {
-        case 24: return launch<24, SPREAD, 24, double>(p, s);
-        case 16: return launch<16, SPREAD, 16, double>(p, s);
+        case 24: return launch<24, SPREAD, 24, double>(p, s, prepare);
+        case 16: return launch<16, SPREAD, 16, double>(p, s, prepare);
+        case 12: return launch<SPREAD ? 16 : 12, SPREAD, 12, double>(p, s, prepare);
+        case 8: return launch<8, SPREAD, 8, double>(p, s, prepare);
         default: return cudaErrorInvalidValue;
         }
     }
-    // fp32 plans: float grid, double records and accumulation; P = 12 spreads on a ring of 16 planes
-    if (p->g.P == 12) return launch<SPREAD ? 16 : 12, SPREAD, 12, float>(p, s);
-    return cudaErrorInvalidValue;
+    switch (p->g.P) {
+    case 12: return launch<SPREAD ? 16 : 12, SPREAD, 12, float>(p, s, prepare);
+    case 8: return launch<8, SPREAD, 8, float>(p, s, prepare);
+    default: return cudaErrorInvalidValue;
+    }
 }
 
 }  // namespace
 
 bool se_mma_supported(int P, int precision)
 {
-    return precision == SE_FP64 ? (P == 24 || P == 16) : P == 12;
+    return precision == SE_FP64 ? (P == 24 || P == 16 || P == 12 || P == 8) : (P == 12 || P == 8);
 }
 int se_mma_ring(int P) { return (P + 7) / 8 * 8; }     // row stride of the spread records
 int se_mma_slots(int P)
@@ -691,8 +694,14 @@ int se_mma_slots(int P)
     switch (P) {
     case 24: return Cfg<24, false>::NSB * Cfg<24, false>::NSC;
     case 16: return Cfg<16, false>::NSB * Cfg<16, false>::NSC;
-    default: return Cfg<12, false>::NSB * Cfg<12, false>::NSC;
+    case 12: return Cfg<12, false>::NSB * Cfg<12, false>::NSC;
+    default: return Cfg<8, false>::NSB * Cfg<8, false>::NSC;
     }
 }
 cudaError_t se_launch_mma_p2g(se_plan *p, cudaStream_t s) { return dispatch<true>(p, s); }
 cudaError_t se_launch_mma_g2p(se_plan *p, cudaStream_t s) { return dispatch<false>(p, s); }
+cudaError_t se_prepare_mma(se_plan *p)
+{
+    cudaError_t e = dispatch<true>(p, nullptr, true);
+    return e != cudaSuccess ? e : dispatch<false>(p, nullptr, true);
+}

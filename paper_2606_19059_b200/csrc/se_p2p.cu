@@ -158,15 +158,19 @@ template <> struct NearMath<float> {
 // every evaluated pair has r <= rc, a rejected one is evaluated at r = rc)
 template <typename Real, bool CLAMP>
 __global__ void __launch_bounds__(P2P_WARPS * 32, P2P_BLOCKS)
-k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, const int *__restrict__ cellp,
-      const int *__restrict__ cell_start, const double *__restrict__ mtab, Real *__restrict__ uN, float rc2m)
+k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, const int *__restrict__ cell_start,
+      const float4 *__restrict__ xq_t, const Real *__restrict__ src_t, const int *__restrict__ cellp,
+      const double *__restrict__ mtab, Real *__restrict__ uN, float rc2m)
 {
+    // sources: xq, src, cell_start (near order of the source set); targets (g.N of them): xq_t, src_t, cellp (near order
+    // of the target set -- the same arrays when the targets are the sources)
     __shared__ Real mt[NearMath<Real>::TAB];
     NearMath<Real>::load(mt, mtab, threadIdx.x, P2P_WARPS * 32);
     __syncthreads();
     __shared__ unsigned short qsm[P2P_WARPS][P2P_QC][32];
     __shared__ int vtab[P2P_WARPS][P2P_NV];                      // virtual cell -> sorted index of its first source
     __shared__ Real vshift[P2P_WARPS][P2P_NV][3];                // virtual cell -> periodic image shift of its sources
+    __shared__ int vzcell[P2P_WARPS][P2P_NV];                    // cell-relative plans: unwrapped z cell of the sources
     __shared__ float4 sbuf[P2P_WARPS][P2P_CHUNK];                // the chunk of sources being tested (broadcast reads)
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -181,18 +185,19 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     constexpr int QSTRIDE = 64, QBYTES = P2P_QC * QSTRIDE;
     int *const VT = vtab[w];
     Real (*const VS)[3] = vshift[w];
+    int *const VZ = vzcell[w];
+    constexpr bool REL = sizeof(Real) == 4;                      // fp32 plans: cell-relative coordinates (g.rel_coords)
     float4 *const SB = sbuf[w];
     int nv = 0, nv_drained = 0;                                  // virtual cells opened / opened at the last full drain
 
     const int64_t i = ((int64_t)blockIdx.x * P2P_WARPS + w) * 32 + lane;
     const bool valid = i < g.N;
     const int64_t ic = valid ? i : g.N - 1;
-    const float4 qi = xq[ic];
+    const float4 qi = xq_t[ic];
     const int pci = cellp[ic];
     const int cz = pci & 1023;
-    const Real X0 = src[6 * ic + 0], X1 = src[6 * ic + 1], X2 = src[6 * ic + 2];
+    const Real X0 = src_t[6 * ic + 0], X1 = src_t[6 * ic + 1], X2 = src_t[6 * ic + 2];
     Real a0 = 0, a1 = 0, a2 = 0;
-    const Real czw = g.rel_coords ? (Real)cz * wc : (Real)0;    // z offset of this target's cell (cell-relative plans)
     int woff = 0, roff = 0;                                      // ring write / read offsets (bytes); empty when equal
 
     auto queued = [&]() { return ((woff - roff) & (QBYTES - 1)) / QSTRIDE; };
@@ -202,7 +207,7 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     // function of the queue lengths, so the summation order stays deterministic.
     // one pair: queue entry at byte offset qo of this lane's (or, mode B, the owner's) column -> contribution d
     // keep = false: evaluate but contribute nothing; d0..d2 are ADDED to (fused into the last FMAs)
-    auto pair = [&](int qo, bool keep, Real T0, Real T1, Real T2, Real tcz, Real &d0, Real &d1, Real &d2) {
+    auto pair = [&](int qo, bool keep, Real T0, Real T1, Real T2, int tcz, Real &d0, Real &d1, Real &d2) {
         const int e = *reinterpret_cast<const unsigned short *>(Qb + qo);
         const int j = VT[e >> P2P_VBITS] + (e & ((1 << P2P_VBITS) - 1));
         const Real *sp = src + 6 * (int64_t)j;
@@ -219,9 +224,11 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
             xj = (Real)p0.x; yj = (Real)p0.y; zj = (Real)p1.x; f0 = (Real)p1.y; f1 = (Real)p2.x; f2 = (Real)p2.y;
         }
         // periodic image of the source as this target sees it: the virtual cell's shift (absolute coordinates:
-        // a multiple of L per axis; cell-relative coordinates: the cell offset, in z from the target's own cell)
+        // a multiple of L per axis; cell-relative coordinates: the cell offset, in z the INTEGER cell difference to
+        // the target's own cell times the cell width, so that the shift carries one rounding, like x and y)
         const Real *vs = VS[e >> P2P_VBITS];
-        const Real sx = vs[0], sy = vs[1], sz = vs[2] - tcz;
+        const Real sx = vs[0], sy = vs[1];
+        const Real sz = REL ? (Real)(VZ[e >> P2P_VBITS] - tcz) * wc : vs[2];
         const Real rx = T0 - (xj + sx), ry = T1 - (yj + sy), rz = T2 - (zj + sz);
         Real r2 = rx * rx + ry * ry + rz * rz;
         const bool ok = keep && (r2 <= rc2) && (r2 > (Real)0);
@@ -243,7 +250,8 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
         if (cB > __popc(m1)) {                                   // mode B (warp-uniform)
             const int o = __ffs(__ballot_sync(0xffffffffu, c == cmax)) - 1;
             const Real T0 = __shfl_sync(0xffffffffu, X0, o), T1 = __shfl_sync(0xffffffffu, X1, o);
-            const Real T2 = __shfl_sync(0xffffffffu, X2, o), tcz = __shfl_sync(0xffffffffu, czw, o);
+            const Real T2 = __shfl_sync(0xffffffffu, X2, o);
+            const int tcz = __shfl_sync(0xffffffffu, cz, o);
             const int ro = (__shfl_sync(0xffffffffu, roff, o) + lane * QSTRIDE) & (QBYTES - 1);
             Real d0 = 0, d1 = 0, d2 = 0;
             if (lane < cB) pair((o - lane) * 2 + ro, true, T0, T1, T2, tcz, d0, d1, d2);
@@ -261,13 +269,13 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                 int ro = roff;
 #pragma unroll
                 for (int k = 0; k < KP; ++k) {
-                    pair(ro, k < c, X0, X1, X2, czw, a0, a1, a2);
+                    pair(ro, k < c, X0, X1, X2, cz, a0, a1, a2);
                     if (k + 1 < c) ro = (ro + QSTRIDE) & (QBYTES - 1);
                 }
                 roff = (roff + min(c, KP) * QSTRIDE) & (QBYTES - 1);
             }
         } else if (c > 0) {                                      // mode A: every lane pops one pair of its own
-            pair(roff, true, X0, X1, X2, czw, a0, a1, a2);
+            pair(roff, true, X0, X1, X2, cz, a0, a1, a2);
             roff = (roff + QSTRIDE) & (QBYTES - 1);
         }
     };
@@ -326,10 +334,11 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                         const int zu = czl - 1 + k;              // unwrapped z cell of the sources
                         const int cu = lane == 0 ? cxl + dx : (lane == 1 ? cyl + dy : zu);
                         Real sh;
-                        if (g.rel_coords) sh = (Real)(lane == 0 ? dx : (lane == 1 ? dy : zu)) * wc;
+                        if (REL) sh = (Real)(lane == 0 ? dx : (lane == 1 ? dy : 0)) * wc;
                         else sh = cu < 0 ? -Lr : (cu >= nc ? Lr : (Real)0);
                         VS[vslot][lane] = sh;
                         if (lane == 0) VT[vslot] = v0;
+                        if (lane == 2) VZ[vslot] = zu;
                     }
                     __syncwarp();
                     const int ve = min(je, v0 + (1 << P2P_VBITS));
@@ -376,21 +385,60 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     if (valid) { uN[3 * i + 0] = a0; uN[3 * i + 1] = a1; uN[3 * i + 2] = a2; }
 }
 
+// Diagnostics for bench.py's K2 roofline (not on the evaluation path): candidates (sources in the 27 colleague cells) and
+// in-range pairs (0 < r <= rc) summed over all targets, from the FP32 cell-relative copies, one thread per target.
+__global__ void __launch_bounds__(256)
+k_count_pairs(SeGeom g, const float4 *__restrict__ xq, const int *__restrict__ cell_start, const float4 *__restrict__ xq_t,
+              const int *__restrict__ cellp, unsigned long long *__restrict__ out)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long cand = 0, hit = 0;
+    if (i < g.N) {
+        const float4 qi = xq_t[i];
+        const int pc = cellp[i], nc = g.ncell;
+        const int cx = pc >> 20, cy = (pc >> 10) & 1023, cz = pc & 1023;
+        const float wf = (float)g.wcell, rc2 = (float)(g.rc * g.rc);
+        for (int dx = -1; dx <= 1; ++dx)
+        for (int dy = -1; dy <= 1; ++dy)
+        for (int dz = -1; dz <= 1; ++dz) {
+            const int nx = (cx + dx + nc) % nc, ny = (cy + dy + nc) % nc, nz = (cz + dz + nc) % nc;
+            const int *cs = cell_start + (size_t)(nx * nc + ny) * nc + nz;
+            const int jb = cs[0], je = cs[1];
+            cand += (unsigned long long)(je - jb);
+            for (int j = jb; j < je; ++j) {
+                const float4 q = __ldg(xq + j);
+                const float rx = qi.x - q.x - dx * wf, ry = qi.y - q.y - dy * wf, rz = qi.z - q.z - dz * wf;
+                const float r2 = rx * rx + ry * ry + rz * rz;
+                hit += (r2 <= rc2 && r2 > 0.f) ? 1u : 0u;
+            }
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        cand += __shfl_down_sync(0xffffffffu, cand, o);
+        hit += __shfl_down_sync(0xffffffffu, hit, o);
+    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(out, cand); atomicAdd(out + 1, hit); }
+}
+
 template <typename Real>
 cudaError_t p2p_impl(se_plan *p, cudaStream_t s)
 {
-    const SeGeom &g = p->g;
+    SeGeom g = p->g;
+    g.N = p->T.n;                                                // a lane per target
+    const SeSet &S = p->S, &T = p->T;
     int64_t per_block = (int64_t)P2P_WARPS * 32;
     unsigned nblk = (unsigned)((g.N + per_block - 1) / per_block);
     // FP32 filter margin: the cell-relative coordinates are < 2 wcell in magnitude, each rounded to 6e-8
     // relative, so |dr| < 1e-6 wcell per component and |d r^2| < 2 sqrt(3) rc 1e-6 wcell
     const double rc2m = g.rc * g.rc * (1.0 + 1e-5) + 4e-6 * g.rc * g.wcell;
     if (g.xi * g.rc > 7.8)
-        k_p2p<Real, true><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)p->xq, (const Real *)p->src_near, p->cell_sorted,
-                                                         p->cell_start, p->mtab, (Real *)p->uN, (float)rc2m);
+        k_p2p<Real, true><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)S.xq, (const Real *)S.src_near, S.cell_start,
+                                                         (const float4 *)T.xq, (const Real *)T.src_near, T.cell_sorted,
+                                                         p->mtab, (Real *)p->uN, (float)rc2m);
     else
-        k_p2p<Real, false><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)p->xq, (const Real *)p->src_near, p->cell_sorted,
-                                                          p->cell_start, p->mtab, (Real *)p->uN, (float)rc2m);
+        k_p2p<Real, false><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)S.xq, (const Real *)S.src_near, S.cell_start,
+                                                          (const float4 *)T.xq, (const Real *)T.src_near, T.cell_sorted,
+                                                          p->mtab, (Real *)p->uN, (float)rc2m);
     p->launches += 1;
     return cudaGetLastError();
 }
@@ -398,12 +446,13 @@ cudaError_t p2p_impl(se_plan *p, cudaStream_t s)
 }  // namespace
 
 // Host side of the function tables: interpolate at Chebyshev nodes in long double, convert to monomials.
-static void cheb_fit(long double (*fn)(long double), long double c, long double hw, int deg, double *out)
+void se_cheb_fit(long double (*fn)(long double, const void *), const void *ctx, long double c, long double hw, int deg,
+                 double *out)
 {
     const int n = deg + 1;
     const long double PI = 3.14159265358979323846264338327950288L;
     long double fv[24], ch[24], T[24][24] = {}, mono[24] = {};
-    for (int k = 0; k < n; ++k) fv[k] = fn(c + hw * cosl(PI * (k + 0.5L) / n));
+    for (int k = 0; k < n; ++k) fv[k] = fn(c + hw * cosl(PI * (k + 0.5L) / n), ctx);
     for (int j = 0; j < n; ++j) {
         long double a = 0;
         for (int k = 0; k < n; ++k) a += fv[k] * cosl(PI * j * (k + 0.5L) / n);
@@ -416,8 +465,8 @@ static void cheb_fit(long double (*fn)(long double), long double c, long double 
         for (int i = 0; i <= j; ++i) mono[i] += ch[j] * T[j][i];
     for (int i = 0; i < n; ++i) out[i] = (double)mono[i];
 }
-static long double erfcx_l(long double x) { return expl(x * x) * erfcl(x); }
-static long double exp_l(long double x) { return expl(x); }
+static long double erfcx_l(long double x, const void *) { return expl(x * x) * erfcl(x); }
+static long double exp_l(long double x, const void *) { return expl(x); }
 
 cudaError_t se_build_mtab(se_plan *p)
 {
@@ -427,8 +476,8 @@ cudaError_t se_build_mtab(se_plan *p)
     for (int i = 0; i < MT_NP; ++i) {
         // pieces centred at i/4, half-width 1/8; monomials in v = x - i/4: divide by (1/8)^k (exact)
         double row[MT_ROW], rowf[MT_ROWF];
-        cheb_fit(erfcx_l, 0.25L * i, 0.125L, MT_DEG, row);
-        cheb_fit(erfcx_l, 0.25L * i, 0.125L, MT_DEGF, rowf);
+        se_cheb_fit(erfcx_l, nullptr, 0.25L * i, 0.125L, MT_DEG, row);
+        se_cheb_fit(erfcx_l, nullptr, 0.25L * i, 0.125L, MT_DEGF, rowf);
         double s = 1.0;
         for (int k = 0; k <= MT_DEG; ++k) { h[i * MT_ROW + k] = row[k] * s; s *= 8.0; }
         s = 1.0;
@@ -437,7 +486,7 @@ cudaError_t se_build_mtab(se_plan *p)
     // e^t: the polynomial is evaluated in t itself, not in t / hw: rescale the monomials
     double e[MT_EXPDEG + 1], ec[MT_EXPDEG + 1];
     const long double hw = 0.34657359027997265470861606072908828L * 1.0001L;   // ln2 / 2 and a little slack
-    cheb_fit(exp_l, 0.0L, hw, MT_EXPDEG, e);
+    se_cheb_fit(exp_l, nullptr, 0.0L, hw, MT_EXPDEG, e);
     long double s = 1;
     for (int k = 0; k <= MT_EXPDEG; ++k) { ec[k] = (double)(e[k] / s); s *= hw; }
     cudaError_t err = cudaMemcpyToSymbol(c_exp, ec, sizeof(ec));
@@ -451,4 +500,25 @@ cudaError_t se_build_mtab(se_plan *p)
 cudaError_t se_launch_p2p(se_plan *p, cudaStream_t s)
 {
     return p->precision == SE_FP64 ? p2p_impl<double>(p, s) : p2p_impl<float>(p, s);
+}
+
+// se.h: counts of the last sorted configuration (synchronises the stream it runs on; allocates 16 bytes)
+extern "C" se_status se_count_pairs(se_plan *p, int64_t *candidates, int64_t *in_range)
+{
+    if (!p || !candidates || !in_range) return SE_EINVAL;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) { cudaGetLastError(); return SE_EINVAL; }
+    unsigned long long *d = nullptr, h[2] = {0, 0};
+    if (cudaMalloc(&d, sizeof(h)) != cudaSuccess) { cudaGetLastError(); return SE_ENOMEM; }
+    cudaMemset(d, 0, sizeof(h));
+    SeGeom g = p->g;
+    g.N = p->T.n;
+    k_count_pairs<<<(unsigned)((g.N + 255) / 256), 256>>>(g, (const float4 *)p->S.xq, p->S.cell_start, (const float4 *)p->T.xq,
+                                                         p->T.cell_sorted, d);
+    cudaError_t e = cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) { cudaGetLastError(); return SE_ECUDA; }
+    *candidates = (int64_t)h[0];
+    *in_range = (int64_t)h[1];
+    return SE_OK;
 }

@@ -1,7 +1,9 @@
 // K4: Fourier-space scaling (CNV), eq. (2.6) with G^F_hat of PAPER.md:69 eq. (2.4b)
-// and the Gaussian window's w_hat(k) = exp(-eta k^2 / 8 xi^2) (reading S4):
+// and the window's transform w_hat(k) = w_hat0(k1) w_hat0(k2) w_hat0(k3):
 //   H~hat(k) = s(k) [k^2 Hhat - k (k.Hhat)],
-//   s(k) = (1/M^3) 8 pi k^-4 (1 + k^2/4xi^2) exp(-(1-eta) k^2/4xi^2),
+//   s(k) = (1/M^3) 8 pi k^-4 (1 + k^2/4xi^2) e(k1) e(k2) e(k3),   e(k_d) = exp(-k_d^2/4xi^2) / w_hat0(k_d)^2
+// (Gaussian window, reading S4: w_hat0 = exp(-eta k_d^2 / 8 xi^2), e = exp(-(1-eta) k_d^2/4xi^2); Kaiser-Bessel:
+// the closed-form transform, reading S20; the table of e per 1-D index is built on the host in se_window.cu),
 // zero at k = 0 (reading S2) and on the Nyquist planes (reading S8).  One thread per stored
 // mode of the R2C half-spectrum (conjugate symmetry).  The exponential factors
 // as a product of three 1-D tables built once per plan, so the kernel is pure HBM streaming:
@@ -14,7 +16,7 @@ template <typename Real> struct Cplx;
 template <> struct Cplx<double> { typedef double2 type; };
 template <> struct Cplx<float> { typedef float2 type; };
 
-// ktab layout: [0..M) k value of index i, [M..2M) exp(-(1-eta) k_i^2 / 4 xi^2)
+// ktab layout: [0..M) k value of index i, [M..2M) e(k_i)
 template <typename Real>
 __global__ void __launch_bounds__(256)
 k_scale(int M, int Mh, Real pref, Real inv4xi2, const Real *__restrict__ ktab,
@@ -45,17 +47,6 @@ k_scale(int M, int Mh, Real pref, Real inv4xi2, const Real *__restrict__ ktab,
 }
 
 template <typename Real>
-__global__ void k_build_ktab(int M, double L, double xi, double eta, Real *ktab)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= M) return;
-    int n = (2 * i >= M) ? i - M : i;
-    double k = 2.0 * SE_PI * (double)n / L;
-    ktab[i] = (Real)k;
-    ktab[M + i] = (Real)exp(-(1.0 - eta) * k * k / (4.0 * xi * xi));
-}
-
-template <typename Real>
 cudaError_t scale_impl(se_plan *p, cudaStream_t s)
 {
     const SeGeom &g = p->g;
@@ -78,16 +69,4 @@ cudaError_t scale_impl(se_plan *p, cudaStream_t s)
 cudaError_t se_launch_scale(se_plan *p, cudaStream_t s)
 {
     return p->precision == SE_FP64 ? scale_impl<double>(p, s) : scale_impl<float>(p, s);
-}
-
-cudaError_t se_build_ktab(se_plan *p)
-{
-    const SeGeom &g = p->g;
-    if (p->precision == SE_FP64)
-        k_build_ktab<double><<<(g.M + 127) / 128, 128>>>(g.M, g.L, g.xi, g.eta, (double *)p->ktab);
-    else
-        k_build_ktab<float><<<(g.M + 127) / 128, 128>>>(g.M, g.L, g.xi, g.eta, (float *)p->ktab);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    return cudaDeviceSynchronize();
 }

@@ -197,20 +197,24 @@ __global__ void k_gather_near(SeGeom g, const Real *__restrict__ x, const Real *
         q[d] = (float)rel;
         if (d == 2) q[3] = (float)v;
         src[6 * p + d] = (Real)(g.rel_coords ? rel : v);
-        src[6 * p + 3 + d] = f[3 * (int64_t)i + d];
+        src[6 * p + 3 + d] = f ? f[3 * (int64_t)i + d] : (Real)0;      // a target set carries no strengths
     }
     xq[p] = make_float4(q[0], q[1], q[2], q[3]);
     cellp[p] = (c[0] << 20) | (c[1] << 10) | c[2];
 }
 
-// one thread per (sorted particle, dim, l): window value exp(-beta (l - (P/2-1) - frac)^2)
-// = exp(-a t_l^2), t_l = (anchor + l) h - x  (reading S11).  Always evaluated in
-// double and rounded once to Real.  In mma mode (fp64) the values go into the per-particle spread and
-// gather records of se_mma.cu (layout in se_common.cuh) instead of the plain [N][3][P] table.
+// one thread per (sorted particle, dim, l): window value at the physical offset t_l = (anchor + l) h - x
+// (reading S11).  Gaussian: exp(-beta (l - (P/2-1) - frac)^2) = exp(-a t_l^2).  Kaiser-Bessel
+// (eq. (2.8)): the polynomial of bin l, degree nu, in s = 2 (t_l/h - (l - P/2)) - 1 by Horner's rule
+// (PAPER.md:421-427), coefficients wcoef[l][0..nu].  Always evaluated in double and rounded once to Rec.  In mma
+// mode the values go into the per-particle spread and gather records of se_mma.cu (layout in se_common.cuh;
+// either pointer may be null: a source-only set has no gather records, a target set no spread records)
+// instead of the plain [N][3][P] table.
 template <typename Real, typename Rec>
 __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *__restrict__ f,
                               const int *__restrict__ perm, short4 *__restrict__ anchor,
-                              Rec *__restrict__ wtab, Rec *__restrict__ recg, Real *__restrict__ fs)
+                              Rec *__restrict__ wtab, Rec *__restrict__ recg, Real *__restrict__ fs,
+                              const double *__restrict__ wcoef)
 {
     // LP = 16 or 32 lanes per particle: lane d < 3 of the group wraps coordinate d and finds its base index once,
     // the group shares them by shuffle, then lane l < P evaluates window value l of each dimension and the rows
@@ -223,32 +227,50 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
     const bool live = p < g.N;
     const int64_t pc = live ? p : g.N - 1;
     const int i = perm[pc];
-    double frac = 0.0;
+    double frac = 0.0, xw = 0.0;
     int i0 = 0;
     Real fd = (Real)0;
     if (l < 3) {
-        i0 = grid_base1(wrap1((double)x[3 * (int64_t)i + l], g.L), g, frac);
-        fd = f[3 * (int64_t)i + l];
+        xw = wrap1((double)x[3 * (int64_t)i + l], g.L);
+        i0 = grid_base1(xw, g, frac);
+        fd = f ? f[3 * (int64_t)i + l] : (Real)0;
     }
     const bool recs = g.grid_mode == 2;
     const int R = recs ? g.ring : P;
     Rec *rs = wtab + pc * SE_MMA_RECS(R), *rg = recg + pc * SE_MMA_RECG(P);
+    const bool kb = g.window == SE_WINDOW_KAISER_BESSEL;
     Rec cf[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) cf[c] = (Rec)g.cw * (Rec)__shfl_sync(0xffffffffu, fd, gbase + c);   // c_w of eq. (2.5) folded in
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         const double fr = __shfl_sync(0xffffffffu, frac, gbase + d);
+        const double xd = __shfl_sync(0xffffffffu, xw, gbase + d);
+        const int id = __shfl_sync(0xffffffffu, i0, gbase + d);
         if (!live || l >= R) continue;
-        const double u = (double)(l - (P / 2 - 1)) - fr;
-        const Rec w = l < P ? (Rec)exp(-g.beta * u * u) : (Rec)0;       // rows are zero beyond the window
+        double wv = 0.0;                                                // rows are zero beyond the window
+        if (l < P) {
+            if (kb) {
+                const double t = (double)(id - (P / 2 - 1) + l) * g.h - xd;
+                const double sv = 2.0 * (t / g.h - (double)(l - P / 2)) - 1.0;
+                const double *cc = wcoef + l * (g.nu + 1);
+                wv = __ldg(cc + g.nu);
+                for (int k = g.nu - 1; k >= 0; --k) wv = fma(wv, sv, __ldg(cc + k));
+            } else {
+                const double u = (double)(l - (P / 2 - 1)) - fr;
+                wv = exp(-g.beta * u * u);
+            }
+        }
+        const Rec w = (Rec)wv;
         if (recs) {
-            if (l < P) rg[d * P + l] = w;
-            if (d == 0) {
+            if (recg && l < P) rg[d * P + l] = w;
+            if (wtab) {
+                if (d == 0) {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) rs[c * R + l] = cf[c] * w;
-            } else
-                rs[(d + 2) * R + l] = w;
+                    for (int c = 0; c < 3; ++c) rs[c * R + l] = cf[c] * w;
+                } else
+                    rs[(d + 2) * R + l] = w;
+            }
         } else if (l < P)
             wtab[pc * P3 + d * P + l] = w;
     }
@@ -260,8 +282,8 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
         if (l == 0) ap[3] = 0;
         fs[3 * p + l] = fd;
         if (recs && l > 0) {
-            reinterpret_cast<int *>(&rs[5 * R])[l - 1] = a;
-            reinterpret_cast<int *>(&rg[P3])[l - 1] = a;
+            if (wtab) reinterpret_cast<int *>(&rs[5 * R])[l - 1] = a;
+            if (recg) reinterpret_cast<int *>(&rg[P3])[l - 1] = a;
         }
     }
 }
@@ -275,45 +297,60 @@ __global__ void k_sum(int64_t N, const Real *__restrict__ uN, const Real *__rest
     if (t >= 3 * N) return;
     int64_t i = t / 3;
     int c = (int)(t - 3 * i);
-    u[t] = uN[3 * (int64_t)inv_near[i] + c] + far_scale * uF[3 * (int64_t)inv_grid[i] + c] - cself * f[t];
+    Real v = uN[3 * (int64_t)inv_near[i] + c] + far_scale * uF[3 * (int64_t)inv_grid[i] + c];
+    if (f) v -= cself * f[t];                        // self term: only when the targets are the sources (reading S3)
+    u[t] = v;
 }
 
+// Sort one point set.  f == nullptr: a target set (no strengths).  spread / gather: which mma-mode records to write.
 template <typename Real>
-cudaError_t sort_impl(se_plan *p, const void *xv, const void *fv, cudaStream_t s)
+cudaError_t sort_set(se_plan *p, SeSet &S, const void *xv, const void *fv, bool spread, bool gather, cudaStream_t s)
 {
-    const SeGeom &g = p->g;
+    SeGeom g = p->g;
+    g.N = S.n;
     const Real *x = (const Real *)xv, *f = (const Real *)fv;
     int nc3 = g.ncell * g.ncell * g.ncell, nb3 = g.nbins_total;
-    cudaMemsetAsync(p->cell_cursor, 0, sizeof(int) * (nc3 + 1), s);
-    cudaMemsetAsync(p->bin_cursor, 0, sizeof(int) * (nb3 + 1), s);
+    cudaError_t e = cudaMemsetAsync(S.cell_cursor, 0, sizeof(int) * (nc3 + 1), s);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(S.bin_cursor, 0, sizeof(int) * (nb3 + 1), s);
+    if (e != cudaSuccess) return e;
     int T = 256;
     unsigned nblk = (unsigned)((g.N + T - 1) / T);
-    k_bin<Real><<<nblk, T, 0, s>>>(g, x, p->cell_of, p->bin_of, p->cell_cursor, p->bin_cursor);
+    k_bin<Real><<<nblk, T, 0, s>>>(g, x, S.cell_of, S.bin_of, S.cell_cursor, S.bin_cursor);
     int tilesA = (nc3 + SCAN_TILE - 1) / SCAN_TILE, tilesB = (nb3 + SCAN_TILE - 1) / SCAN_TILE;
     int tiles = tilesA > tilesB ? tilesA : tilesB;
-    // tile sums live behind the CSR arrays' scratch: reuse perm arrays (N >= 1) is unsafe for tiny N,
-    // so the plan allocates cell_start/bin_start with room for the tile sums after entry n.
-    int *sumsA = p->cell_start + (nc3 + 1), *sumsB = p->bin_start + (nb3 + 1);
-    k_tile_sums<<<dim3(tiles, 2), SCAN_T, 0, s>>>(p->cell_cursor, nc3, sumsA, p->bin_cursor, nb3, sumsB);
-    k_tile_scan<<<dim3(tiles, 2), SCAN_T, 0, s>>>(p->cell_cursor, p->cell_start, nc3, sumsA,
-                                                   p->bin_cursor, p->bin_start, nb3, sumsB);
-    // scatter into scratch permutations (cell_sorted / inv arrays double as scratch), then re-rank
-    int *tmp_near = p->cell_sorted, *tmp_grid = (int *)p->uF;     // both >= N ints, overwritten later
-    k_scatter<<<nblk, T, 0, s>>>(g.N, p->cell_of, p->bin_of, p->cell_cursor, p->bin_cursor,
-                                 tmp_near, p->inv_near, tmp_grid, p->inv_grid);
-    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, p->cell_of, p->cell_start, tmp_near, p->perm_near, p->inv_near);
-    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, p->bin_of, p->bin_start, tmp_grid, p->perm_grid, p->inv_grid);
-    k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, p->perm_near, p->cell_of, (Real *)p->src_near,
-                                           (float4 *)p->xq, p->cell_sorted);
+    // tile sums live behind the CSR arrays: the plan allocates cell_start / bin_start with room for them after entry n
+    int *sumsA = S.cell_start + (nc3 + 1), *sumsB = S.bin_start + (nb3 + 1);
+    k_tile_sums<<<dim3(tiles, 2), SCAN_T, 0, s>>>(S.cell_cursor, nc3, sumsA, S.bin_cursor, nb3, sumsB);
+    k_tile_scan<<<dim3(tiles, 2), SCAN_T, 0, s>>>(S.cell_cursor, S.cell_start, nc3, sumsA,
+                                                   S.bin_cursor, S.bin_start, nb3, sumsB);
+    // scatter into scratch permutations (cell_sorted and the fs_grid array double as scratch), then re-rank
+    int *tmp_near = S.cell_sorted, *tmp_grid = (int *)S.fs_grid;  // both >= n ints, overwritten later
+    k_scatter<<<nblk, T, 0, s>>>(g.N, S.cell_of, S.bin_of, S.cell_cursor, S.bin_cursor,
+                                 tmp_near, S.inv_near, tmp_grid, S.inv_grid);
+    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, S.cell_of, S.cell_start, tmp_near, S.perm_near, S.inv_near);
+    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, S.bin_of, S.bin_start, tmp_grid, S.perm_grid, S.inv_grid);
+    k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, S.perm_near, S.cell_of, (Real *)S.src_near,
+                                           (float4 *)S.xq, S.cell_sorted);
     int64_t nt = (g.N + (g.P <= 16 ? 1 : 0)) / (g.P <= 16 ? 2 : 1) * 32;   // 16 or 32 lanes per particle
     if (g.grid_mode == 2)                                      // records are double for every plan precision
         k_gather_grid<Real, double><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(
-            g, x, f, p->perm_grid, p->anchor, (double *)p->wtab, (double *)p->recg, (Real *)p->fs_grid);
+            g, x, f, S.perm_grid, S.anchor, spread ? (double *)S.wtab : nullptr, gather ? (double *)S.recg : nullptr,
+            (Real *)S.fs_grid, p->wcoef);
     else
         k_gather_grid<Real, Real><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(
-            g, x, f, p->perm_grid, p->anchor, (Real *)p->wtab, (Real *)p->recg, (Real *)p->fs_grid);
+            g, x, f, S.perm_grid, S.anchor, (Real *)S.wtab, (Real *)S.recg, (Real *)S.fs_grid, p->wcoef);
     p->launches += 8;
     return cudaGetLastError();
+}
+
+template <typename Real>
+cudaError_t sort_impl(se_plan *p, const void *xv, const void *fv, const void *xt, cudaStream_t s)
+{
+    if (!p->own_targets) return sort_set<Real>(p, p->S, xv, fv, true, true, s);
+    cudaError_t e = sort_set<Real>(p, p->S, xv, fv, true, false, s);
+    if (e != cudaSuccess) return e;
+    return sort_set<Real>(p, p->T, xt, nullptr, false, true, s);
 }
 
 template <typename Real>
@@ -323,18 +360,20 @@ cudaError_t sum_impl(se_plan *p, const void *f, void *u, cudaStream_t s)
     double far_scale = g.h * g.h * g.h * g.cw;                 // eq. (2.7) h^3 and the window's c_w
     double cself = 4.0 * g.xi / sqrt(SE_PI);                   // self term, reading S3
     int T = 256;
-    k_sum<Real><<<(unsigned)((3 * g.N + T - 1) / T), T, 0, s>>>(g.N, (const Real *)p->uN, (const Real *)p->uF,
-                                                               (const Real *)f, p->inv_near, p->inv_grid,
-                                                               (Real)far_scale, (Real)cself, (Real *)u);
+    const int64_t nt = p->T.n;
+    k_sum<Real><<<(unsigned)((3 * nt + T - 1) / T), T, 0, s>>>(nt, (const Real *)p->uN, (const Real *)p->uF,
+                                                              p->own_targets ? nullptr : (const Real *)f,
+                                                              p->T.inv_near, p->T.inv_grid,
+                                                              (Real)far_scale, (Real)cself, (Real *)u);
     p->launches += 1;
     return cudaGetLastError();
 }
 
 }  // namespace
 
-cudaError_t se_launch_sort(se_plan *p, const void *x, const void *f, cudaStream_t s)
+cudaError_t se_launch_sort(se_plan *p, const void *x, const void *f, const void *xt, cudaStream_t s)
 {
-    return p->precision == SE_FP64 ? sort_impl<double>(p, x, f, s) : sort_impl<float>(p, x, f, s);
+    return p->precision == SE_FP64 ? sort_impl<double>(p, x, f, xt, s) : sort_impl<float>(p, x, f, xt, s);
 }
 
 cudaError_t se_launch_sum(se_plan *p, const void *f, void *u, cudaStream_t s)

@@ -36,6 +36,7 @@ class Config:
     precision: str  # "fp64" | "fp32"
     kind: str       # "uniform" | "spheres"
     label: str
+    window: str = "gaussian"   # "gaussian" | "kb" (Kaiser-Bessel, eq. (2.8))
 
 
 CONFIGS = {

@@ -46,7 +46,7 @@ def run_stages(c, x, f):
     fd = torch.as_tensor(f, dtype=dt, device="cuda").contiguous()
     ud = torch.empty_like(xd)
     out = {}
-    with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P, c.precision) as plan:
+    with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P, c.precision, window=c.window) as plan:
         info = plan.info()
         out["info"] = {k: getattr(info, k) for k, _ in info._fields_}
         plan.stage("sort", x=xd, f=fd)

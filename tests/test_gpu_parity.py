@@ -24,7 +24,8 @@ TOL = {
 
 
 def check_all(c, x, f, tol_override=None):
-    o = oracle.se_eval(x, f, c.L, c.xi, c.rc, c.M, c.P, keep=True)
+    # the CUDA path's Kaiser-Bessel window IS the piecewise polynomial: compare with that variant
+    o = oracle.se_eval(x, f, c.L, c.xi, c.rc, c.M, c.P, keep=True, window="kb_poly" if c.window == "kb" else c.window)
     g = run_stages(c, x, f)
     tol = dict(TOL[c.precision], **(tol_override or {}))
     N = c.N

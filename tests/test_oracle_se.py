@@ -248,3 +248,18 @@ def test_cfg4_like_accuracy():
     ud = oracle.direct_ewald(x, f, c.L, min(c.xi, 12.0))
     e = rel(o["u"], ud)
     assert 1e-7 < e < 1e-4
+
+
+def test_separate_targets(cfg1, cfg1_direct):
+    """N_t != N_s (eq. (1.1)): at targets that ARE the sources the target form gives u + self term
+    (the i = j pair is skipped by r > 0 in both); at other points it matches O1 evaluated at those targets."""
+    c, x, f, o = cfg1
+    sel = np.arange(0, c.N, 7)
+    ot = oracle.se_eval_targets(x, f, x[sel], c.L, c.xi, c.rc, c.M, c.P)
+    self_term = 4 * c.xi / np.sqrt(np.pi) * f[sel]
+    assert rel(ot["u"] - self_term, o["u"][sel]) < 1e-13
+    np.testing.assert_allclose(ot["uN"], o["uN"][sel], rtol=1e-12, atol=1e-12 * np.abs(o["uN"]).max())
+    xt = np.random.default_rng(12).random((150, 3)) * c.L
+    ot = oracle.se_eval_targets(x, f, xt, c.L, c.xi, c.rc, c.M, c.P)
+    ud = oracle.direct_ewald(x, f, c.L, c.xi, targets=xt)
+    assert rel(ot["u"], ud) < 1e-9
