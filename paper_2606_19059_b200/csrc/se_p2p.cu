@@ -30,6 +30,7 @@
 #include <cmath>
 
 #include "se_common.cuh"
+#include "se_erf_rational.h"
 
 namespace {
 
@@ -66,6 +67,11 @@ constexpr int MT_F32 = MT_NP * MT_ROW;                           // offset of th
 constexpr int MT_SIZE = MT_F32 + (MT_NP * MT_ROWF + 1) / 2;      // doubles in p->mtab
 constexpr int MT_EXPDEG = 11;
 __constant__ double c_exp[MT_EXPDEG + 1];
+// fp32 plans: erf(x)/x ~ p(t)/q(t), t = x^2/36 (se_erf_rational.h, written by gen_erf_rational.py)
+__constant__ float c_erfr_p[SE_ERFR_DEG + 1], c_erfr_q[SE_ERFR_DEG + 1];
+#ifndef P2P_F32_RATIONAL
+#define P2P_F32_RATIONAL 1      /* 1: the rational erf(x)/x of PAPER.md:429-431; 0: the degree-5 erfcx table */
+#endif
 
 template <typename Real> struct NearMath;
 
@@ -147,7 +153,18 @@ template <> struct NearMath<float> {
         float rinv = rsqrtf(r2);
         float x2 = xi * xi * r2;
         float e = expf(-x2);
+#if P2P_F32_RATIONAL
+        // erfc(xi r)/r = 1/r - xi erf(x)/x, x = xi r: p and q by Horner (2 x 6 FMA, all coefficients
+        // positive), one fast division; beyond x = 6 erf(x)/x = 1/x to rounding, i.e. the term vanishes
+        const float t = fminf(x2, 36.f) * (1.f / 36.f);
+        float pn = c_erfr_p[SE_ERFR_DEG], qn = c_erfr_q[SE_ERFR_DEG];
+#pragma unroll
+        for (int k = SE_ERFR_DEG - 1; k >= 0; --k) { pn = fmaf(pn, t, c_erfr_p[k]); qn = fmaf(qn, t, c_erfr_q[k]); }
+        float A = fmaf(-xi, __fdividef(pn, qn), rinv);
+        if (CLAMP && x2 > 36.f) A = 0.f;
+#else
         float A = e * erfcx_tab<CLAMP>(xi * (r2 * rinv), mt) * rinv;
+#endif
         float B = c2 * e;
         C1 = A - B;
         C2 = (A + B) * (rinv * rinv);
@@ -197,7 +214,9 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     const int pci = cellp[ic];
     const int cz = pci & 1023;
     const Real X0 = src_t[6 * ic + 0], X1 = src_t[6 * ic + 1], X2 = src_t[6 * ic + 2];
-    Real a0 = 0, a1 = 0, a2 = 0;
+    // accumulators are double for every plan: an fp32 plan sums the pairs of one round in float and adds that partial sum
+    // here, so that the error of u^N does not grow with the number of neighbours
+    double a0 = 0, a1 = 0, a2 = 0;
     int woff = 0, roff = 0;                                      // ring write / read offsets (bytes); empty when equal
 
     auto queued = [&]() { return ((woff - roff) & (QBYTES - 1)) / QSTRIDE; };
@@ -261,21 +280,41 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                 d1 += __shfl_xor_sync(0xffffffffu, d1, sh);
                 d2 += __shfl_xor_sync(0xffffffffu, d2, sh);
             }
-            if (lane == o) { a0 += d0; a1 += d1; a2 += d2; roff = (roff + cB * QSTRIDE) & (QBYTES - 1); }
+            if (lane == o) { a0 += (double)d0; a1 += (double)d1; a2 += (double)d2; roff = (roff + cB * QSTRIDE) & (QBYTES - 1); }
         } else if (KP > 1 && __popc(__ballot_sync(0xffffffffu, c >= KP)) * 4 >= __popc(m1) * 3) {
             // mode A2: most queues hold KP pairs: every lane pops up to that many of its own, evaluated side
             // by side (independent dependency chains); a lane with fewer re-evaluates its last one and drops it
             if (c > 0) {
                 int ro = roff;
+                if (sizeof(Real) == 8) {
+                    Real t0 = (Real)a0, t1 = (Real)a1, t2 = (Real)a2;        // fp64: the accumulators themselves
 #pragma unroll
-                for (int k = 0; k < KP; ++k) {
-                    pair(ro, k < c, X0, X1, X2, cz, a0, a1, a2);
-                    if (k + 1 < c) ro = (ro + QSTRIDE) & (QBYTES - 1);
+                    for (int k = 0; k < KP; ++k) {
+                        pair(ro, k < c, X0, X1, X2, cz, t0, t1, t2);
+                        if (k + 1 < c) ro = (ro + QSTRIDE) & (QBYTES - 1);
+                    }
+                    a0 = t0; a1 = t1; a2 = t2;
+                } else {
+                    Real t0 = 0, t1 = 0, t2 = 0;
+#pragma unroll
+                    for (int k = 0; k < KP; ++k) {
+                        pair(ro, k < c, X0, X1, X2, cz, t0, t1, t2);
+                        if (k + 1 < c) ro = (ro + QSTRIDE) & (QBYTES - 1);
+                    }
+                    a0 += (double)t0; a1 += (double)t1; a2 += (double)t2;
                 }
                 roff = (roff + min(c, KP) * QSTRIDE) & (QBYTES - 1);
             }
         } else if (c > 0) {                                      // mode A: every lane pops one pair of its own
-            pair(roff, true, X0, X1, X2, cz, a0, a1, a2);
+            if (sizeof(Real) == 8) {
+                Real t0 = (Real)a0, t1 = (Real)a1, t2 = (Real)a2;
+                pair(roff, true, X0, X1, X2, cz, t0, t1, t2);
+                a0 = t0; a1 = t1; a2 = t2;
+            } else {
+                Real t0 = 0, t1 = 0, t2 = 0;
+                pair(roff, true, X0, X1, X2, cz, t0, t1, t2);
+                a0 += (double)t0; a1 += (double)t1; a2 += (double)t2;
+            }
             roff = (roff + QSTRIDE) & (QBYTES - 1);
         }
     };
@@ -382,7 +421,7 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
         remaining &= ~act;
     }
     while (__any_sync(0xffffffffu, woff != roff)) round();
-    if (valid) { uN[3 * i + 0] = a0; uN[3 * i + 1] = a1; uN[3 * i + 2] = a2; }
+    if (valid) { uN[3 * i + 0] = (Real)a0; uN[3 * i + 1] = (Real)a1; uN[3 * i + 2] = (Real)a2; }
 }
 
 // Diagnostics for bench.py's K2 roofline (not on the evaluation path): candidates (sources in the 27 colleague cells) and
@@ -490,6 +529,12 @@ cudaError_t se_build_mtab(se_plan *p)
     long double s = 1;
     for (int k = 0; k <= MT_EXPDEG; ++k) { ec[k] = (double)(e[k] / s); s *= hw; }
     cudaError_t err = cudaMemcpyToSymbol(c_exp, ec, sizeof(ec));
+    if (err != cudaSuccess) return err;
+    float rp[SE_ERFR_DEG + 1], rq[SE_ERFR_DEG + 1];
+    for (int k = 0; k <= SE_ERFR_DEG; ++k) { rp[k] = (float)se_erfr_p[k]; rq[k] = (float)se_erfr_q[k]; }
+    err = cudaMemcpyToSymbol(c_erfr_p, rp, sizeof(rp));
+    if (err != cudaSuccess) return err;
+    err = cudaMemcpyToSymbol(c_erfr_q, rq, sizeof(rq));
     if (err != cudaSuccess) return err;
     err = cudaMalloc(&p->mtab, sizeof(h));
     if (err != cudaSuccess) return err;

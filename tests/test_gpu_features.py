@@ -217,3 +217,34 @@ def test_plan_is_bound_to_its_device():
         ua, ub = a.eval(xd, fd), b.eval(xd, fd)
         torch.cuda.synchronize()
         assert rel(ua.cpu().numpy(), ub.cpu().numpy()) < 1e-5
+
+
+def test_fp32_near_field_with_thirty_thousand_neighbours():
+    """fp32 K2 on a dense blob (40,000 points in a ball of radius 0.08, rc = 0.2: ~30,000 in-range sources per target):
+    K2 sums the pairs of a round in float and the rounds in double, so u^N stays inside the 3e-6 gate however many
+    neighbours a target has (a float accumulator drifted to 2.7e-5 here, VERDICT r01 weak #7).  Not a BASELINE workload."""
+    import torch
+    import paper_2606_19059_b200 as se
+    rng = np.random.default_rng(190590 + 77)
+    N, L, rc = 40000, 1.0, 0.2
+    xi = 3.195 / rc                                            # config 4's xi rc
+    v = rng.standard_normal((N, 3))
+    v /= np.linalg.norm(v, axis=1)[:, None]
+    x = (0.5 + 0.08 * rng.random((N, 1)) ** (1.0 / 3.0) * v).astype(np.float32)
+    f = rng.standard_normal((N, 3)).astype(np.float32)
+    xd = torch.as_tensor(x, device="cuda"); fd = torch.as_tensor(f, device="cuda")
+    with se.Plan(N, L, xi, rc, 32, 12, "fp32") as plan:
+        plan.stage("sort", x=xd, f=fd)
+        perm = plan.read(se.SE_BUF_PERM_NEAR).cpu().numpy()
+        plan.stage("p2p")
+        uN_sorted = plan.read(se.SE_BUF_UN).cpu().numpy()
+        cand, hits = plan.count_pairs()
+    assert hits / N > 25000
+    uN = np.empty_like(uN_sorted)
+    uN[perm] = uN_sorted
+    # the oracle on a sample of targets (O(N) each), in double on the rounded inputs (reading S17)
+    xw = oracle.wrap(x.astype(np.float64), L)
+    idx = rng.choice(N, 256, replace=False)
+    ref = oracle.near_brute(xw, f.astype(np.float64), L, xi, rc, targets=idx)
+    e, m = gate("uN dense blob fp32", uN[idx], ref, TOL["fp32"]["uN"])
+    print(f"fp32 u^N with {hits / N:.0f} neighbours per target: rel-L2 {e:.2e}, max-abs {m:.2e}")
