@@ -16,17 +16,22 @@
 //   phase B (heavy; FP64 pipe, FP32 for fp32 plans): in a round every lane pops one pair of its own queue:
 //            exact r from the full-precision coordinates in the form of eq. (2.2), x_i - (x_j + p), the exact
 //            test 0 < r^2 <= rc^2 (reading S6), and G^N evaluated in registers as
-//              C1 = A - B,  C2 = (A + B)/r^2,  A = e^{-xi^2 r^2} erfcx(xi r)/r,  B = 2 xi e^{-xi^2 r^2}/sqrt(pi)
-//            (erfc(x) = e^{-x^2} erfcx(x): one exponential serves both terms of (2.3)).  Rounds run only when
-//            the fullest queue of the warp needs room, so that all lanes stay busy; the lane adds into its own
-//            three accumulators (no reduction) and writes u^N_i itself.
+//              C1 = A - B,  C2 = (A + B)/r^2,  A = erfc(xi r)/r = 1/r - xi erf(x)/x (x = xi r),  B = 2 xi e^{-x^2}/sqrt(pi),
+//            erf(x)/x being the rational p(x^2)/q(x^2) of PAPER.md:429-431 (degree 12 over 12 in double, 6 over 6 in
+//            single precision; se_erf_rational.h), 1/r a hardware seed with one correction, e^{-x^2} a degree-11
+//            polynomial (expf in single precision): no libm calls, no table look-ups.  (A table-driven erfcx, the first
+//            design, is kept behind P2P_F64_RATIONAL = 0 / P2P_F32_RATIONAL = 0: same accuracy, 11 shared-memory loads
+//            per pair more, and K2 is bound by shared-memory wavefronts before FP64 issue, profiles/r02a.)  Rounds run
+//            only when the fullest queue of the warp needs room, so that all lanes stay busy; the lane adds into its
+//            own three accumulators (no reduction; double for every plan, an fp32 plan adding one float partial sum
+//            per round) and writes u^N_i itself.
 // A warp whose targets span several cells processes them in passes: the targets of one z-row of cells whose
 // cell index is within P2P_ZSPAN of the first; a lane only accepts sources of its own 27 colleague cells.
 // A queue entry is 16 bits: (virtual cell << 9) | offset, a virtual cell being <= 512 consecutive sources of one
 // colleague cell; a per-warp table maps it to the first source index and to the periodic image shift p of that
 // cell (three reals, written once when the virtual cell is opened).  fp32 plans use cell-relative positions in
-// phase B too, so that r keeps full float precision across images; their erfcx is a degree-5 table of the same
-// form as the double one (the fresh single-precision path: no libm erfc, no division).
+// phase B too, so that r keeps full float precision across images (the fresh single-precision path of north_star: the
+// rational erf(x)/x, no libm erfc).
 #include <cmath>
 
 #include "se_common.cuh"
@@ -67,16 +72,21 @@ constexpr int MT_F32 = MT_NP * MT_ROW;                           // offset of th
 constexpr int MT_SIZE = MT_F32 + (MT_NP * MT_ROWF + 1) / 2;      // doubles in p->mtab
 constexpr int MT_EXPDEG = 11;
 __constant__ double c_exp[MT_EXPDEG + 1];
-// fp32 plans: erf(x)/x ~ p(t)/q(t), t = x^2/36 (se_erf_rational.h, written by gen_erf_rational.py)
-__constant__ float c_erfr_p[SE_ERFR_DEG + 1], c_erfr_q[SE_ERFR_DEG + 1];
+// erf(x)/x ~ p(t)/q(t), t = x^2/36 (se_erf_rational.h, written by gen_erf_rational.py): degree 6 over 6
+// for fp32 plans, 12 over 12 for fp64 plans; in constant memory, so that the coefficients are FMA operands, not loads
+__constant__ float c_erfr_p32[SE_ERFR_DEG_F32 + 1], c_erfr_q32[SE_ERFR_DEG_F32 + 1];
+__constant__ double c_erfr_p64[SE_ERFR_DEG_F64 + 1], c_erfr_q64[SE_ERFR_DEG_F64 + 1];
 #ifndef P2P_F32_RATIONAL
 #define P2P_F32_RATIONAL 1      /* 1: the rational erf(x)/x of PAPER.md:429-431; 0: the degree-5 erfcx table */
+#endif
+#ifndef P2P_F64_RATIONAL
+#define P2P_F64_RATIONAL 1      /* 1: rational erf(x)/x (no table look-ups: K2 is bound by shared-memory wavefronts); 0: erfcx table */
 #endif
 
 template <typename Real> struct NearMath;
 
 template <> struct NearMath<double> {
-    static constexpr int TAB = MT_NP * MT_ROW;                   // table entries in shared memory
+    static constexpr int TAB = P2P_F64_RATIONAL ? 1 : MT_NP * MT_ROW;     // table entries in shared memory
     static __device__ __forceinline__ void load(double *mt, const double *mtab, int tid, int nt)
     {
         for (int e = tid; e < TAB; e += nt) mt[e] = mtab[e];
@@ -116,12 +126,36 @@ template <> struct NearMath<double> {
         const double e = fma(-(x * y), y, 1.0);
         return fma(y * e, fma(0.375, e, 0.5), y);
     }
+    // 1/x, x in [1, 1e6]: hardware seed (2^-23) and two Newton steps
+    static __device__ __forceinline__ double rcp(double x)
+    {
+        double y;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+        y = fma(y, fma(-x, y, 1.0), y);
+        return fma(y, fma(-x, y, 1.0), y);
+    }
     template <bool CLAMP>
     static __device__ __forceinline__ void coeffs(double r2, double xi, double c2, const double *mt, double &C1, double &C2)
     {
         const double rinv = rsq(r2);
-        const double e = exp_neg<CLAMP>(xi * xi * r2);
+        const double x2 = xi * xi * r2;
+        const double e = exp_neg<CLAMP>(x2);
+#if P2P_F64_RATIONAL
+        // erfc(xi r)/r = 1/r - xi erf(x)/x, x = xi r: p and q by Horner (2 x 12 FMA, all coefficients
+        // positive: no cancellation), q >= 1; the quotient gets one residual correction.  The difference cancels for
+        // large x, which costs nothing: its error, ~1e-16 / r, is that of the two terms, i.e. of every near pair.
+        const double t = fmin(x2, 36.0) * (1.0 / 36.0);
+        double pn = c_erfr_p64[SE_ERFR_DEG_F64], qn = c_erfr_q64[SE_ERFR_DEG_F64];
+#pragma unroll
+        for (int k = SE_ERFR_DEG_F64 - 1; k >= 0; --k) { pn = fma(pn, t, c_erfr_p64[k]); qn = fma(qn, t, c_erfr_q64[k]); }
+        const double y = rcp(qn);
+        double R = pn * y;
+        R = fma(fma(-qn, R, pn), y, R);
+        double A = fma(-xi, R, rinv);
+        if (CLAMP && x2 > 36.0) A = 0.0;
+#else
         const double A = e * erfcx_tab<CLAMP>(xi * (r2 * rinv), mt) * rinv;
+#endif
         const double B = c2 * e;
         C1 = A - B;
         C2 = (A + B) * (rinv * rinv);
@@ -129,7 +163,7 @@ template <> struct NearMath<double> {
 };
 
 template <> struct NearMath<float> {
-    static constexpr int TAB = MT_NP * MT_ROWF;
+    static constexpr int TAB = P2P_F32_RATIONAL ? 1 : MT_NP * MT_ROWF;
     static __device__ __forceinline__ void load(float *mt, const double *mtab, int tid, int nt)
     {
         const float *src = reinterpret_cast<const float *>(mtab + MT_F32);
@@ -157,9 +191,9 @@ template <> struct NearMath<float> {
         // erfc(xi r)/r = 1/r - xi erf(x)/x, x = xi r: p and q by Horner (2 x 6 FMA, all coefficients
         // positive), one fast division; beyond x = 6 erf(x)/x = 1/x to rounding, i.e. the term vanishes
         const float t = fminf(x2, 36.f) * (1.f / 36.f);
-        float pn = c_erfr_p[SE_ERFR_DEG], qn = c_erfr_q[SE_ERFR_DEG];
+        float pn = c_erfr_p32[SE_ERFR_DEG_F32], qn = c_erfr_q32[SE_ERFR_DEG_F32];
 #pragma unroll
-        for (int k = SE_ERFR_DEG - 1; k >= 0; --k) { pn = fmaf(pn, t, c_erfr_p[k]); qn = fmaf(qn, t, c_erfr_q[k]); }
+        for (int k = SE_ERFR_DEG_F32 - 1; k >= 0; --k) { pn = fmaf(pn, t, c_erfr_p32[k]); qn = fmaf(qn, t, c_erfr_q32[k]); }
         float A = fmaf(-xi, __fdividef(pn, qn), rinv);
         if (CLAMP && x2 > 36.f) A = 0.f;
 #else
@@ -171,8 +205,8 @@ template <> struct NearMath<float> {
     }
 };
 
-// CLAMP: xi rc is so large that the table argument must be clamped (plans with xi rc <= 7.8 never leave the tables:
-// every evaluated pair has r <= rc, a rejected one is evaluated at r = rc)
+// CLAMP: xi rc is so large that the arguments of the function approximations must be clamped (other plans never leave
+// their range: every evaluated pair has r <= rc, a rejected one is evaluated at r = rc)
 template <typename Real, bool CLAMP>
 __global__ void __launch_bounds__(P2P_WARPS * 32, P2P_BLOCKS)
 k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, const int *__restrict__ cell_start,
@@ -470,7 +504,10 @@ cudaError_t p2p_impl(se_plan *p, cudaStream_t s)
     // FP32 filter margin: the cell-relative coordinates are < 2 wcell in magnitude, each rounded to 6e-8
     // relative, so |dr| < 1e-6 wcell per component and |d r^2| < 2 sqrt(3) rc 1e-6 wcell
     const double rc2m = g.rc * g.rc * (1.0 + 1e-5) + 4e-6 * g.rc * g.wcell;
-    if (g.xi * g.rc > 7.8)
+    // CLAMP instantiation: plans whose arguments can leave the range of the function approximations (x = xi r <= 6 for
+    // the rational erf(x)/x, 7.8 for the erfcx tables); every evaluated pair has r <= rc
+    const bool rational = p->precision == SE_FP64 ? P2P_F64_RATIONAL != 0 : P2P_F32_RATIONAL != 0;
+    if (g.xi * g.rc > (rational ? 5.99 : 7.8))
         k_p2p<Real, true><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)S.xq, (const Real *)S.src_near, S.cell_start,
                                                          (const float4 *)T.xq, (const Real *)T.src_near, T.cell_sorted,
                                                          p->mtab, (Real *)p->uN, (float)rc2m);
@@ -530,11 +567,15 @@ cudaError_t se_build_mtab(se_plan *p)
     for (int k = 0; k <= MT_EXPDEG; ++k) { ec[k] = (double)(e[k] / s); s *= hw; }
     cudaError_t err = cudaMemcpyToSymbol(c_exp, ec, sizeof(ec));
     if (err != cudaSuccess) return err;
-    float rp[SE_ERFR_DEG + 1], rq[SE_ERFR_DEG + 1];
-    for (int k = 0; k <= SE_ERFR_DEG; ++k) { rp[k] = (float)se_erfr_p[k]; rq[k] = (float)se_erfr_q[k]; }
-    err = cudaMemcpyToSymbol(c_erfr_p, rp, sizeof(rp));
+    float rp[SE_ERFR_DEG_F32 + 1], rq[SE_ERFR_DEG_F32 + 1];
+    for (int k = 0; k <= SE_ERFR_DEG_F32; ++k) { rp[k] = (float)se_erfr_p32[k]; rq[k] = (float)se_erfr_q32[k]; }
+    err = cudaMemcpyToSymbol(c_erfr_p32, rp, sizeof(rp));
     if (err != cudaSuccess) return err;
-    err = cudaMemcpyToSymbol(c_erfr_q, rq, sizeof(rq));
+    err = cudaMemcpyToSymbol(c_erfr_q32, rq, sizeof(rq));
+    if (err != cudaSuccess) return err;
+    err = cudaMemcpyToSymbol(c_erfr_p64, se_erfr_p64, sizeof(se_erfr_p64));
+    if (err != cudaSuccess) return err;
+    err = cudaMemcpyToSymbol(c_erfr_q64, se_erfr_q64, sizeof(se_erfr_q64));
     if (err != cudaSuccess) return err;
     err = cudaMalloc(&p->mtab, sizeof(h));
     if (err != cudaSuccess) return err;
