@@ -45,13 +45,16 @@ constexpr int P2P_CHUNK = 32;       // sources scanned between two queue-room ch
 constexpr int P2P_VBITS = 9;        // a queue entry = (virtual cell << VBITS) | offset: virtual cells of <= 512 sources
 constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV << VBITS) = 2^15)
 #ifndef P2P_TWO
-#define P2P_TWO 3
+#define P2P_TWO 4
 #endif
 #ifndef P2P_TWO_F32
 #define P2P_TWO_F32 6
 #endif
 #ifndef P2P_FU
-#define P2P_FU 4            /* filter group (sources loaded ahead of the queue stores): fp64; fp32 uses twice as many */
+#define P2P_FU 16           /* filter group (sources loaded ahead of the queue stores), fp64 plans */
+#endif
+#ifndef P2P_FU_F32
+#define P2P_FU_F32 8        /* the same for fp32 plans */
 #endif
 #ifndef P2P_BLOCKS
 #define P2P_BLOCKS 4
@@ -374,7 +377,10 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
             int nx = cxl + dx, ny = cyl + dy;
             if (nx < 0) nx += nc; else if (nx >= nc) nx -= nc;
             if (ny < 0) ny += nc; else if (ny >= nc) ny -= nc;
-            const float tx = tx0 - (float)dx * wf, ty = qi.y - (float)dy * wf;
+            float tx = tx0 - (float)dx * wf, ty = qi.y - (float)dy * wf;
+            // opaque: under register pressure the compiler re-derives both from rr inside the filter loop (18 of its 74
+            // instructions per 4 sources, profiles/r02k)
+            asm volatile("" : "+f"(tx), "+f"(ty));
             // lane k holds the CSR range of source cell k of this row
             int cb = 0, ce = 0;
             if (lane < ncl) {
@@ -432,7 +438,7 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                         const int ebase = (vslot << P2P_VBITS) + (j0 - v0);
                         // groups of P2P_FU sources: all broadcast loads of a group first (the queue stores that
                         // follow are shared-memory stores the compiler must order against later loads)
-                        constexpr int FU = sizeof(Real) == 8 ? P2P_FU : 2 * P2P_FU;
+                        constexpr int FU = sizeof(Real) == 8 ? P2P_FU : P2P_FU_F32;
 #pragma unroll 1
                         for (int jb = 0; jb < n; jb += FU) {
                             float4 q[FU];
