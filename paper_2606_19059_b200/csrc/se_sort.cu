@@ -210,7 +210,8 @@ __global__ void k_gather_near(SeGeom g, const Real *__restrict__ x, const Real *
 // mode the values go into the per-particle spread and gather records of se_mma.cu (layout in se_common.cuh;
 // either pointer may be null: a source-only set has no gather records, a target set no spread records)
 // instead of the plain [N][3][P] table.
-template <typename Real, typename Rec>
+// KB: Kaiser-Bessel plans (compile-time: the Gaussian path keeps its registers and its schedule)
+template <typename Real, typename Rec, bool KB>
 __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *__restrict__ f,
                               const int *__restrict__ perm, short4 *__restrict__ anchor,
                               Rec *__restrict__ wtab, Rec *__restrict__ recg, Real *__restrict__ fs,
@@ -238,7 +239,6 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
     const bool recs = g.grid_mode == 2;
     const int R = recs ? g.ring : P;
     Rec *rs = wtab + pc * SE_MMA_RECS(R), *rg = recg + pc * SE_MMA_RECG(P);
-    const bool kb = g.window == SE_WINDOW_KAISER_BESSEL;
     Rec cf[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) cf[c] = (Rec)g.cw * (Rec)__shfl_sync(0xffffffffu, fd, gbase + c);   // c_w of eq. (2.5) folded in
@@ -250,7 +250,7 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
         if (!live || l >= R) continue;
         double wv = 0.0;                                                // rows are zero beyond the window
         if (l < P) {
-            if (kb) {
+            if (KB) {
                 const double t = (double)(id - (P / 2 - 1) + l) * g.h - xd;
                 const double sv = 2.0 * (t / g.h - (double)(l - P / 2)) - 1.0;
                 const double *cc = wcoef + l * (g.nu + 1);
@@ -333,13 +333,20 @@ cudaError_t sort_set(se_plan *p, SeSet &S, const void *xv, const void *fv, bool 
     k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, S.perm_near, S.cell_of, (Real *)S.src_near,
                                            (float4 *)S.xq, S.cell_sorted);
     int64_t nt = (g.N + (g.P <= 16 ? 1 : 0)) / (g.P <= 16 ? 2 : 1) * 32;   // 16 or 32 lanes per particle
-    if (g.grid_mode == 2)                                      // records are double for every plan precision
-        k_gather_grid<Real, double><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(
-            g, x, f, S.perm_grid, S.anchor, spread ? (double *)S.wtab : nullptr, gather ? (double *)S.recg : nullptr,
-            (Real *)S.fs_grid, p->wcoef);
+    const unsigned ngb = (unsigned)((nt + T - 1) / T);
+    const bool kb = g.window == SE_WINDOW_KAISER_BESSEL;
+    if (g.grid_mode == 2) {                                    // records are double for every plan precision
+        double *ws = spread ? (double *)S.wtab : nullptr, *wg = gather ? (double *)S.recg : nullptr;
+        if (kb)
+            k_gather_grid<Real, double, true><<<ngb, T, 0, s>>>(g, x, f, S.perm_grid, S.anchor, ws, wg, (Real *)S.fs_grid, p->wcoef);
+        else
+            k_gather_grid<Real, double, false><<<ngb, T, 0, s>>>(g, x, f, S.perm_grid, S.anchor, ws, wg, (Real *)S.fs_grid, p->wcoef);
+    } else if (kb)
+        k_gather_grid<Real, Real, true><<<ngb, T, 0, s>>>(g, x, f, S.perm_grid, S.anchor, (Real *)S.wtab, (Real *)S.recg,
+                                                            (Real *)S.fs_grid, p->wcoef);
     else
-        k_gather_grid<Real, Real><<<(unsigned)((nt + T - 1) / T), T, 0, s>>>(
-            g, x, f, S.perm_grid, S.anchor, (Real *)S.wtab, (Real *)S.recg, (Real *)S.fs_grid, p->wcoef);
+        k_gather_grid<Real, Real, false><<<ngb, T, 0, s>>>(g, x, f, S.perm_grid, S.anchor, (Real *)S.wtab, (Real *)S.recg,
+                                                             (Real *)S.fs_grid, p->wcoef);
     p->launches += 8;
     return cudaGetLastError();
 }
