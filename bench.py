@@ -36,8 +36,10 @@ UNIT = "particles/s"
 # 1.965 GHz) and the fallback HBM figure of /opt/skills/guides/B200_PROFILING.md; used only when the measured ones
 # (se_measure_peak: register-only DFMA / DMMA / FFMA chains, run before the timed region) are unavailable.
 NOMINAL_TFLOPS = {"fp64": 148 * 64 * 2 * 1.965e9 / 1e12, "fp32": 148 * 128 * 2 * 1.965e9 / 1e12}
-# FP64 (FP32) arithmetic instructions K2 spends per in-range pair (DESIGN.md section 6 "K2"): the "alu" work of P2P
-P2P_INSTR_PER_PAIR = 64
+# FP64 (FP32) arithmetic instructions K2 spends per in-range pair (DESIGN.md section 6 "K2"): the "alu" work of P2P.
+# fp64: 60 DFMA + 10.5 DMUL + 7 DADD + 3 DSETP per pair in the SASS of the evaluation round (profiles/r02m_final.md);
+# fp32: the same algorithm with the degree-6 rational and expf, counted from the source
+P2P_INSTR_PER_PAIR = {"fp64": 80, "fp32": 50}
 # sub-results of the default run (world size 1): (key, config, steps, plan overrides)
 SUB_RESULTS = [("cfg5", 5, 3, {}), ("cfg4", 4, 5, {}),
                ("cfg3_kb_P12", 3, 5, {"window": "kb", "P": 12}), ("cfg5_kb_P12", 5, 3, {"window": "kb", "P": 12}),
@@ -108,7 +110,7 @@ def stage_work(c, P, stage, pairs):
     if stage in ("p2g", "g2p"):
         return {"bound": "alu", "work": 2.0 * 3 * P ** 3 * N, "unit": "TFLOP/s"}
     if stage == "p2p" and pairs:
-        return {"bound": "alu", "work": 2.0 * P2P_INSTR_PER_PAIR * pairs, "unit": "TFLOP/s"}
+        return {"bound": "alu", "work": 2.0 * P2P_INSTR_PER_PAIR[c.precision] * pairs, "unit": "TFLOP/s"}
     if stage == "scale":
         return {"bound": "hbm", "work": 12.0 * B * nk, "unit": "GB/s"}
     if stage in ("fft", "ifft"):
