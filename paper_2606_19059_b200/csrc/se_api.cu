@@ -31,7 +31,7 @@ void free_all(se_plan *p)
 {
     if (!p) return;
     auto free_set = [](SeSet &Q) {
-        void *ptrs[] = {Q.cell_of, Q.cell_start, Q.cell_cursor, Q.perm_near, Q.inv_near, Q.cell_sorted, Q.src_near, Q.xq,
+        void *ptrs[] = {Q.cell_of, Q.cell_start, Q.cell_cursor, Q.perm_near, Q.inv_near, Q.cell_sorted, Q.src_near, Q.xq, Q.xp,
                         Q.bin_of, Q.bin_start, Q.bin_cursor, Q.perm_grid, Q.inv_grid, Q.anchor, Q.wtab, Q.recg, Q.fs_grid};
         for (void *q : ptrs) if (q) cudaFree(q);
     };
@@ -258,6 +258,7 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
         A.get(&Q.cell_sorted, n * sizeof(int));
         A.get(&Q.src_near, n * 6 * rb);
         A.get(&Q.xq, n * sizeof(float4));
+        A.get(&Q.xp, 2 * (size_t)SE_XP_LEN(n) * 16);
         A.get(&Q.bin_of, n * sizeof(int));
         A.get(&Q.bin_start, (nb3 + 1 + scan_tiles) * sizeof(int));
         A.get(&Q.bin_cursor, (nb3 + 1) * sizeof(int));

@@ -32,6 +32,7 @@ constexpr int SE_MMA_ZBIN = 8;
 constexpr int SE_MMA_NWY = 2, SE_MMA_NWZ = 6;
 #define SE_MMA_RECS(P) (5 * (P) + 4)
 #define SE_MMA_RECG(P) (3 * (P) + 4)
+#define SE_XP_LEN(n) (((n) + 1) / 2 + 1)
 
 struct SeGeom {
     int64_t N;          // points of the set a launch works on (sources or targets; the launchers set it)
@@ -68,7 +69,10 @@ struct SeSet {
     int *inv_near;                 // [n] user index -> sorted pos
     int *cell_sorted;              // [n] packed cell coordinates (cx << 20 | cy << 10 | cz) of sorted particle
     void *src_near;                // [n][6] Real: x, y, z (absolute fp64 / cell-relative fp32), f_x, f_y, f_z (0 for targets)
-    void *xq;                      // [n] float4: cell-relative x, y, z and absolute z in FP32 (K2 candidate filter)
+    void *xq;                      // [n] float4: cell-relative x, y, z and absolute z in FP32 (K2: the targets' side of the filter)
+    void *xp;                      // K2 candidate filter, the sources' side: FP16 PAIR records (x0 x1 | y0 y1 | z0 z1 | 0), coordinates
+                                   // relative to the cell in units of the cell width; two arrays of SE_XP_LEN(n) records: [0] pairs
+                                   // (2m, 2m + 1), [1] pairs (2m + 1, 2m + 2), so that a cell's sources pair up from its first one
     // grid path (K1b, K3, K5)
     int *bin_of;                   // [n]
     int *bin_start;                // [nbins_total + 1]

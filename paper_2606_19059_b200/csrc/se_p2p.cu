@@ -5,14 +5,16 @@
 // thread-per-target loop runs the expensive erfc/exp code at ~15% lane utilisation, and on
 // B200 the FP64 pipe (64 lanes per SM) is the scarce resource.  Here a LANE owns a target (32 consecutive
 // targets of the near-sorted order per warp) and the work is split by pipe:
-//   phase A (filter; FP32 pipe; sources fetched 32 at a time, one coalesced 16-byte load per lane one chunk ahead,
-//            and broadcast from a shared-memory line): the warp walks the sources of the
-//            colleague cells; every lane forms r^2 to its own target in FP32 from the compact copy `xq` K1
-//            wrote (coordinates relative to the particle's cell, so periodic images cost nothing) and, if
-//            r^2 <= rc^2 (1 + margin), appends the source index to ITS OWN ring queue in shared memory
-//            (one predicated store; no ballot, no compaction, ~11 instructions per 32 pair tests).  The
-//            margin bounds the FP32 rounding, so no in-range pair is lost; the few extra ones are rejected
-//            exactly in phase B;
+//   phase A (filter; packed FP16, two sources per instruction; sources fetched 32 at a time as 16 pair records, one
+//            coalesced 16-byte load per lane one chunk ahead, and broadcast from a shared-memory line): the warp walks
+//            the sources of the colleague cells; every lane forms r^2 to its own target from the FP16 pair records
+//            `xp` K1 wrote (coordinates relative to the particle's cell in units of the cell width, so periodic images
+//            cost nothing): 3 HADD2, HMUL2, 2 HFMA2 and one packed compare per PAIR of sources, whose two predicates
+//            guard the appends of the source indices to the lane's OWN ring queue in shared memory (predicated
+//            stores; no ballot, no compaction; ~10 instructions per 32 pair tests).  The threshold carries a margin
+//            that bounds the FP16 rounding (p2p_impl below), so no in-range pair is lost; the ~2 % extra ones are
+//            rejected exactly in phase B.  (P2P_HALF2 = 0 selects the first design, the same test in FP32 from `xq`:
+//            15 instructions per 32 tests.)
 //   phase B (heavy; FP64 pipe, FP32 for fp32 plans): in a round every lane pops one pair of its own queue:
 //            exact r from the full-precision coordinates in the form of eq. (2.2), x_i - (x_j + p), the exact
 //            test 0 < r^2 <= rc^2 (reading S6), and G^N evaluated in registers as
@@ -33,6 +35,8 @@
 // phase B too, so that r keeps full float precision across images (the fresh single-precision path of north_star: the
 // rational erf(x)/x, no libm erfc).
 #include <cmath>
+
+#include <cuda_fp16.h>
 
 #include "se_common.cuh"
 #include "se_erf_rational.h"
@@ -58,6 +62,9 @@ constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV 
 #endif
 #ifndef P2P_BLOCKS
 #define P2P_BLOCKS 4
+#endif
+#ifndef P2P_HALF2
+#define P2P_HALF2 1         /* 1: the filter tests two sources per instruction in packed FP16; 0: one per instruction in FP32 */
 #endif
 constexpr int P2P_ZSPAN = 6;        // cells along z a pass may span (<= 29: one lane per source cell)
 
@@ -212,7 +219,8 @@ template <> struct NearMath<float> {
 // their range: every evaluated pair has r <= rc, a rejected one is evaluated at r = rc)
 template <typename Real, bool CLAMP>
 __global__ void __launch_bounds__(P2P_WARPS * 32, P2P_BLOCKS)
-k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, const int *__restrict__ cell_start,
+k_p2p(SeGeom g, const float4 *__restrict__ xq, const uint4 *__restrict__ xp, int64_t ns, const Real *__restrict__ src,
+      const int *__restrict__ cell_start,
       const float4 *__restrict__ xq_t, const Real *__restrict__ src_t, const int *__restrict__ cellp,
       const double *__restrict__ mtab, Real *__restrict__ uN, float rc2m)
 {
@@ -233,8 +241,10 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     const Real xi = (Real)g.xi;
     const Real c2 = (Real)(2.0 * g.xi / sqrt(SE_PI));
     const Real Lr = (Real)g.L, wc = (Real)g.wcell;
+#if !P2P_HALF2
     const float wf = (float)g.wcell;
     constexpr float FAR = 1.0e18f;                               // coordinate of a lane that must not match
+#endif
     char *const Qb = reinterpret_cast<char *>(&qsm[w][0][lane]); // this lane's queue column, slot stride 64 B
     constexpr int QSTRIDE = 64, QBYTES = P2P_QC * QSTRIDE;
     int *const VT = vtab[w];
@@ -248,6 +258,15 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
     const bool valid = i < g.N;
     const int64_t ic = valid ? i : g.N - 1;
     const float4 qi = xq_t[ic];
+#if P2P_HALF2
+    const float inv_wf = (float)(1.0 / g.wcell);
+    const float ux = qi.x * inv_wf, uy = qi.y * inv_wf, uz = qi.z * inv_wf;      // target, in units of the cell width
+    const __half2 thr2 = __halves2half2(__float2half_ru(rc2m), __float2half_ru(rc2m));
+    const unsigned qb_s = (unsigned)__cvta_generic_to_shared(Qb);
+    const uint4 *const xpo = xp + SE_XP_LEN(ns);                  // the odd-pair array
+    constexpr float FAR_T = 200.f;                               // target coordinate of a lane that must not match
+    const unsigned far2 = 0xd640d640u;                           // (-100, -100) in FP16: a source that is never in range
+#endif
     const int pci = cellp[ic];
     const int cz = pci & 1023;
     const Real X0 = src_t[6 * ic + 0], X1 = src_t[6 * ic + 1], X2 = src_t[6 * ic + 2];
@@ -367,7 +386,9 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
         const unsigned act = __ballot_sync(0xffffffffu, member) & remaining;
         const int span = __reduce_max_sync(0xffffffffu, member ? dzl : 0);
         const int ncl = span + 3;                                // source cells k = 0 .. ncl-1 <-> cell czl - 1 + k
+#if !P2P_HALF2
         const float tx0 = ((act >> lane) & 1u) ? qi.x : FAR;
+#endif
 
         // colleague rows in centre-out order, alternating sides, and the cells of a row centre-out as well: every
         // lane then receives its hits at a roughly steady rate, which keeps all 32 queues non-empty
@@ -377,10 +398,12 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
             int nx = cxl + dx, ny = cyl + dy;
             if (nx < 0) nx += nc; else if (nx >= nc) nx -= nc;
             if (ny < 0) ny += nc; else if (ny >= nc) ny -= nc;
-            float tx = tx0 - (float)dx * wf, ty = qi.y - (float)dy * wf;
-            // opaque: under register pressure the compiler re-derives both from rr inside the filter loop (18 of its 74
-            // instructions per 4 sources, profiles/r02k)
-            asm volatile("" : "+f"(tx), "+f"(ty));
+#if P2P_HALF2
+            const __half2 hx2 = __float2half2_rn((((act >> lane) & 1u) ? ux : FAR_T) - (float)dx);
+            const __half2 hy2 = __float2half2_rn(uy - (float)dy);
+#else
+            const float tx = tx0 - (float)dx * wf, ty = qi.y - (float)dy * wf;
+#endif
             // lane k holds the CSR range of source cell k of this row
             int cb = 0, ce = 0;
             if (lane < ncl) {
@@ -396,7 +419,11 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                 const int jb = __shfl_sync(0xffffffffu, cb, k), je = __shfl_sync(0xffffffffu, ce, k);
                 // a lane accepts the cell only if it is one of its own three colleague cells of this row
                 const int dk = k - 1 - dzl;
+#if P2P_HALF2
+                const __half2 hz2 = __float2half2_rn((dk >= -1 && dk <= 1) ? uz - (float)dk : FAR_T);
+#else
                 const float tz = (dk >= -1 && dk <= 1) ? qi.z - (float)dk * wf : FAR;
+#endif
 #pragma unroll 1
                 for (int v0 = jb; v0 < je; v0 += (1 << P2P_VBITS)) {
                     // open a virtual cell; its table slot may still be referenced by queued entries of the
@@ -421,6 +448,67 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                     }
                     __syncwarp();
                     const int ve = min(je, v0 + (1 << P2P_VBITS));
+#if P2P_HALF2
+                    // The 32 sources of a chunk are 16 FP16 pair records (K1: relative to the cell, in units of its width):
+                    // lanes 0..15 fetch one each, one chunk ahead, and the warp reads them back as broadcasts.  A cell pairs
+                    // its sources up from its first one (even or odd pair array by the parity of that index); a half past
+                    // the cell's end is replaced by a coordinate that is never in range.
+                    const uint4 *const xpc = (v0 & 1) ? xpo : xp;
+                    auto load_pair = [&](int j0) {
+                        uint4 r = make_uint4(far2, far2, far2, 0u);
+                        const int s0 = j0 + 2 * lane;
+                        if (lane < 16 && s0 < ve) {
+                            r = __ldg(xpc + (s0 >> 1));
+                            if (s0 + 1 >= ve) { r.x = (r.x & 0xffffu) | (far2 << 16); r.y = (r.y & 0xffffu) | (far2 << 16); r.z = (r.z & 0xffffu) | (far2 << 16); }
+                        }
+                        return r;
+                    };
+                    uint4 nxt = load_pair(v0);
+                    uint4 *const SB2 = reinterpret_cast<uint4 *>(SB);
+#pragma unroll 1
+                    for (int j0 = v0; j0 < ve; j0 += P2P_CHUNK) {
+                        const uint4 cur = nxt;
+                        nxt = load_pair(j0 + P2P_CHUNK);
+                        while (__any_sync(0xffffffffu, queued() > P2P_QC - 1 - P2P_CHUNK)) round();
+                        const int n2 = (min(P2P_CHUNK, ve - j0) + 1) >> 1;       // pairs in this chunk
+                        if (lane < 16) SB2[lane] = cur;
+                        __syncwarp();
+                        const int ebase = (vslot << P2P_VBITS) + (j0 - v0);
+                        // groups of FU2 pairs: all broadcast loads of a group first; per pair 3 HADD2, 1 HMUL2, 2 HFMA2 and one
+                        // packed compare whose two predicates guard the two queue pushes
+                        constexpr int FU2 = 8;
+#pragma unroll 1
+                        for (int pb = 0; pb < n2; pb += FU2) {
+                            uint4 q[FU2];
+#pragma unroll
+                            for (int u = 0; u < FU2; ++u) q[u] = SB2[pb + u];
+#pragma unroll
+                            for (int u = 0; u < FU2; ++u) {
+                                const __half2 rx = __hsub2(hx2, *reinterpret_cast<const __half2 *>(&q[u].x));
+                                const __half2 ry = __hsub2(hy2, *reinterpret_cast<const __half2 *>(&q[u].y));
+                                const __half2 rz = __hsub2(hz2, *reinterpret_cast<const __half2 *>(&q[u].z));
+                                const __half2 r2 = __hfma2(rz, rz, __hfma2(ry, ry, __hmul2(rx, rx)));
+                                const unsigned short e0 = (unsigned short)(ebase + 2 * (pb + u)), e1 = (unsigned short)(e0 + 1);
+                                asm volatile("{\n"
+                                             ".reg .pred p, q;\n"
+                                             ".reg .b32 a;\n"
+                                             "setp.le.f16x2 p|q, %1, %2;\n"
+                                             "add.u32 a, %3, %0;\n"
+                                             "@p st.shared.u16 [a], %4;\n"
+                                             "@p add.u32 %0, %0, 64;\n"
+                                             "@p and.b32 %0, %0, %6;\n"
+                                             "add.u32 a, %3, %0;\n"
+                                             "@q st.shared.u16 [a], %5;\n"
+                                             "@q add.u32 %0, %0, 64;\n"
+                                             "@q and.b32 %0, %0, %6;\n"
+                                             "}"
+                                             : "+r"(woff)
+                                             : "r"(*reinterpret_cast<const unsigned *>(&r2)), "r"(*reinterpret_cast<const unsigned *>(&thr2)),
+                                               "r"(qb_s), "h"(e0), "h"(e1), "r"(QBYTES - 1)
+                                             : "memory");
+                            }
+                        }
+#else
                     // the 32 sources of a chunk are fetched with one coalesced 16-byte load per lane, one chunk
                     // ahead (the load of chunk k + 1 is in flight while chunk k is tested), and broadcast through
                     // a per-warp shared-memory line
@@ -453,6 +541,7 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const Real *__restrict__ src, con
                                 }
                             }
                         }
+#endif
                         __syncwarp();
                     }
                 }
@@ -507,18 +596,28 @@ cudaError_t p2p_impl(se_plan *p, cudaStream_t s)
     const SeSet &S = p->S, &T = p->T;
     int64_t per_block = (int64_t)P2P_WARPS * 32;
     unsigned nblk = (unsigned)((g.N + per_block - 1) / per_block);
+#if P2P_HALF2
+    // Filter threshold on r^2 in units of the cell width w (rho = rc / w <= 1), in FP16 arithmetic.  Rounding moves a source
+    // (s in [0, 1)) by at most 2^-12, a target (|t| < 2) by 2^-11 and their difference (|d| <= 1 for a pair in range) by
+    // 2^-11 per component: |d - r_c| <= 1.22e-3, so sum d^2 <= rho^2 + 4.3e-3 rho + 4.5e-6; the three roundings of the sum
+    // add at most 3 x 2^-11 of it.  The threshold is rounded up to FP16; ~1.7 % of the candidates it lets through are out
+    // of range and rejected exactly in phase B.
+    const double rho = g.rc / g.wcell;
+    const double rc2m = (rho * rho + 4.3e-3 * rho + 4.5e-6) * (1.0 + 1.5e-3) + 1e-4;
+#else
     // FP32 filter margin: the cell-relative coordinates are < 2 wcell in magnitude, each rounded to 6e-8
     // relative, so |dr| < 1e-6 wcell per component and |d r^2| < 2 sqrt(3) rc 1e-6 wcell
     const double rc2m = g.rc * g.rc * (1.0 + 1e-5) + 4e-6 * g.rc * g.wcell;
+#endif
     // CLAMP instantiation: plans whose arguments can leave the range of the function approximations (x = xi r <= 6 for
     // the rational erf(x)/x, 7.8 for the erfcx tables); every evaluated pair has r <= rc
     const bool rational = p->precision == SE_FP64 ? P2P_F64_RATIONAL != 0 : P2P_F32_RATIONAL != 0;
     if (g.xi * g.rc > (rational ? 5.99 : 7.8))
-        k_p2p<Real, true><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)S.xq, (const Real *)S.src_near, S.cell_start,
+        k_p2p<Real, true><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)S.xq, (const uint4 *)S.xp, S.n, (const Real *)S.src_near, S.cell_start,
                                                          (const float4 *)T.xq, (const Real *)T.src_near, T.cell_sorted,
                                                          p->mtab, (Real *)p->uN, (float)rc2m);
     else
-        k_p2p<Real, false><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)S.xq, (const Real *)S.src_near, S.cell_start,
+        k_p2p<Real, false><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)S.xq, (const uint4 *)S.xp, S.n, (const Real *)S.src_near, S.cell_start,
                                                           (const float4 *)T.xq, (const Real *)T.src_near, T.cell_sorted,
                                                           p->mtab, (Real *)p->uN, (float)rc2m);
     p->launches += 1;

@@ -5,6 +5,8 @@
 // the lists are CSR (start offsets + a permutation), so clustered inputs cost no padding.
 // The grid ordering also stores, per particle, the anchor grid index and the
 // three 1-D Gaussian window tables of P values each, so that P2G and G2P never evaluate exp.
+#include <cuda_fp16.h>
+
 #include "se_common.cuh"
 
 namespace {
@@ -182,7 +184,8 @@ __global__ void k_rank_in_cell(int64_t N, const int *__restrict__ key_of, const 
 template <typename Real>
 __global__ void k_gather_near(SeGeom g, const Real *__restrict__ x, const Real *__restrict__ f,
                               const int *__restrict__ perm, const int *__restrict__ cell_of,
-                              Real *__restrict__ src, float4 *__restrict__ xq, int *__restrict__ cellp)
+                              Real *__restrict__ src, float4 *__restrict__ xq, unsigned short *__restrict__ xp,
+                              int *__restrict__ cellp)
 {
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= g.N) return;
@@ -201,6 +204,20 @@ __global__ void k_gather_near(SeGeom g, const Real *__restrict__ x, const Real *
     }
     xq[p] = make_float4(q[0], q[1], q[2], q[3]);
     cellp[p] = (c[0] << 20) | (c[1] << 10) | c[2];
+    // FP16 pair records of the K2 filter (se_common.cuh): this point is half (p & 1) of even pair p >> 1 and half
+    // ((p - 1) & 1) of odd pair (p - 1) >> 1; a half without a point (past the end) holds a coordinate that is never in range
+    const size_t odd = (size_t)SE_XP_LEN(g.N) * 8;             // offset of the odd-pair array, in halves
+    const unsigned short farh = 0xd640;                         // -100 in FP16
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const unsigned short hv = __half_as_ushort(__float2half_rn(q[d] * (float)(1.0 / g.wcell)));
+        xp[(size_t)(p >> 1) * 8 + 2 * d + (p & 1)] = hv;
+        if (p > 0) xp[odd + (size_t)((p - 1) >> 1) * 8 + 2 * d + ((p - 1) & 1)] = hv;
+        if (p == g.N - 1) {                                     // the halves behind the last point
+            if (!(p & 1)) xp[(size_t)(p >> 1) * 8 + 2 * d + 1] = farh;
+            if (p > 0 && !((p - 1) & 1)) xp[odd + (size_t)((p - 1) >> 1) * 8 + 2 * d + 1] = farh;
+        }
+    }
 }
 
 // one thread per (sorted particle, dim, l): window value at the physical offset t_l = (anchor + l) h - x
@@ -331,7 +348,7 @@ cudaError_t sort_set(se_plan *p, SeSet &S, const void *xv, const void *fv, bool 
     k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, S.cell_of, S.cell_start, tmp_near, S.perm_near, S.inv_near);
     k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, S.bin_of, S.bin_start, tmp_grid, S.perm_grid, S.inv_grid);
     k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, S.perm_near, S.cell_of, (Real *)S.src_near,
-                                           (float4 *)S.xq, S.cell_sorted);
+                                           (float4 *)S.xq, (unsigned short *)S.xp, S.cell_sorted);
     int64_t nt = (g.N + (g.P <= 16 ? 1 : 0)) / (g.P <= 16 ? 2 : 1) * 32;   // 16 or 32 lanes per particle
     const unsigned ngb = (unsigned)((nt + T - 1) / T);
     const bool kb = g.window == SE_WINDOW_KAISER_BESSEL;
