@@ -116,6 +116,7 @@ typedef struct {
     int window;          /* se_window                                                    */
     int nu;              /* Kaiser-Bessel: degree of the piecewise polynomial            */
     double kb_beta;      /* Kaiser-Bessel: beta = 2.5 P ; a_w = P h / 2                  */
+    int Mx, px0;         /* planes of the plan's grid along x (M unless a slab plan) and global index of plane 0 */
 } se_info;
 
 /* Everything se_plan_create takes, plus the window and an optional separate target count. */
@@ -127,6 +128,14 @@ typedef struct {
     int M, P;
     int precision;       /* se_precision */
     int window;          /* se_window    */
+    int Mx;              /* 0: the plan's grid is the whole M^3 grid.  > 0: SLAB plan ("equisized slabs along the
+                            periodic spatial dimension"): the plan's grid holds Mx x M x M points, local plane l being global
+                            plane (px0 + l) mod M; every SOURCE / TARGET handed to it must have its window inside that
+                            range, i.e. floor(x/h) - (P/2 - 1) - px0 (mod M) in [0, Mx - P].  A slab plan runs the stages
+                            SORT, P2P, P2G, G2P, SUM; FFT / SCALE / IFFT return SE_EINVAL (the transform of the assembled
+                            grid belongs to a whole-grid plan).  Needs a (P, precision) of the tensor-core gridding
+                            kernels and Mx >= P rounded up to a multiple of 8. */
+    int px0;             /* slab plans: global index of local plane 0, in [0, M)            */
 } se_plan_desc;
 
 /*

@@ -37,12 +37,13 @@ class SeInfo(C.Structure):
                 ("ncell", C.c_int), ("nbin", C.c_int), ("grid_mode", C.c_int), ("nbins_total", C.c_int),
                 ("nchunk", C.c_int), ("nmodes", C.c_int64),
                 ("workspace_bytes", C.c_size_t), ("Nt", C.c_int64), ("window", C.c_int), ("nu", C.c_int),
-                ("kb_beta", C.c_double)]
+                ("kb_beta", C.c_double), ("Mx", C.c_int), ("px0", C.c_int)]
 
 
 class SePlanDesc(C.Structure):
     _fields_ = [("N", C.c_int64), ("Nt", C.c_int64), ("L", C.c_double), ("xi", C.c_double), ("rc", C.c_double),
-                ("M", C.c_int), ("P", C.c_int), ("precision", C.c_int), ("window", C.c_int)]
+                ("M", C.c_int), ("P", C.c_int), ("precision", C.c_int), ("window", C.c_int),
+                ("Mx", C.c_int), ("px0", C.c_int)]
 
 
 class SeParams(C.Structure):
@@ -129,7 +130,8 @@ def measure_peak(which, reps=5) -> float:
 class Plan:
     """se_plan_create[_ex|_tol] / se_eval / se_plan_destroy with torch tensors for memory."""
 
-    def __init__(self, N, L, xi=None, rc=None, M=None, P=None, precision="fp64", window="gaussian", Nt=0, eps=None):
+    def __init__(self, N, L, xi=None, rc=None, M=None, P=None, precision="fp64", window="gaussian", Nt=0, eps=None,
+                 Mx=0, px0=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_19059_b200 needs a CUDA device (no CPU fallback)")
@@ -144,13 +146,14 @@ class Plan:
             _check(lib().se_plan_create_tol(C.byref(self._h), int(N), int(Nt), float(L), float(eps), win, prec,
                                             C.byref(self.chosen)), "se_plan_create_tol")
             M, P = self.chosen.M, self.chosen.P
-        elif win == SE_WINDOW_GAUSSIAN and not Nt:
+        elif win == SE_WINDOW_GAUSSIAN and not Nt and not Mx:
             _check(lib().se_plan_create(C.byref(self._h), int(N), float(L), float(xi), float(rc), int(M), int(P), prec),
                    "se_plan_create")
         else:
-            d = SePlanDesc(int(N), int(Nt), float(L), float(xi), float(rc), int(M), int(P), prec, win)
+            d = SePlanDesc(int(N), int(Nt), float(L), float(xi), float(rc), int(M), int(P), prec, win, int(Mx), int(px0))
             _check(lib().se_plan_create_ex(C.byref(self._h), C.byref(d)), "se_plan_create_ex")
         self.N, self.M, self.P, self.Nt = int(N), int(M), int(P), int(Nt)
+        self.Mx, self.px0 = (int(Mx), int(px0)) if Mx else (int(M), 0)       # slab plans (se.h se_plan_desc)
 
     # -- lifetime -----------------------------------------------------------------------
     def destroy(self):
@@ -232,7 +235,7 @@ class Plan:
         if which in (SE_BUF_UN, SE_BUF_UF):
             return (self.Nt or self.N, 3), self.dtype
         if which == SE_BUF_GRID:
-            return (3, M, M, M), self.dtype
+            return (3, self.Mx, M, M), self.dtype
         if which == SE_BUF_SPEC:
             return (3, M, M, M // 2 + 1, 2), self.dtype
         if which in (SE_BUF_PERM_NEAR, SE_BUF_PERM_GRID):

@@ -74,9 +74,9 @@ se_status run_stage(se_plan *p, int stage, const void *x, const void *f, void *u
         break;
     case SE_STAGE_P2P: e = se_launch_p2p(p, s); break;
     case SE_STAGE_P2G: e = se_launch_p2g(p, s); break;
-    case SE_STAGE_FFT: return run_fft(p, true, s);
-    case SE_STAGE_SCALE: e = se_launch_scale(p, s); break;
-    case SE_STAGE_IFFT: return run_fft(p, false, s);
+    case SE_STAGE_FFT: if (p->slab) return SE_EINVAL; return run_fft(p, true, s);
+    case SE_STAGE_SCALE: if (p->slab) return SE_EINVAL; e = se_launch_scale(p, s); break;
+    case SE_STAGE_IFFT: if (p->slab) return SE_EINVAL; return run_fft(p, false, s);
     case SE_STAGE_G2P: e = se_launch_g2p(p, s); break;
     case SE_STAGE_SUM:
         if ((!f && !p->own_targets) || !u) return SE_EINVAL;
@@ -91,13 +91,13 @@ size_t buffer_bytes(const se_plan *p, int which, void **ptr)
 {
     const SeGeom &g = p->g;
     size_t rb = p->real_bytes;
-    size_t M3 = (size_t)g.M * g.M * g.M, nm = (size_t)g.M * g.M * (g.M / 2 + 1);
+    size_t M3 = (size_t)g.Mx * g.M * g.M, nm = p->slab ? 0 : (size_t)g.M * g.M * (g.M / 2 + 1);
     const SeSet &Q = (which & SE_BUF_TARGETS) ? p->T : p->S;       // PERM / START ids: which point set
     switch (which & ~SE_BUF_TARGETS) {
     case SE_BUF_UN: *ptr = p->uN; return (size_t)p->T.n * 3 * rb;
     case SE_BUF_UF: *ptr = p->uF; return (size_t)p->T.n * 3 * rb;
     case SE_BUF_GRID: *ptr = p->grid; return 3 * M3 * rb;
-    case SE_BUF_SPEC: *ptr = p->spec; return 3 * nm * 2 * rb;
+    case SE_BUF_SPEC: *ptr = p->slab ? nullptr : p->spec; return 3 * nm * 2 * rb;
     case SE_BUF_PERM_NEAR: *ptr = Q.perm_near; return (size_t)Q.n * sizeof(int);
     case SE_BUF_PERM_GRID: *ptr = Q.perm_grid; return (size_t)Q.n * sizeof(int);
     case SE_BUF_CELL_START: *ptr = Q.cell_start; return ((size_t)g.ncell * g.ncell * g.ncell + 1) * sizeof(int);
@@ -127,7 +127,7 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
 {
     se_plan_desc d{};
     d.N = N; d.Nt = 0; d.L = L; d.xi = xi; d.rc = rc; d.M = M; d.P = P;
-    d.precision = (int)prec; d.window = SE_WINDOW_GAUSSIAN;
+    d.precision = (int)prec; d.window = SE_WINDOW_GAUSSIAN; d.Mx = 0; d.px0 = 0;
     return se_plan_create_ex(out, &d);
 }
 
@@ -139,6 +139,8 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
     const int64_t N = d->N, Nt = d->Nt;
     const double L = d->L, xi = d->xi, rc = d->rc;
     const int M = d->M, P = d->P, prec = d->precision, window = d->window;
+    const int Mx = d->Mx > 0 ? d->Mx : M, px0 = d->Mx > 0 ? d->px0 : 0;
+    const bool slab = d->Mx > 0;
     if (!(N >= 1) || N >= ((int64_t)1 << 31) || Nt < 0 || Nt >= ((int64_t)1 << 31) || !(L > 0) || !(xi > 0) || !(rc > 0) ||
         !std::isfinite(L) || !std::isfinite(xi) || !std::isfinite(rc))
         return SE_EINVAL;
@@ -146,6 +148,7 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
     if (prec != SE_FP64 && prec != SE_FP32) return SE_EINVAL;
     if (window != SE_WINDOW_GAUSSIAN && window != SE_WINDOW_KAISER_BESSEL) return SE_EINVAL;
     if (window == SE_WINDOW_KAISER_BESSEL && P > 16) return SE_EINVAL;
+    if (slab && (Mx > M || Mx < se_mma_ring(P) || Mx < P || px0 < 0 || px0 >= M || !se_mma_supported(P, prec))) return SE_EINVAL;
     double ncd = std::floor(L / rc);
     if (!(ncd >= 3)) return SE_EINVAL;
     // near cells: floor(L / rc) per dimension (reading S7), but no more than ~8 cells per point (wider cells stay
@@ -163,8 +166,10 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
     p->precision = prec;
     p->real_bytes = prec == SE_FP64 ? 8 : 4;
     p->own_targets = Nt > 0;
+    p->slab = slab ? 1 : 0;
     SeGeom &g = p->g;
     g.N = N; g.M = M; g.P = P; g.L = L; g.xi = xi; g.rc = rc;
+    g.Mx = Mx; g.px0 = px0;
     g.window = window;
     g.nu = window == SE_WINDOW_KAISER_BESSEL ? se_kb_degree(P) : 0;
     g.ncell = ncell;
@@ -178,13 +183,13 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
         const bool want_tile = force && std::strcmp(force, "tile") == 0;
         const int zb = (M + SE_MMA_ZBIN - 1) / SE_MMA_ZBIN;
         // the sort key has M * zb * M bins: beyond ~64 bins per point the per-evaluation scan would dominate
-        const double nbins_mma = (double)M * zb * M;
-        if (se_mma_supported(P, prec) && se_mma_ring(P) <= M && nbins_mma < 5.0e8 &&
-            nbins_mma <= 64.0 * (double)std::max(N, Nt) + 4.0e6 && !want_tile) {
+        const double nbins_mma = (double)Mx * zb * M;
+        if (se_mma_supported(P, prec) && se_mma_ring(P) <= Mx && nbins_mma < 5.0e8 &&
+            (slab || (nbins_mma <= 64.0 * (double)std::max(N, Nt) + 4.0e6 && !want_tile))) {
             g.grid_mode = 2;
             g.ring = se_mma_ring(P);
             g.nbin = zb;
-            g.nbins_total = M * zb * M;
+            g.nbins_total = Mx * zb * M;
             const int BY = 4 * SE_MMA_NWY, BZ = 4 * SE_MMA_NWZ;
             const int tiles = ((M + BY - 1) / BY) * ((M + BZ - 1) / BZ);
             // One block per SM, so the grid should fill whole waves of one block per SM (148).  A P2G chunk re-spreads P - 1
@@ -201,19 +206,19 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
                 for (int n = 1; n <= std::max(1, nmax); ++n) {
                     const double w = (double)tiles * n / nsm;
                     double cost = std::ceil(w) / w;
-                    const double cl = (double)M / n;
+                    const double cl = (double)Mx / n;
                     if (spread) cost *= n == 1 ? 1.0 : (cl + P - 1) / cl;
                     else cost *= 1.0 + 0.15 * (P - 1) / cl;
                     if (cost < bc - 1e-9) { bc = cost; best = n; }
                 }
                 return best;
             };
-            int nch = pick(M / (4 * P), true);
-            int nchg = pick(2 * M / P, false);                  // G2P chunks may be as short as P / 2 planes
+            int nch = pick(Mx / (4 * P), true);
+            int nchg = pick(2 * Mx / P, false);                  // G2P chunks may be as short as P / 2 planes
             const char *e = std::getenv("SE_NCHUNK");
-            if (e && std::atoi(e) > 0) nch = std::min(std::atoi(e), M);
+            if (e && std::atoi(e) > 0) nch = std::min(std::atoi(e), Mx);
             e = std::getenv("SE_NCHUNK_G2P");
-            if (e && std::atoi(e) > 0) nchg = std::min(std::atoi(e), M);
+            if (e && std::atoi(e) > 0) nchg = std::min(std::atoi(e), Mx);
             g.nchunk = std::max(nch, 1);
             g.nchunk_g2p = std::max(nchg, 1);
             // P2G with whole sweeps: if the last wave is partly filled, split only its tiles along x (each piece pays
@@ -222,8 +227,8 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
             const int R = tiles % nsm;
             if (g.nchunk == 1 && R > 0 && tiles > nsm && !std::getenv("SE_NCHUNK")) {
                 double best = 0.95;
-                for (int k = 2; k <= 4 && M / k >= P; ++k) {
-                    const double cost = std::ceil((double)R * k / nsm) * ((double)M / k + P - 1) / M;
+                for (int k = 2; k <= 4 && Mx / k >= P; ++k) {
+                    const double cost = std::ceil((double)R * k / nsm) * ((double)Mx / k + P - 1) / Mx;
                     if (cost < best) { best = cost; g.nsplit = k; g.nfull = tiles - R; }
                 }
             }
@@ -244,7 +249,8 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
 
     size_t rb = p->real_bytes;
     size_t nc3 = (size_t)ncell * ncell * ncell, nb3 = (size_t)g.nbins_total;
-    size_t M3 = (size_t)M * M * M, nm = (size_t)M * M * (M / 2 + 1);
+    if (slab && g.grid_mode != 2) { delete p; return SE_EINVAL; }
+    size_t M3 = (size_t)Mx * M * M, nm = slab ? 0 : (size_t)M * M * (M / 2 + 1);
     size_t scan_tiles = (std::max(nc3, nb3) + 2047) / 2048 + 1;
 
     Alloc A{p};
@@ -291,13 +297,16 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
     int n[3] = {M, M, M};
     cufftType tf = prec == SE_FP64 ? CUFFT_D2Z : CUFFT_R2C, ti = prec == SE_FP64 ? CUFFT_Z2D : CUFFT_C2R;
     size_t wsz = 0;
-    cufftResult r = cufftPlanMany(&p->fft_fwd, 3, n, nullptr, 1, (int)0, nullptr, 1, (int)0, tf, 3);
-    if (r == CUFFT_SUCCESS) {
+    cufftResult r = slab ? CUFFT_SUCCESS : cufftPlanMany(&p->fft_fwd, 3, n, nullptr, 1, (int)0, nullptr, 1, (int)0, tf, 3);
+    if (slab) {
+        // a slab plan transforms nothing: the assembled grid belongs to a whole-grid plan
+    } else if (r == CUFFT_SUCCESS) {
         p->fft_ok |= 1;
         if (cufftGetSize(p->fft_fwd, &wsz) == CUFFT_SUCCESS) p->fft_work_bytes += wsz;
         r = cufftPlanMany(&p->fft_inv, 3, n, nullptr, 1, (int)0, nullptr, 1, (int)0, ti, 3);
     }
-    if (r == CUFFT_SUCCESS) {
+    if (slab) {
+    } else if (r == CUFFT_SUCCESS) {
         p->fft_ok |= 2;
         if (cufftGetSize(p->fft_inv, &wsz) == CUFFT_SUCCESS) p->fft_work_bytes += wsz;
     } else {
@@ -369,6 +378,7 @@ se_status se_plan_info(const se_plan *p, se_info *o)
     o->ncell = g.ncell; o->nbin = g.nbin;
     o->grid_mode = g.grid_mode; o->nbins_total = g.nbins_total; o->nchunk = g.nchunk;
     o->nmodes = (int64_t)g.M * g.M * (g.M / 2 + 1);
+    o->Mx = g.Mx; o->px0 = g.px0;
     o->workspace_bytes = p->workspace_bytes;
     return SE_OK;
 }
@@ -409,13 +419,13 @@ static se_status run_all(se_plan *p, const void *x, const void *f, void *u, void
 
 se_status se_eval(se_plan *p, const void *x, const void *f, void *u, void *stream)
 {
-    if (!p || !x || !f || !u || p->own_targets || !on_device(p)) return SE_EINVAL;
+    if (!p || !x || !f || !u || p->own_targets || p->slab || !on_device(p)) return SE_EINVAL;
     return run_all(p, x, f, u, stream);
 }
 
 se_status se_eval_targets(se_plan *p, const void *xs, const void *f, const void *xt, void *ut, void *stream)
 {
-    if (!p || !xs || !f || !xt || !ut || !p->own_targets || !on_device(p)) return SE_EINVAL;
+    if (!p || !xs || !f || !xt || !ut || !p->own_targets || p->slab || !on_device(p)) return SE_EINVAL;
     p->xt_stage = xt;
     return run_all(p, xs, f, ut, stream);
 }

@@ -37,6 +37,7 @@ constexpr int SE_MMA_NWY = 2, SE_MMA_NWZ = 6;
 struct SeGeom {
     int64_t N;          // points of the set a launch works on (sources or targets; the launchers set it)
     int M, P;
+    int Mx, px0;        // planes of the grid along x (M unless a slab plan) and global index of local plane 0
     int window;         // se_window
     int nu;             // Kaiser-Bessel: polynomial degree per bin
     int ncell;          // near cells per dimension
@@ -95,6 +96,7 @@ struct se_plan {
     SeSet S;                       // sources
     SeSet T;                       // targets: a copy of S (same pointers) unless the plan has its own targets
     int own_targets;               // 1: T has its own arrays (se_eval_targets)
+    int slab;                      // 1: slab plan (grid Mx x M x M, no transforms; se.h se_plan_desc)
     const void *xt_stage;          // se_set_targets: target positions for se_eval_stage(SE_STAGE_SORT)
     double *wcoef;                 // Kaiser-Bessel: [P][nu + 1] polynomial coefficients (always double)
     void *uN;                      // [Nt][3] Real, the targets' near-sorted order

@@ -161,7 +161,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
     Smem<P, SPREAD> &S = *reinterpret_cast<Smem<P, SPREAD> *>(smem_raw);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int M = g.M, nzb = g.nbin;
+    const int M = g.M, Mx = g.Mx, nzb = g.nbin;            // Mx planes along x (the sweep direction), M along y and z
     const int ntY = (M + BY - 1) / BY, ntZ = (M + BZ - 1) / BZ;
     int tile = blockIdx.x % (ntZ * ntY), chunk = blockIdx.x / (ntZ * ntY);
     int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
@@ -171,9 +171,9 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
         else { const int bb = blockIdx.x - g.nfull; tile = g.nfull + bb / g.nsplit; chunk = bb % g.nsplit; nchunk = g.nsplit; }
     }
     const int tz = tile % ntZ, ty = tile / ntZ;
-    const int CL = (M + nchunk - 1) / nchunk;
+    const int CL = (Mx + nchunk - 1) / nchunk;
     const int X0 = chunk * CL;
-    const int CLen = min(CL, M - X0);
+    const int CLen = min(CL, Mx - X0);
     if (CLen <= 0) return;
     const int Y0 = ty * BY, Z0 = tz * BZ;
     // P2G: a chunk re-spreads the P - 1 anchor planes in front of it (warm-up) -- except when one chunk covers the
@@ -253,7 +253,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
         auto run_of = [&](int s, int &beg, int &len) {
             beg = 0; len = 0;
             if (s < s_end && r1 > r0) {
-                const int base = modM(s, M) * nzb * M + zoff;
+                const int base = modM(s, Mx) * nzb * M + zoff;
                 beg = __ldg(&bin_start[base + r0]);
                 len = __ldg(&bin_start[base + r1]) - beg;
             }
@@ -317,17 +317,17 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
     const int wy0 = 4 * (warp / NWZ), wz0 = 4 * (warp % NWZ);       // warp patch inside the block tile
     const int Yw = Y0 + wy0, Zw = Z0 + wz0;
     const int nyw = min(4, M - Yw), nzw = min(4, M - Zw);           // valid rows / columns of the patch
-    const size_t MM = (size_t)M * M, M3 = MM * M;
+    const size_t MM = (size_t)M * M, M3 = MM * Mx;
     WarpScratch<P, SPREAD> &WS = S.ws[warp];
     // Both kernels see the patch as two n-tiles of 8 columns: column n of n-tile j is row 2j + (n >> 2),
     // z-column n & 3 of the patch.
 
     // cur: P2G first plane not yet flushed; G2P first plane not yet in the ring.  curP = cur mod P, curM = cur mod M.
-    int cur = s_begin, curP = modM(s_begin, P), curM = modM(s_begin, M);
+    int cur = s_begin, curP = modM(s_begin, P), curM = modM(s_begin, Mx);
     auto advance = [&]() {
         ++cur;
         if (++curP == P) curP = 0;
-        if (++curM == M) curM = 0;
+        if (++curM == Mx) curM = 0;
     };
 
     // this warp's hits of a round: packed list (candidate, window index of the patch origin in y and z), padded
@@ -530,16 +530,16 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                 break;
             }
             // planes s .. s+P-1 must be in the ring; plane cur may be waiting in `pre`
-            if (cur < s) { cur = s; curP = rs; curM = modM(s, M); pre_X = INT_MIN; }   // planes nobody gathers from
+            if (cur < s) { cur = s; curP = rs; curM = modM(s, Mx); pre_X = INT_MIN; }  // planes nobody gathers from
             if (s + P - cur > 2) {
                 // (re)fill after a chunk start or a jump: all missing planes of this lane's k-columns at once (one
                 // memory latency instead of one per plane); residue 4 ks + tq holds plane s + ((4 ks + tq - rs) mod P)
-                const int sM = modM(s, M);
+                const int sM = modM(s, Mx);
 #pragma unroll
                 for (int ks = 0; ks < KS; ++ks) {
                     int l = 4 * ks + tq - rs; if (l < 0) l += P;
                     if (s + l < cur) continue;                       // still valid in the ring
-                    int XM = sM + l; if (XM >= M) XM -= M;
+                    int XM = sM + l; if (XM >= Mx) XM -= Mx;
                     const size_t off = (size_t)XM * MM + colG;
 #pragma unroll
                     for (int c = 0; c < 3; ++c)
@@ -547,7 +547,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
                         for (int j = 0; j < 2; ++j)
                             rg[ks][c][j] = (gz_ok && 2 * j + gyl < nyw) ? (double)__ldg(&grid[c * M3 + off + (size_t)(2 * j) * M]) : 0.0;
                 }
-                cur = s + P; curP = rs; curM = modM(cur, M); pre_X = INT_MIN;
+                cur = s + P; curP = rs; curM = modM(cur, Mx); pre_X = INT_MIN;
             }
             while (cur < s + P) {
                 if (pre_X != cur) fetch_plane(cur, curP, curM);

@@ -54,6 +54,9 @@ __global__ void k_bin(SeGeom g, const Real *__restrict__ x, int *__restrict__ ce
         int a[3];                                    // anchors, wrapped into [0, M)
 #pragma unroll
         for (int d = 0; d < 3; ++d) { a[d] = b[d] - (g.P / 2 - 1); if (a[d] < 0) a[d] += g.M; }
+        // slab plans: local plane of the anchor (a point whose window leaves the slab is the caller's error: clamped)
+        a[0] -= g.px0; if (a[0] < 0) a[0] += g.M;
+        if (g.Mx < g.M) a[0] = min(a[0], g.Mx - g.P);
         bi = (a[0] * g.nbin + a[2] / SE_MMA_ZBIN) * g.M + a[1];
     } else
         bi = ((b[0] / SE_BIN) * g.nbin + b[1] / SE_BIN) * g.nbin + b[2] / SE_BIN;
