@@ -136,6 +136,10 @@ typedef struct {
                             grid belongs to a whole-grid plan).  Needs a (P, precision) of the tensor-core gridding
                             kernels and Mx >= P rounded up to a multiple of 8. */
     int px0;             /* slab plans: global index of local plane 0, in [0, M)            */
+    int64_t Nown;        /* slab plans with targets (Nt > 0): 0, or Nown == Nt: the targets ARE the first Nt sources (the
+                            points this slab owns; the sources behind them are ghost copies of the neighbours' points, needed by
+                            P2P only, "exchanging ghost source points").  Then K3 spreads only the first Nown
+                            sources and SE_STAGE_SUM adds the self term with f[0 .. Nt).  */
 } se_plan_desc;
 
 /*

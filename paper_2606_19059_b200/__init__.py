@@ -43,7 +43,7 @@ class SeInfo(C.Structure):
 class SePlanDesc(C.Structure):
     _fields_ = [("N", C.c_int64), ("Nt", C.c_int64), ("L", C.c_double), ("xi", C.c_double), ("rc", C.c_double),
                 ("M", C.c_int), ("P", C.c_int), ("precision", C.c_int), ("window", C.c_int),
-                ("Mx", C.c_int), ("px0", C.c_int)]
+                ("Mx", C.c_int), ("px0", C.c_int), ("Nown", C.c_int64)]
 
 
 class SeParams(C.Structure):
@@ -131,7 +131,7 @@ class Plan:
     """se_plan_create[_ex|_tol] / se_eval / se_plan_destroy with torch tensors for memory."""
 
     def __init__(self, N, L, xi=None, rc=None, M=None, P=None, precision="fp64", window="gaussian", Nt=0, eps=None,
-                 Mx=0, px0=0):
+                 Mx=0, px0=0, Nown=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_19059_b200 needs a CUDA device (no CPU fallback)")
@@ -150,10 +150,11 @@ class Plan:
             _check(lib().se_plan_create(C.byref(self._h), int(N), float(L), float(xi), float(rc), int(M), int(P), prec),
                    "se_plan_create")
         else:
-            d = SePlanDesc(int(N), int(Nt), float(L), float(xi), float(rc), int(M), int(P), prec, win, int(Mx), int(px0))
+            d = SePlanDesc(int(N), int(Nt), float(L), float(xi), float(rc), int(M), int(P), prec, win, int(Mx), int(px0), int(Nown))
             _check(lib().se_plan_create_ex(C.byref(self._h), C.byref(d)), "se_plan_create_ex")
         self.N, self.M, self.P, self.Nt = int(N), int(M), int(P), int(Nt)
         self.Mx, self.px0 = (int(Mx), int(px0)) if Mx else (int(M), 0)       # slab plans (se.h se_plan_desc)
+        self.Nown = int(Nown)
 
     # -- lifetime -----------------------------------------------------------------------
     def destroy(self):
@@ -222,7 +223,9 @@ class Plan:
     def stage(self, stage, x=None, f=None, u=None, stream=None):
         if isinstance(stage, str):
             stage = STAGES.index(stage)
-        _check(lib().se_eval_stage(self._h, int(stage), self._dev(x, "x"), self._dev(f, "f"),
+        # the sum stage of a slab plan with ghost sources (Nown = Nt) takes the strengths of the owned points only
+        nf = self.Nt if (self.Nown and stage == STAGES.index("sum")) else self.N
+        _check(lib().se_eval_stage(self._h, int(stage), self._dev(x, "x"), self._dev(f, "f", nf),
                                    self._dev(u, "u", self.Nt or self.N), _stream_ptr(stream)), f"se_eval_stage({stage})")
 
     # -- buffers ------------------------------------------------------------------------------

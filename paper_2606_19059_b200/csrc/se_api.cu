@@ -79,7 +79,7 @@ se_status run_stage(se_plan *p, int stage, const void *x, const void *f, void *u
     case SE_STAGE_IFFT: if (p->slab) return SE_EINVAL; return run_fft(p, false, s);
     case SE_STAGE_G2P: e = se_launch_g2p(p, s); break;
     case SE_STAGE_SUM:
-        if ((!f && !p->own_targets) || !u) return SE_EINVAL;
+        if ((!f && (!p->own_targets || p->nown)) || !u) return SE_EINVAL;
         e = se_launch_sum(p, f, u, s);
         break;
     default: return SE_EINVAL;
@@ -127,7 +127,7 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, double xi, double r
 {
     se_plan_desc d{};
     d.N = N; d.Nt = 0; d.L = L; d.xi = xi; d.rc = rc; d.M = M; d.P = P;
-    d.precision = (int)prec; d.window = SE_WINDOW_GAUSSIAN; d.Mx = 0; d.px0 = 0;
+    d.precision = (int)prec; d.window = SE_WINDOW_GAUSSIAN; d.Mx = 0; d.px0 = 0; d.Nown = 0;
     return se_plan_create_ex(out, &d);
 }
 
@@ -141,6 +141,8 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
     const int M = d->M, P = d->P, prec = d->precision, window = d->window;
     const int Mx = d->Mx > 0 ? d->Mx : M, px0 = d->Mx > 0 ? d->px0 : 0;
     const bool slab = d->Mx > 0;
+    const int64_t Nown = d->Nown;
+    if (Nown != 0 && (!slab || Nown != Nt || Nown > N)) return SE_EINVAL;
     if (!(N >= 1) || N >= ((int64_t)1 << 31) || Nt < 0 || Nt >= ((int64_t)1 << 31) || !(L > 0) || !(xi > 0) || !(rc > 0) ||
         !std::isfinite(L) || !std::isfinite(xi) || !std::isfinite(rc))
         return SE_EINVAL;
@@ -167,6 +169,7 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
     p->real_bytes = prec == SE_FP64 ? 8 : 4;
     p->own_targets = Nt > 0;
     p->slab = slab ? 1 : 0;
+    p->nown = Nown;
     SeGeom &g = p->g;
     g.N = N; g.M = M; g.P = P; g.L = L; g.xi = xi; g.rc = rc;
     g.Mx = Mx; g.px0 = px0;
@@ -248,7 +251,7 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
     }
 
     size_t rb = p->real_bytes;
-    size_t nc3 = (size_t)ncell * ncell * ncell, nb3 = (size_t)g.nbins_total;
+    size_t nc3 = (size_t)ncell * ncell * ncell, nb3 = (size_t)g.nbins_total + 1;       // + the bin of the sources that are not spread
     if (slab && g.grid_mode != 2) { delete p; return SE_EINVAL; }
     size_t M3 = (size_t)Mx * M * M, nm = slab ? 0 : (size_t)M * M * (M / 2 + 1);
     size_t scan_tiles = (std::max(nc3, nb3) + 2047) / 2048 + 1;

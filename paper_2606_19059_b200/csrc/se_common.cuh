@@ -97,6 +97,7 @@ struct se_plan {
     SeSet T;                       // targets: a copy of S (same pointers) unless the plan has its own targets
     int own_targets;               // 1: T has its own arrays (se_eval_targets)
     int slab;                      // 1: slab plan (grid Mx x M x M, no transforms; se.h se_plan_desc)
+    int64_t nown;                  // slab plans with ghost sources: the first nown sources are spread, the targets are those points
     const void *xt_stage;          // se_set_targets: target positions for se_eval_stage(SE_STAGE_SORT)
     double *wcoef;                 // Kaiser-Bessel: [P][nu + 1] polynomial coefficients (always double)
     void *uN;                      // [Nt][3] Real, the targets' near-sorted order

@@ -36,7 +36,7 @@ __device__ __forceinline__ int grid_base1(double v, const SeGeom &g, double &fra
 
 template <typename Real>
 __global__ void k_bin(SeGeom g, const Real *__restrict__ x, int *__restrict__ cell_of,
-                      int *__restrict__ bin_of, int *__restrict__ cell_cnt, int *__restrict__ bin_cnt)
+                      int *__restrict__ bin_of, int *__restrict__ cell_cnt, int *__restrict__ bin_cnt, int64_t nspread)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.N) return;
@@ -60,6 +60,7 @@ __global__ void k_bin(SeGeom g, const Real *__restrict__ x, int *__restrict__ ce
         bi = (a[0] * g.nbin + a[2] / SE_MMA_ZBIN) * g.M + a[1];
     } else
         bi = ((b[0] / SE_BIN) * g.nbin + b[1] / SE_BIN) * g.nbin + b[2] / SE_BIN;
+    if (i >= nspread) bi = g.nbins_total;          // ghost sources of a slab plan: the extra bin no gridding tile visits
     cell_of[i] = ci;
     bin_of[i] = bi;
     atomicAdd(&cell_cnt[ci], 1);
@@ -329,14 +330,15 @@ cudaError_t sort_set(se_plan *p, SeSet &S, const void *xv, const void *fv, bool 
     SeGeom g = p->g;
     g.N = S.n;
     const Real *x = (const Real *)xv, *f = (const Real *)fv;
-    int nc3 = g.ncell * g.ncell * g.ncell, nb3 = g.nbins_total;
+    int nc3 = g.ncell * g.ncell * g.ncell, nb3 = g.nbins_total + 1;
     cudaError_t e = cudaMemsetAsync(S.cell_cursor, 0, sizeof(int) * (nc3 + 1), s);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(S.bin_cursor, 0, sizeof(int) * (nb3 + 1), s);
     if (e != cudaSuccess) return e;
     int T = 256;
     unsigned nblk = (unsigned)((g.N + T - 1) / T);
-    k_bin<Real><<<nblk, T, 0, s>>>(g, x, S.cell_of, S.bin_of, S.cell_cursor, S.bin_cursor);
+    k_bin<Real><<<nblk, T, 0, s>>>(g, x, S.cell_of, S.bin_of, S.cell_cursor, S.bin_cursor,
+                                   (spread && p->nown > 0) ? p->nown : g.N);
     int tilesA = (nc3 + SCAN_TILE - 1) / SCAN_TILE, tilesB = (nb3 + SCAN_TILE - 1) / SCAN_TILE;
     int tiles = tilesA > tilesB ? tilesA : tilesB;
     // tile sums live behind the CSR arrays: the plan allocates cell_start / bin_start with room for them after entry n
@@ -389,7 +391,7 @@ cudaError_t sum_impl(se_plan *p, const void *f, void *u, cudaStream_t s)
     int T = 256;
     const int64_t nt = p->T.n;
     k_sum<Real><<<(unsigned)((3 * nt + T - 1) / T), T, 0, s>>>(nt, (const Real *)p->uN, (const Real *)p->uF,
-                                                              p->own_targets ? nullptr : (const Real *)f,
+                                                              (p->own_targets && !p->nown) ? nullptr : (const Real *)f,
                                                               p->T.inv_near, p->T.inv_grid,
                                                               (Real)far_scale, (Real)cself, (Real *)u);
     p->launches += 1;
