@@ -219,6 +219,15 @@ se_status se_last_launch_count(const se_plan *p, int *count);
  * in-range pairs per second with them.  Synchronises the device. */
 se_status se_count_pairs(se_plan *p, int64_t *candidates, int64_t *in_range);
 
+/*
+ * K4 (SE_STAGE_SCALE, eq. (2.6)) on a caller-owned DEVICE block of the spectrum: spec = [3][M][nky][M/2 + 1]
+ * complex numbers of the plan's precision, holding the modes (i_x, i_y, i_z) with ky0 <= i_y < ky0 + nky (all i_x, all stored
+ * i_z): what one rank holds between the two 1-D transforms of a slab-decomposed 3-D FFT (PAPER.md:664 (4)).  In place,
+ * asynchronous on `stream`; valid on slab plans (only the plan's multiplier tables are used).  SE_EINVAL on a null pointer or a
+ * range outside [0, M).
+ */
+se_status se_scale_block(se_plan *p, void *spec, int ky0, int nky, void *stream);
+
 /* ---- parameter selection from a tolerance (section 2.4, eq. (2.9)) ------- */
 
 typedef struct {

@@ -27,7 +27,7 @@ SE_NSTAGES = 8
 EXPORTS = ("se_plan_create", "se_plan_create_ex", "se_plan_create_tol", "se_select_params", "se_eval",
            "se_eval_targets", "se_set_targets", "se_eval_host", "se_plan_destroy", "se_strerror",
            "se_plan_info", "se_eval_stage", "se_buffer_read", "se_buffer_write",
-           "se_set_profiling", "se_stage_ms", "se_last_launch_count", "se_measure_peak", "se_count_pairs")
+           "se_set_profiling", "se_stage_ms", "se_last_launch_count", "se_measure_peak", "se_count_pairs", "se_scale_block")
 
 
 class SeInfo(C.Structure):
@@ -81,6 +81,7 @@ def lib() -> C.CDLL:
         L.se_set_targets.argtypes = [vp, vp]
         L.se_measure_peak.argtypes = [i32, i32, C.POINTER(dbl)]
         L.se_count_pairs.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
+        L.se_scale_block.argtypes = [vp, vp, i32, i32, vp]
         L.se_eval_host.argtypes = [vp, vp, vp, vp, vp]
         L.se_plan_destroy.argtypes = [vp]
         L.se_strerror.argtypes = [i32]
@@ -267,6 +268,17 @@ class Plan:
                "se_buffer_write")
 
     # -- timing ---------------------------------------------------------------------------------
+    def scale_block(self, spec, ky0, nky, stream=None):
+        """K4 in place on a complex block [3, M, nky, M // 2 + 1] of the spectrum (modes ky0 <= i_y < ky0 + nky)."""
+        import torch
+        cdt = torch.complex128 if self.precision == "fp64" else torch.complex64
+        if not (spec.is_cuda and spec.is_contiguous() and spec.dtype == cdt and
+                tuple(spec.shape) == (3, self.M, int(nky), self.M // 2 + 1)):
+            raise ValueError("scale_block: need a contiguous CUDA complex tensor [3, M, nky, M // 2 + 1] of the plan's precision")
+        _check(lib().se_scale_block(self._h, C.c_void_p(spec.data_ptr()), int(ky0), int(nky), _stream_ptr(stream)),
+               "se_scale_block")
+        return spec
+
     def set_profiling(self, on: bool):
         _check(lib().se_set_profiling(self._h, int(bool(on))), "se_set_profiling")
 

@@ -19,15 +19,16 @@ template <> struct Cplx<float> { typedef float2 type; };
 // ktab layout: [0..M) k value of index i, [M..2M) e(k_i)
 template <typename Real>
 __global__ void __launch_bounds__(256)
-k_scale(int M, int Mh, Real pref, Real inv4xi2, const Real *__restrict__ ktab,
+k_scale(int M, int Mh, int y0, int ny, Real pref, Real inv4xi2, const Real *__restrict__ ktab,
         typename Cplx<Real>::type *__restrict__ spec)
 {
+    // spec: [3][M][ny][Mh], the modes with second index y0 .. y0 + ny - 1 (the whole spectrum: y0 = 0, ny = M)
     typedef typename Cplx<Real>::type C;
     const int iz = blockIdx.x * blockDim.x + threadIdx.x;
-    const int iy = blockIdx.y, ix = blockIdx.z;
+    const int iy = y0 + blockIdx.y, ix = blockIdx.z;
     if (iz >= Mh) return;
-    const size_t nm = (size_t)M * M * Mh;
-    const size_t idx = ((size_t)ix * M + iy) * Mh + iz;
+    const size_t nm = (size_t)M * ny * Mh;
+    const size_t idx = ((size_t)ix * ny + blockIdx.y) * Mh + iz;
     const Real kx = ktab[ix], ky = ktab[iy], kz = ktab[iz];
     const Real k2 = kx * kx + ky * ky + kz * kz;
     const bool nyq = (2 * ix == M) || (2 * iy == M) || (2 * iz == M);
@@ -47,7 +48,7 @@ k_scale(int M, int Mh, Real pref, Real inv4xi2, const Real *__restrict__ ktab,
 }
 
 template <typename Real>
-cudaError_t scale_impl(se_plan *p, cudaStream_t s)
+cudaError_t scale_impl(se_plan *p, void *spec, int y0, int ny, cudaStream_t s)
 {
     const SeGeom &g = p->g;
     int Mh = g.M / 2 + 1;
@@ -55,11 +56,11 @@ cudaError_t scale_impl(se_plan *p, cudaStream_t s)
     // (h^3 / V) * 8 pi  with h^3/V = 1/M^3
     Real pref = (Real)(8.0 * SE_PI / M3);
     Real inv4xi2 = (Real)(1.0 / (4.0 * g.xi * g.xi));
-    dim3 grid((Mh + 255) / 256, g.M, g.M);
+    dim3 grid((Mh + 255) / 256, ny, g.M);
     int T = Mh < 256 ? ((Mh + 31) / 32) * 32 : 256;
     grid.x = (Mh + T - 1) / T;
-    k_scale<Real><<<grid, T, 0, s>>>(g.M, Mh, pref, inv4xi2, (const Real *)p->ktab,
-                                     (typename Cplx<Real>::type *)p->spec);
+    k_scale<Real><<<grid, T, 0, s>>>(g.M, Mh, y0, ny, pref, inv4xi2, (const Real *)p->ktab,
+                                     (typename Cplx<Real>::type *)spec);
     p->launches += 1;
     return cudaGetLastError();
 }
@@ -68,5 +69,16 @@ cudaError_t scale_impl(se_plan *p, cudaStream_t s)
 
 cudaError_t se_launch_scale(se_plan *p, cudaStream_t s)
 {
-    return p->precision == SE_FP64 ? scale_impl<double>(p, s) : scale_impl<float>(p, s);
+    return p->precision == SE_FP64 ? scale_impl<double>(p, p->spec, 0, p->g.M, s) : scale_impl<float>(p, p->spec, 0, p->g.M, s);
+}
+
+// se.h: K4 on a caller-owned block of the spectrum (the ky-pencil a rank holds in a slab-decomposed transform)
+extern "C" se_status se_scale_block(se_plan *p, void *spec, int ky0, int nky, void *stream)
+{
+    if (!p || !spec || ky0 < 0 || nky < 1 || ky0 + nky > p->g.M) return SE_EINVAL;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) { cudaGetLastError(); return SE_EINVAL; }
+    cudaError_t e = p->precision == SE_FP64 ? scale_impl<double>(p, spec, ky0, nky, (cudaStream_t)stream)
+                                            : scale_impl<float>(p, spec, ky0, nky, (cudaStream_t)stream);
+    return e == cudaSuccess ? SE_OK : SE_ECUDA;
 }

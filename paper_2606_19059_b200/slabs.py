@@ -6,15 +6,15 @@ and the particles whose base grid index floor(x/h) lies in them.  The paper's co
   MPI-SORT           `partition`: every rank sends each of its points to the owner of its slab (all-to-all, sizes first);
   MPI-GHOST-SOURCE   `ghost_sources`: the points within rc of a slab face go to that neighbour, which needs them as
                      P2P sources only (a slab plan spreads its first `Nown` sources, se.h se_plan_desc);
-  ghost grid planes  after P2G the P/2 - 1 planes below and the P/2 planes above the owned range are ADDED to the neighbours'
-                     owned planes (`reduce_ghost_planes`); before G2P the same planes are filled with the neighbours' values
-                     (MPI-GHOST-GRID; here they come out of the assembled grid);
-  FFT / IFFT         the owned planes of all ranks are all-gathered and every rank transforms and scales the whole grid with
-                     a whole-grid plan (cuFFT, K4): the grid work is replicated, not distributed -- the paper uses cuFFTMp
-                     for this step; a slab/pencil transpose around 2-D + 1-D cuFFT plans is what is missing here.
+  MPI-GHOST-GRID     after P2G the P/2 - 1 planes below and the P/2 planes above the owned range are ADDED to the neighbours'
+                     owned planes (`SlabEval.owned_planes`); between IFFT and G2P the same planes are filled with the
+                     neighbours' values (`planes_back` / `gather_and_sum`);
+  FFT / IFFT         slab-decomposed: 2-D R2C over (y, z) on the owned planes, all-to-all into ky-pencils, 1-D transform over
+                     x, K4 on the pencil (se_scale_block), and the same way back (the paper uses cuFFTMp here; the local
+                     transforms are cuFFT's, called through torch.fft).
 
-All arithmetic of the method runs in the library's kernels through the stage hooks of the C-ABI (K1, K2, K3, K5, K6 on a slab
-plan, FFT + K4 + IFFT on a whole-grid plan); this module only moves data: torch for device memory and indexing,
+All arithmetic of the method runs in the library's kernels through the C-ABI (K1, K2, K3, K5, K6 by the stage hooks of a slab
+plan, K4 by se_scale_block); this module only moves data: torch for device memory, indexing and the cuFFT calls,
 `torch.distributed` (NCCL between GPUs, gloo in the CPU tests of the host logic) for the exchanges.  `SlabLayout` is pure
 index arithmetic and needs no GPU.
 """
@@ -122,30 +122,64 @@ class SlabEval:
         own[:, lay.Ml - lay.nlo:] += from_right                    # their planes below their range = my last P/2 - 1
         return own
 
-    # -- phase 4: transform of the assembled grid (replicated) and phase 5: K5, K6 ---------------------------------------
-    def far_and_sum(self, owned_blocks, stream=None):
-        """owned blocks of all ranks (list in rank order) -> FFT, K4, IFFT on the whole grid, G2P from the planes of this
-        slab, u = u^N + u^F - self term for the owned points ([n, 3])"""
+    # -- phase 4: slab-decomposed 3-D transform with K4 in the middle -----------------------------------------------------
+    # x-slabs --2-D R2C over (y, z)--> all-to-all --> ky-pencils --1-D C2C over x, K4, inverse 1-D--> all-to-all --> x-slabs
+    # --2-D C2R--> owned planes.  The transforms are cuFFT's (through torch.fft; unnormalised in both directions, as in the
+    # one-GPU plan), K4 is the library's kernel on the pencil block this rank holds (se_scale_block).
+    def spectrum_out(self, own):
+        """owned planes [3, Ml, M, M] -> one message per rank: the ky-block of the 2-D transforms that rank's pencil takes"""
         import torch
-        from . import Plan, SE_BUF_GRID
+        lay = self.lay
+        A = torch.fft.rfft2(own, dim=(2, 3))                            # [3, Ml, M, M/2+1]
+        Ky = lay.M // lay.world
+        return [A[:, :, d * Ky:(d + 1) * Ky].contiguous() for d in range(lay.world)]
+
+    def pencil(self, blocks, stream=None):
+        """the ky-blocks of all ranks' planes (rank order = plane order) -> scaled pencil -> one message per rank: the
+        x-block of planes that rank owns"""
+        import torch
+        lay = self.lay
+        Ky = lay.M // lay.world
+        S = torch.fft.fft(torch.cat(list(blocks), dim=1), dim=1).contiguous()        # [3, M, Ky, M/2+1]
+        self._tables().scale_block(S, self.rank * Ky, Ky, stream=stream)
+        B = torch.fft.ifft(S, dim=1, norm="forward")                    # unnormalised inverse
+        return [B[:, d * lay.Ml:(d + 1) * lay.Ml].contiguous() for d in range(lay.world)]
+
+    def planes_back(self, blocks):
+        """the x-blocks of all pencils (rank order = ky order) -> H~ on the owned planes; returns the ghost planes the
+        neighbours gather from: (my first P/2 planes for the left one, my last P/2 - 1 for the right one)"""
+        import torch
+        lay = self.lay
+        A = torch.cat(list(blocks), dim=2)                              # [3, Ml, M, M/2+1]
+        self.Ht = torch.fft.irfft2(A, s=(lay.M, lay.M), dim=(2, 3), norm="forward").contiguous()
+        return self.Ht[:, :lay.nhi].contiguous(), self.Ht[:, lay.Ml - lay.nlo:].contiguous()
+
+    # -- phase 5: K5, K6 -----------------------------------------------------------------------------------------------------
+    def gather_and_sum(self, from_left, from_right, stream=None):
+        """ghost planes received (the left neighbour's last P/2 - 1 planes, the right neighbour's first P/2) -> local grid ->
+        G2P -> u = u^N + u^F - self term for the owned points ([n, 3])"""
+        import torch
+        from . import SE_BUF_GRID
         lay = self.lay
         if self.x.shape[0] == 0:
             return self.x.clone()
-        Hg = torch.cat(list(owned_blocks), dim=1).contiguous()         # [3, M, M, M]
-        if self.grid_plan is None:
-            self.grid_plan = Plan(1, lay.L, self.xi, lay.rc, lay.M, lay.P, self.precision, window=self.window)
-        g = self.grid_plan
-        g.write(SE_BUF_GRID, Hg, stream=stream)
-        g.stage("fft", stream=stream)
-        g.stage("scale", stream=stream)
-        g.stage("ifft", stream=stream)
-        Ht = g.read(SE_BUF_GRID, stream=stream)
-        planes = torch.as_tensor(lay.local_planes(self.rank), device=Ht.device)
-        self.plan.write(SE_BUF_GRID, Ht.index_select(1, planes).contiguous(), stream=stream)
+        spare = torch.zeros_like(self.Ht[:, :lay.Mx - lay.nlo - lay.Ml - lay.nhi])
+        self.plan.write(SE_BUF_GRID, torch.cat([from_left, self.Ht, from_right, spare], dim=1).contiguous(), stream=stream)
         self.plan.stage("g2p", stream=stream)
         u = torch.empty_like(self.x)
         self.plan.stage("sum", f=self.f, u=u, stream=stream)
         return u
+
+    def _tables(self):
+        """a plan whose multiplier tables K4 uses: this rank's slab plan, or a one-point one if the slab holds no points"""
+        from . import Plan
+        if self.plan is not None:
+            return self.plan
+        if self.grid_plan is None:
+            lay = self.lay
+            self.grid_plan = Plan(1, lay.L, self.xi, lay.rc, lay.M, lay.P, self.precision, window=self.window,
+                                  Mx=lay.Mx, px0=lay.px0(self.rank))
+        return self.grid_plan
 
     def destroy(self):
         for p in (self.plan, self.grid_plan):
@@ -163,7 +197,10 @@ def evaluate_emulated(lay: SlabLayout, xi, xs_per_rank, fs_per_rank, precision="
         out = [ranks[r].ghost_out(xs_per_rank[r], fs_per_rank[r]) for r in range(W)]
         gp = [ranks[r].near_and_spread(out[(r - 1) % W][1], out[(r + 1) % W][0]) for r in range(W)]
         own = [ranks[r].owned_planes(gp[(r - 1) % W][1], gp[(r + 1) % W][0]) for r in range(W)]
-        return [ranks[r].far_and_sum(own) for r in range(W)]
+        a = [ranks[r].spectrum_out(own[r]) for r in range(W)]                     # a[src][dst]
+        b = [ranks[r].pencil([a[s][r] for s in range(W)]) for r in range(W)]
+        g = [ranks[r].planes_back([b[s][r] for s in range(W)]) for r in range(W)]  # (for left, for right)
+        return [ranks[r].gather_and_sum(g[(r - 1) % W][1], g[(r + 1) % W][0]) for r in range(W)]
     finally:
         for e in ranks:
             e.destroy()
@@ -218,12 +255,29 @@ def partition(lay: SlabLayout, x, f, group=None):
     return a2a(x), a2a(f), (src_rank, idx)
 
 
+def _all_to_all(blocks, group=None):
+    """blocks[d] goes to rank d; returns the list of blocks received, in rank order (all blocks have one shape).  Point to
+    point operations: they exist on every backend (gloo has no all_to_all)."""
+    import torch
+    import torch.distributed as dist
+    rank, world = dist.get_rank(group), dist.get_world_size(group)
+    out = [torch.empty_like(blocks[rank]) for _ in range(world)]
+    out[rank].copy_(blocks[rank])
+    ops = []
+    for k in range(1, world):                   # same pairing order on both sides of every pair
+        dst, src = (rank + k) % world, (rank - k) % world
+        ops.append(dist.P2POp(dist.isend, blocks[dst].contiguous(), dst, group))
+        ops.append(dist.P2POp(dist.irecv, out[src], src, group))
+    if ops:
+        for w in dist.batch_isend_irecv(ops):
+            w.wait()
+    return out
+
+
 def evaluate_distributed(ev: SlabEval, x, f, group=None, stream=None):
     """One slab-decomposed evaluation under torch.distributed (one process per GPU): x, f are the points this rank owns
     (see `partition`); returns u for them."""
     import torch
-    import torch.distributed as dist
-    world = dist.get_world_size(group)
     (xl, fl), (xr, fr) = ev.ghost_out(x, f)
     gl, gr = _exchange(torch.cat([xl, fl], dim=1), torch.cat([xr, fr], dim=1), group)
     lo_planes, hi_planes = ev.near_and_spread((gl[:, :3].contiguous(), gl[:, 3:].contiguous()),
@@ -231,6 +285,8 @@ def evaluate_distributed(ev: SlabEval, x, f, group=None, stream=None):
     # planes travel with the plane index first
     pl, pr = _exchange(lo_planes.transpose(0, 1).contiguous(), hi_planes.transpose(0, 1).contiguous(), group)
     own = ev.owned_planes(pl.transpose(0, 1), pr.transpose(0, 1))
-    blocks = [torch.empty_like(own) for _ in range(world)]
-    dist.all_gather(blocks, own.contiguous(), group=group)
-    return ev.far_and_sum(blocks, stream=stream)
+    pencil_in = _all_to_all(ev.spectrum_out(own), group)
+    planes_in = _all_to_all(ev.pencil(pencil_in, stream=stream), group)
+    for_left, for_right = ev.planes_back(planes_in)
+    gl, gr = _exchange(for_left.transpose(0, 1).contiguous(), for_right.transpose(0, 1).contiguous(), group)
+    return ev.gather_and_sum(gl.transpose(0, 1).contiguous(), gr.transpose(0, 1).contiguous(), stream=stream)
