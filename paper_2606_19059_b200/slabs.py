@@ -41,11 +41,21 @@ class SlabLayout:
         """global index of local plane 0 of `rank`"""
         return (rank * self.Ml - self.nlo) % self.M
 
+    def _wrap(self, x0):
+        """x0 wrapped into [0, L) exactly as K1 does it (a result that is not in [0, L), e.g. L itself after rounding, is 0)"""
+        if hasattr(x0, "floor"):                    # torch
+            import torch
+            xw = x0 - self.L * (x0 / self.L).floor()
+            return torch.where((xw >= 0) & (xw < self.L), xw, torch.zeros_like(xw))
+        xw = x0 - self.L * np.floor(x0 / self.L)
+        return np.where((xw >= 0) & (xw < self.L), xw, 0.0)
+
     def base_plane(self, x0):
-        """floor(x_w / h) of wrapped first coordinates (numpy or torch), as the library takes it: in double"""
-        xw = x0 - self.L * (x0 / self.L).floor() if hasattr(x0, "floor") else x0 - self.L * np.floor(x0 / self.L)
-        b = (xw / self.h).floor().long() if hasattr(xw, "floor") else np.floor(xw / self.h).astype(np.int64)
-        return b.clamp(0, self.M - 1) if hasattr(b, "clamp") else np.clip(b, 0, self.M - 1)
+        """floor(x_w / h) of first coordinates (numpy or torch, double), as the library takes it"""
+        xw = self._wrap(x0)
+        if hasattr(xw, "floor"):
+            return (xw / self.h).floor().long().clamp(0, self.M - 1)
+        return np.clip(np.floor(xw / self.h).astype(np.int64), 0, self.M - 1)
 
     def owner(self, x0):
         """rank that owns each point (by the base grid plane of its first coordinate)"""
@@ -54,7 +64,7 @@ class SlabLayout:
     def ghost_masks(self, x0, rank: int):
         """(to_left, to_right): which of this rank's points lie within rc of its lower / upper face (periodic)"""
         lo, hi = rank * self.Ml * self.h, (rank + 1) * self.Ml * self.h
-        xw = x0 - self.L * (x0 / self.L).floor() if hasattr(x0, "floor") else x0 - self.L * np.floor(x0 / self.L)
+        xw = self._wrap(x0)
         to_left, to_right = (xw - lo) < self.rc, (hi - xw) <= self.rc
         if self.world == 2:                         # both neighbours are the same rank: a point goes there once
             to_left = to_left & ~to_right
