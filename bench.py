@@ -428,6 +428,54 @@ def run_b200(args):
     return 0
 
 
+def run_slabs(args):
+    """--mode slabs: ONE evaluation of the config cut into x-slabs, one per rank (paper_2606_19059_b200/
+    slabs.py): strong scaling, value = N / time of one evaluation.  Needs torchrun with >= 2 ranks (NCCL).  Not the default
+    multi-GPU arm (that is the replica arm, `north_star`: "everything runs on one GPU"): the boxes of this build have one
+    GPU, so this arm has only been run through its single-GPU emulation (tests/test_gpu_slabs.py) and under gloo on CPU
+    (tests/test_slabs_host.py)."""
+    import torch
+    import torch.distributed as dist
+    import paper_2606_19059_b200 as se
+    from paper_2606_19059_b200 import slabs, workloads as W
+    rank, world, local = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
+    if world < 2:
+        raise SystemExit("bench.py --mode slabs needs torchrun with at least 2 ranks")
+    torch.cuda.set_device(local)
+    dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    c, x, f = W.make(args.config)
+    lay = slabs.SlabLayout(c.L, c.M, c.P, c.rc, world)
+    mine = np.nonzero(lay.owner(x[:, 0].astype(np.float64)) == rank)[0]
+    xd, fd = torch.as_tensor(x[mine], device="cuda"), torch.as_tensor(f[mine], device="cuda")
+    ev = slabs.SlabEval(lay, rank, c.xi, precision=c.precision)
+    for _ in range(max(args.warmup, 3)):
+        u = slabs.evaluate_distributed(ev, xd, fd)
+    torch.cuda.synchronize(); dist.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        u = slabs.evaluate_distributed(ev, xd, fd)
+    e1.record()
+    torch.cuda.synchronize(); dist.barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    fin = torch.tensor([float(torch.isfinite(u).all())], device="cuda")
+    dist.all_reduce(fin, op=dist.ReduceOp.MIN)
+    ms = float(t[0]) / args.steps
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": c.N / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64" if c.precision == "fp64" else "f32", "data": "synthetic",
+            "config": {"workload": c.label, "N": c.N, "xi": c.xi, "rc": c.rc, "M": c.M, "P": c.P, "precision": c.precision,
+                       "parallelism": f"x-slabs{world}: ghost sources, ghost planes, slab-decomposed FFT",
+                       "planes_per_rank": lay.Ml, "points_rank0": int(len(mine))},
+            "finite": bool(fin[0] > 0)}), flush=True)
+    ev.destroy()
+    dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -437,9 +485,13 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sub", action="store_true", help="skip the sub-results (configs 4, 5, Kaiser-Bessel variants)")
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "slabs"],
+                    help="multi-GPU arm: independent replicas (default, weak scaling) or one evaluation cut into x-slabs")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.mode == "slabs":
+        return run_slabs(args)
     world = env_int("WORLD_SIZE", 1)
     if world == 1 and args.gpus > 1:
         raise SystemExit("bench.py: --gpus %d needs torchrun with --nproc-per-node %d" % (args.gpus, args.gpus))
