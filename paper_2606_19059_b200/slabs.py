@@ -85,6 +85,7 @@ class SlabEval:
         self.lay, self.rank, self.xi, self.precision, self.window = layout, rank, float(xi), precision, window
         self.plan = None
         self.grid_plan = None
+        self.side = None                            # side stream of the P2P stage
 
     # -- phase 1: ghost sources ------------------------------------------------------------------------------------
     def ghost_out(self, x, f):
@@ -116,9 +117,15 @@ class SlabEval:
         p = self.plan
         p.set_targets(self.x)
         p.stage("sort", x=xs, f=fs, stream=stream)
-        p.stage("p2p", stream=stream)
         p.stage("p2g", stream=stream)
         self.H = p.read(SE_BUF_GRID, stream=stream)                    # [3, Mx, M, M]
+        # P2P does not depend on the grid chain ("can be overlapped"): it runs on a side stream, next to the
+        # exchanges and transforms that follow, and is joined before the sum
+        main = stream if stream is not None else torch.cuda.current_stream()
+        if self.side is None:
+            self.side = torch.cuda.Stream()
+        self.side.wait_stream(main)
+        p.stage("p2p", stream=self.side)
         lo, hi = lay.nlo, lay.nhi
         return self.H[:, :lo].contiguous(), self.H[:, lo + lay.Ml:lo + lay.Ml + hi].contiguous()
 
@@ -177,6 +184,7 @@ class SlabEval:
         self.plan.write(SE_BUF_GRID, torch.cat([from_left, self.Ht, from_right, spare], dim=1).contiguous(), stream=stream)
         self.plan.stage("g2p", stream=stream)
         u = torch.empty_like(self.x)
+        (stream if stream is not None else torch.cuda.current_stream()).wait_stream(self.side)     # u^N is ready
         self.plan.stage("sum", f=self.f, u=u, stream=stream)
         return u
 
