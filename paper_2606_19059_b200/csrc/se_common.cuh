@@ -34,23 +34,26 @@ constexpr int SE_MMA_NWY = 2, SE_MMA_NWZ = 6;
 #define SE_MMA_RECG(P) (3 * (P) + 4)
 #define SE_XP_LEN(n) (((n) + 1) / 2 + 1)
 
+// Passed to every kernel BY VALUE and captured by the kernels' lambdas: keep it at 128 bytes (at 136 the compiler stopped
+// keeping its fields in registers: k_mma<gather> executed 5.6 % more instructions, 5.76 -> 6.14 ms on config 3).
 struct SeGeom {
     int64_t N;          // points of the set a launch works on (sources or targets; the launchers set it)
     int M, P;
     int Mx, px0;        // planes of the grid along x (M unless a slab plan) and global index of local plane 0
-    int window;         // se_window
-    int nu;             // Kaiser-Bessel: polynomial degree per bin
     int ncell;          // near cells per dimension
     int nbin;           // grid bins per dimension = ceil(M / SE_BIN) (tile mode) or z-bins ceil(M / 8) (mma mode)
-    int grid_mode;      // 0: tile-stationary k_grid (any even P),
-                        // 2: FP64 tensor-core sweep (se_mma.cu; fp64 P = 16, 24; fp32 P = 12)
-    int nbins_total;    // nbin^3 (tile mode), M * nbin * M (mma mode)
+    int nbins_total;    // nbin^3 (tile mode), Mx * nbin * M (mma mode)
     int nchunk;         // mma mode: chunks along x (P2G)
     int nchunk_g2p;     // mma mode: chunks along x (G2P)
     int nfull, nsplit;  // mma mode, P2G with nchunk = 1: the last `tiles - nfull` block tiles (those of the partly filled
                         // last wave) are split into nsplit x-chunks each (nsplit = 1: no split)
-    int ring;           // mma mode: row stride of the spread records = P rounded up to a multiple of 8
-    int rel_coords;     // 1: near-sorted positions are cell-relative (fp32 path)
+    short window;       // se_window
+    short nu;           // Kaiser-Bessel: polynomial degree per bin
+    short grid_mode;    // 0: tile-stationary k_grid (any even P),
+                        // 2: FP64 tensor-core sweep (se_mma.cu; fp64 P = 8, 12, 16, 24; fp32 P = 8, 12)
+    short ring;         // mma mode: row stride of the spread records = P rounded up to a multiple of 8
+    short rel_coords;   // 1: near-sorted positions are cell-relative (fp32 path)
+    short pad_;
     double L, xi, rc;
     double h;           // L / M
     double wcell;       // L / ncell
@@ -58,6 +61,7 @@ struct SeGeom {
     double cw;          // (a/pi)^{3/2}
     double eta;
 };
+static_assert(sizeof(SeGeom) == 128, "SeGeom is a by-value kernel parameter: see the comment above");
 
 // One point set (the sources, or a plan's own targets) in its two sorted orders.
 struct SeSet {

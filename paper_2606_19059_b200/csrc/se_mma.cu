@@ -149,9 +149,17 @@ template <> struct GV<float> {
 
 // P: ring size = row stride of the records (a multiple of 8 for P2G, of 4 for G2P); W <= P: window support (the
 // record rows are zero beyond W); GR: grid storage type.
-template <int P, bool SPREAD, int W, typename GR>
+// SLAB: the grid has g.Mx planes along x instead of M (slab plans, se.h se_plan_desc); a compile-time switch, so that the
+// whole-grid kernels keep one grid size in registers (the extra live value cost G2P 7 %)
+// what k_mma needs of the plan's geometry: a compact by-value parameter (see the note at SeGeom)
+struct MmaGeom {
+    int64_t N;
+    int M, Mx, nbin, nchunk, nchunk_g2p, nfull, nsplit;
+};
+
+template <int P, bool SPREAD, int W, typename GR, bool SLAB>
 __global__ void __launch_bounds__((NWY * NWZ + 4) * 32, 1)
-k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_start, GR *__restrict__ grid,
+k_mma(MmaGeom g, const double *__restrict__ recs, const int *__restrict__ bin_start, GR *__restrict__ grid,
       double *__restrict__ uFpart)
 {
     static_assert(W <= P && (SPREAD || W == P), "window / ring");
@@ -161,7 +169,7 @@ k_mma(SeGeom g, const double *__restrict__ recs, const int *__restrict__ bin_sta
     Smem<P, SPREAD> &S = *reinterpret_cast<Smem<P, SPREAD> *>(smem_raw);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int M = g.M, Mx = g.Mx, nzb = g.nbin;            // Mx planes along x (the sweep direction), M along y and z
+    const int M = g.M, Mx = SLAB ? g.Mx : g.M, nzb = g.nbin;      // Mx planes along x (the sweep direction), M along y and z
     const int ntY = (M + BY - 1) / BY, ntZ = (M + BZ - 1) / BZ;
     int tile = blockIdx.x % (ntZ * ntY), chunk = blockIdx.x / (ntZ * ntY);
     int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
@@ -637,8 +645,8 @@ __global__ void k_reduce_slots(SeGeom g, const short4 *__restrict__ anchor, cons
 }
 
 // prepare == true: only opt this plan's device in to the kernel's dynamic shared memory (once per plan, at creation)
-template <int P, bool SPREAD, int W, typename GR>
-cudaError_t launch(se_plan *p, cudaStream_t s, bool prepare)
+template <int P, bool SPREAD, int W, typename GR, bool SLAB>
+cudaError_t launch_k(se_plan *p, cudaStream_t s, bool prepare)
 {
     typedef Cfg<P, SPREAD> C;
     SeGeom g = p->g;
@@ -646,12 +654,13 @@ cudaError_t launch(se_plan *p, cudaStream_t s, bool prepare)
     g.N = Q.n;
     constexpr size_t smem = sizeof(Smem<P, SPREAD>);
     static_assert(smem <= 227 * 1024, "shared memory per block");
-    auto kern = k_mma<P, SPREAD, W, GR>;
+    auto kern = k_mma<P, SPREAD, W, GR, SLAB>;
     if (prepare) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int ntY = (g.M + C::BY - 1) / C::BY, ntZ = (g.M + C::BZ - 1) / C::BZ;
     const int nchunk = SPREAD ? g.nchunk : g.nchunk_g2p;
     const int nblocks = (SPREAD && g.nsplit > 1) ? g.nfull + g.nsplit * (ntY * ntZ - g.nfull) : nchunk * ntY * ntZ;
-    kern<<<(unsigned)nblocks, C::NT, smem, s>>>(g, (const double *)(SPREAD ? Q.wtab : Q.recg), Q.bin_start,
+    const MmaGeom mg{g.N, g.M, g.Mx, g.nbin, g.nchunk, g.nchunk_g2p, g.nfull, g.nsplit};
+    kern<<<(unsigned)nblocks, C::NT, smem, s>>>(mg, (const double *)(SPREAD ? Q.wtab : Q.recg), Q.bin_start,
                                                              (GR *)p->grid, (double *)p->uFpart);
     p->launches += 1;
     if (!SPREAD) {
@@ -660,6 +669,12 @@ cudaError_t launch(se_plan *p, cudaStream_t s, bool prepare)
         p->launches += 1;
     }
     return cudaGetLastError();
+}
+
+template <int P, bool SPREAD, int W, typename GR>
+cudaError_t launch(se_plan *p, cudaStream_t s, bool prepare)
+{
+    return p->slab ? launch_k<P, SPREAD, W, GR, true>(p, s, prepare) : launch_k<P, SPREAD, W, GR, false>(p, s, prepare);
 }
 
 template <bool SPREAD>
