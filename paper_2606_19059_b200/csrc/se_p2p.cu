@@ -63,6 +63,12 @@ constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV 
 #ifndef P2P_BLOCKS
 #define P2P_BLOCKS 4
 #endif
+#ifndef P2P_BFAN
+#define P2P_BFAN 2          /* mode B: pairs per lane and cooperative round, fp64 plans */
+#endif
+#ifndef P2P_BFAN_F32
+#define P2P_BFAN_F32 1      /* the same for fp32 plans */
+#endif
 #ifndef P2P_HALF2
 #define P2P_HALF2 1         /* 1: the filter tests two sources per instruction in packed FP16; 0: one per instruction in FP32 */
 #endif
@@ -217,9 +223,16 @@ template <> struct NearMath<float> {
 
 // CLAMP: xi rc is so large that the arguments of the function approximations must be clamped (other plans never leave
 // their range: every evaluated pair has r <= rc, a rejected one is evaluated at r = rc)
+// what k_p2p needs of the plan's geometry: a compact by-value parameter (see the note at SeGeom)
+struct P2PGeom {
+    int64_t N;
+    int ncell, pad_;
+    double L, xi, rc, wcell;
+};
+
 template <typename Real, bool CLAMP>
 __global__ void __launch_bounds__(P2P_WARPS * 32, P2P_BLOCKS)
-k_p2p(SeGeom g, const float4 *__restrict__ xq, const uint4 *__restrict__ xp, int64_t ns, const Real *__restrict__ src,
+k_p2p(P2PGeom g, const float4 *__restrict__ xq, const uint4 *__restrict__ xp, int64_t ns, const Real *__restrict__ src,
       const int *__restrict__ cell_start,
       const float4 *__restrict__ xq_t, const Real *__restrict__ src_t, const int *__restrict__ cellp,
       const double *__restrict__ mtab, Real *__restrict__ uN, float rc2m)
@@ -327,16 +340,29 @@ k_p2p(SeGeom g, const float4 *__restrict__ xq, const uint4 *__restrict__ xp, int
             const Real T0 = __shfl_sync(0xffffffffu, X0, o), T1 = __shfl_sync(0xffffffffu, X1, o);
             const Real T2 = __shfl_sync(0xffffffffu, X2, o);
             const int tcz = __shfl_sync(0xffffffffu, cz, o);
-            const int ro = (__shfl_sync(0xffffffffu, roff, o) + lane * QSTRIDE) & (QBYTES - 1);
+            // up to KB pairs per lane (entries lane, lane + 32, ... of the owner's queue), evaluated side by side like the
+            // pairs of mode A2, then ONE butterfly: independent dependency chains, and the reduction is paid once per
+            // 32 KB pairs (config 5 spends half of its pairs here).  A lane past the end re-evaluates the owner's last entry
+            // and drops it.
+            constexpr int KB = sizeof(Real) == 8 ? P2P_BFAN : P2P_BFAN_F32;
+            const int nB = cmax >= 32 ? min(cmax & ~31, 32 * KB) : cmax;      // whole waves of 32 pairs, or the rest
+            const int ro0 = __shfl_sync(0xffffffffu, roff, o);
             Real d0 = 0, d1 = 0, d2 = 0;
-            if (lane < cB) pair((o - lane) * 2 + ro, true, T0, T1, T2, tcz, d0, d1, d2);
+#pragma unroll
+            for (int k = 0; k < KB; ++k) {
+                if (32 * k < nB) {                               // warp-uniform
+                    const int idx = lane + 32 * k;
+                    const int qo = (ro0 + min(idx, nB - 1) * QSTRIDE) & (QBYTES - 1);
+                    pair((o - lane) * 2 + qo, idx < nB, T0, T1, T2, tcz, d0, d1, d2);
+                }
+            }
 #pragma unroll
             for (int sh = 16; sh > 0; sh >>= 1) {
                 d0 += __shfl_xor_sync(0xffffffffu, d0, sh);
                 d1 += __shfl_xor_sync(0xffffffffu, d1, sh);
                 d2 += __shfl_xor_sync(0xffffffffu, d2, sh);
             }
-            if (lane == o) { a0 += (double)d0; a1 += (double)d1; a2 += (double)d2; roff = (roff + cB * QSTRIDE) & (QBYTES - 1); }
+            if (lane == o) { a0 += (double)d0; a1 += (double)d1; a2 += (double)d2; roff = (roff + nB * QSTRIDE) & (QBYTES - 1); }
         } else if (KP > 1 && __popc(__ballot_sync(0xffffffffu, c >= KP)) * 4 >= __popc(m1) * 3) {
             // mode A2: most queues hold KP pairs: every lane pops up to that many of its own, evaluated side
             // by side (independent dependency chains); a lane with fewer re-evaluates its last one and drops it
@@ -612,12 +638,13 @@ cudaError_t p2p_impl(se_plan *p, cudaStream_t s)
     // CLAMP instantiation: plans whose arguments can leave the range of the function approximations (x = xi r <= 6 for
     // the rational erf(x)/x, 7.8 for the erfcx tables); every evaluated pair has r <= rc
     const bool rational = p->precision == SE_FP64 ? P2P_F64_RATIONAL != 0 : P2P_F32_RATIONAL != 0;
+    const P2PGeom pg{g.N, g.ncell, 0, g.L, g.xi, g.rc, g.wcell};
     if (g.xi * g.rc > (rational ? 5.99 : 7.8))
-        k_p2p<Real, true><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)S.xq, (const uint4 *)S.xp, S.n, (const Real *)S.src_near, S.cell_start,
+        k_p2p<Real, true><<<nblk, P2P_WARPS * 32, 0, s>>>(pg, (const float4 *)S.xq, (const uint4 *)S.xp, S.n, (const Real *)S.src_near, S.cell_start,
                                                          (const float4 *)T.xq, (const Real *)T.src_near, T.cell_sorted,
                                                          p->mtab, (Real *)p->uN, (float)rc2m);
     else
-        k_p2p<Real, false><<<nblk, P2P_WARPS * 32, 0, s>>>(g, (const float4 *)S.xq, (const uint4 *)S.xp, S.n, (const Real *)S.src_near, S.cell_start,
+        k_p2p<Real, false><<<nblk, P2P_WARPS * 32, 0, s>>>(pg, (const float4 *)S.xq, (const uint4 *)S.xp, S.n, (const Real *)S.src_near, S.cell_start,
                                                           (const float4 *)T.xq, (const Real *)T.src_near, T.cell_sorted,
                                                           p->mtab, (Real *)p->uN, (float)rc2m);
     p->launches += 1;
