@@ -69,6 +69,9 @@ constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV 
 #ifndef P2P_BFAN_F32
 #define P2P_BFAN_F32 1      /* the same for fp32 plans */
 #endif
+#ifndef P2P_BT
+#define P2P_BT 8            /* mode B only if the fullest queue could feed this many lanes more than there are non-empty queues */
+#endif
 #ifndef P2P_HALF2
 #define P2P_HALF2 1         /* 1: the filter tests two sources per instruction in packed FP16; 0: one per instruction in FP32 */
 #endif
@@ -290,8 +293,9 @@ k_p2p(P2PGeom g, const float4 *__restrict__ xq, const uint4 *__restrict__ xp, in
 
     auto queued = [&]() { return ((woff - roff) & (QBYTES - 1)) / QSTRIDE; };
     // One round of phase B.  Mode A (balanced): every lane with a queued pair pops and evaluates one of its own.
-    // Mode B (imbalanced: fewer non-empty queues than the fullest one could feed): the 32 lanes evaluate up to 32
-    // pairs of the fullest queue together and a butterfly sum hands the result to its owner.  The choice is a pure
+    // Mode B (imbalanced: at least P2P_BT fewer non-empty queues than the fullest one could feed; a measured threshold: with
+    // fewer idle lanes a plain round is cheaper than the reduction): the 32 lanes evaluate pairs of the fullest queue together
+    // and a butterfly sum hands the result to its owner.  The choice is a pure
     // function of the queue lengths, so the summation order stays deterministic.
     // one pair: queue entry at byte offset qo of this lane's (or, mode B, the owner's) column -> contribution d
     // keep = false: evaluate but contribute nothing; d0..d2 are ADDED to (fused into the last FMAs)
@@ -335,7 +339,7 @@ k_p2p(P2PGeom g, const float4 *__restrict__ xq, const uint4 *__restrict__ xp, in
         const unsigned m1 = __ballot_sync(0xffffffffu, c > 0);
         const int cmax = __reduce_max_sync(0xffffffffu, c);
         const int cB = min(cmax, 32);
-        if (cB > __popc(m1)) {                                   // mode B (warp-uniform)
+        if (cB > __popc(m1) + P2P_BT) {                          // mode B (warp-uniform)
             const int o = __ffs(__ballot_sync(0xffffffffu, c == cmax)) - 1;
             const Real T0 = __shfl_sync(0xffffffffu, X0, o), T1 = __shfl_sync(0xffffffffu, X1, o);
             const Real T2 = __shfl_sync(0xffffffffu, X2, o);
