@@ -72,6 +72,9 @@ constexpr int P2P_NV = 64;          // virtual-cell table entries per warp ((NV 
 #ifndef P2P_BT
 #define P2P_BT 8            /* mode B only if the fullest queue could feed this many lanes more than there are non-empty queues */
 #endif
+#ifndef P2P_A2Q
+#define P2P_A2Q 2          /* mode A2 when at least this many quarters of the non-empty queues hold KP pairs */
+#endif
 #ifndef P2P_HALF2
 #define P2P_HALF2 1         /* 1: the filter tests two sources per instruction in packed FP16; 0: one per instruction in FP32 */
 #endif
@@ -367,8 +370,8 @@ k_p2p(P2PGeom g, const float4 *__restrict__ xq, const uint4 *__restrict__ xp, in
                 d2 += __shfl_xor_sync(0xffffffffu, d2, sh);
             }
             if (lane == o) { a0 += (double)d0; a1 += (double)d1; a2 += (double)d2; roff = (roff + nB * QSTRIDE) & (QBYTES - 1); }
-        } else if (KP > 1 && __popc(__ballot_sync(0xffffffffu, c >= KP)) * 4 >= __popc(m1) * 3) {
-            // mode A2: most queues hold KP pairs: every lane pops up to that many of its own, evaluated side
+        } else if (KP > 1 && __popc(__ballot_sync(0xffffffffu, c >= KP)) * 4 >= __popc(m1) * P2P_A2Q) {
+            // mode A2: at least P2P_A2Q quarters of the non-empty queues hold KP pairs: every lane pops up to that many of its own, evaluated side
             // by side (independent dependency chains); a lane with fewer re-evaluates its last one and drops it
             if (c > 0) {
                 int ro = roff;
