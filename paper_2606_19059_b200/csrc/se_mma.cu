@@ -43,7 +43,16 @@
 
 namespace {
 
-constexpr int CAP = 48;              // candidates per round (one step's candidates, split if more)
+#ifndef SE_CAP
+#define SE_CAP 48
+#endif
+#ifndef SE_NST_P2G
+#define SE_NST_P2G 3
+#endif
+#ifndef SE_NST_G2P
+#define SE_NST_G2P 5
+#endif
+constexpr int CAP = SE_CAP;          // candidates per round (one step's candidates, split if more)
 constexpr int ZBW = SE_MMA_ZBIN;     // z-bin width of the sort key
 constexpr int NWY = SE_MMA_NWY, NWZ = SE_MMA_NWZ;
 
@@ -98,7 +107,7 @@ struct Cfg {
     static constexpr int MT = P / 8;                           // m-tiles in the ring
     static constexpr int REC = SPREAD ? SE_MMA_RECS(P) : SE_MMA_RECG(P);   // doubles per record
     static constexpr int OY = SPREAD ? 3 * P : P, OZ = OY + P, OM = OZ + P; // offsets of Wy, Wz, (a_y, a_z)
-    static constexpr int NST = SPREAD ? 3 : 5;                 // stages (measured: P2G 4 = 3, G2P 5 > 4)
+    static constexpr int NST = SPREAD ? SE_NST_P2G : SE_NST_G2P;   // stages (measured: P2G 4 = 3, G2P 5 > 4)
     static constexpr int GRP = SPREAD ? 4 : 8;                 // candidates per K-group (P2G: k = 4; G2P: n = 8)
     static constexpr int NSB = (P + BY - 2) / BY + 2, NSC = (P + BZ - 2) / BZ + 2;   // block tiles a window can meet
     static_assert(P % 4 == 0 && (!SPREAD || P % 8 == 0) && (REC % 2) == 0 && NCW % 4 == 0 && CAP % GRP == 0, "layout");

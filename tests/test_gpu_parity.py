@@ -278,7 +278,7 @@ def test_side_stream_overlap_is_bit_identical(monkeypatch):
 
 
 def test_large_xi_rc_clamp_path_and_tiny_N():
-    """xi rc = 9 > 7.8 selects the K2 instantiation that clamps the function-table arguments; N = 2 and N = 33
+    """xi rc = 9 selects the K2 instantiation that clamps the arguments of its function approximations; N = 2 and N = 33
     exercise warps with a single live lane and a ragged last warp."""
     from dataclasses import replace
     rng = np.random.default_rng(82)
@@ -291,6 +291,11 @@ def test_large_xi_rc_clamp_path_and_tiny_N():
     c = replace(W.CONFIGS[4], N=700, rc=0.3, xi=30.0, M=96, P=12, label="clamp fp32")
     x = rng.random((700, 3)).astype(np.float32); f = rng.standard_normal((700, 3)).astype(np.float32)
     check_all(c, x, f)
+    # xi rc = 7: beyond the range of the rational erf(x)/x (x <= 6) but inside that of the first design's tables (7.8)
+    c = replace(W.CONFIGS[1], N=700, rc=0.3, xi=7.0 / 0.3, M=80, P=24, label="xi rc = 7")
+    check_all(c, rng.random((700, 3)), rng.standard_normal((700, 3)))
+    c = replace(W.CONFIGS[4], N=700, rc=0.3, xi=7.0 / 0.3, M=80, P=12, label="xi rc = 7 fp32")
+    check_all(c, rng.random((700, 3)).astype(np.float32), rng.standard_normal((700, 3)).astype(np.float32))
 
 
 @pytest.mark.parametrize("P,M", [(16, 48), (32, 64), (8, 40), (2, 24)])
