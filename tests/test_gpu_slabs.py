@@ -84,3 +84,31 @@ def test_slab_plan_rejects_bad_arguments():
         assert (i.Mx, i.px0, i.grid_mode) == (48, 3, 2)
         with pytest.raises(se.SeError):
             p.stage("fft")                                          # a slab plan transforms nothing
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_scale_block_equals_the_scale_stage(prec):
+    """se_scale_block on ky-pencils [3, M, nky, M/2 + 1] reproduces, block by block and bit for bit, what SE_STAGE_SCALE does
+    to the whole spectrum (same kernel, ky offset), and agrees with the oracle's multiplier on sampled modes."""
+    import torch
+    import paper_2606_19059_b200 as se
+    c, x, f = W.scaled(3 if prec == "fp64" else 4, 4000)
+    M, Mh = c.M, c.M // 2 + 1
+    rdt, cdt = (torch.float64, torch.complex128) if prec == "fp64" else (torch.float32, torch.complex64)
+    g = torch.Generator(device="cuda").manual_seed(5)
+    spec = torch.randn(3, M, M, Mh, 2, dtype=rdt, device="cuda", generator=g)
+    with se.Plan(c.N, c.L, c.xi, c.rc, M, c.P, prec) as p:
+        p.write(se.SE_BUF_SPEC, spec.clone())
+        p.stage("scale")
+        whole = torch.view_as_complex(p.read(se.SE_BUF_SPEC))
+        sc = torch.view_as_complex(spec)
+        for ky0, nky in ((0, 7), (7, M // 2 - 7), (M // 2, M - M // 2)):
+            blk = sc[:, :, ky0:ky0 + nky].contiguous().to(cdt)
+            p.scale_block(blk, ky0, nky)
+            assert torch.equal(blk, whole[:, :, ky0:ky0 + nky])
+    rng = np.random.default_rng(3)
+    idx = np.stack([rng.integers(0, M, 300), rng.integers(0, M, 300), rng.integers(0, Mh, 300)], axis=1)
+    vals = sc[:, idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy().T.astype(np.complex128)
+    ref = oracle.scale_modes(idx, vals, c.L, c.xi, M, c.P)
+    got = whole[:, idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy().T
+    gate("scaled modes", got, ref, TOL[prec]["Hs"])
