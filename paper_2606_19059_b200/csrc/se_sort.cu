@@ -169,12 +169,17 @@ __global__ void k_scatter(int64_t N, const int *__restrict__ cell_of, const int 
 // summation order) is a pure function of the input.  One thread per sorted slot, O(s) each.
 __global__ void k_rank_in_cell(int64_t N, const int *__restrict__ key_of, const int *__restrict__ start,
                                const int *__restrict__ perm_in, int *__restrict__ perm_out,
-                               int *__restrict__ inv)
+                               int *__restrict__ inv, int skip_key)
 {
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= N) return;
     int i = perm_in[p];
     int c = key_of[i];
+    if (c == skip_key) {                 // the bin of a slab plan's ghost sources: never gridded, any order will do (it
+        perm_out[p] = i;                 // can hold tens of thousands of points, and the ranking below is O(occupancy))
+        inv[i] = (int)p;
+        return;
+    }
     int s = start[c], e = start[c + 1];
     int r = 0;
     for (int q = s; q < e; ++q) r += (perm_in[q] < i);
@@ -350,8 +355,8 @@ cudaError_t sort_set(se_plan *p, SeSet &S, const void *xv, const void *fv, bool 
     int *tmp_near = S.cell_sorted, *tmp_grid = (int *)S.fs_grid;  // both >= n ints, overwritten later
     k_scatter<<<nblk, T, 0, s>>>(g.N, S.cell_of, S.bin_of, S.cell_cursor, S.bin_cursor,
                                  tmp_near, S.inv_near, tmp_grid, S.inv_grid);
-    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, S.cell_of, S.cell_start, tmp_near, S.perm_near, S.inv_near);
-    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, S.bin_of, S.bin_start, tmp_grid, S.perm_grid, S.inv_grid);
+    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, S.cell_of, S.cell_start, tmp_near, S.perm_near, S.inv_near, -1);
+    k_rank_in_cell<<<nblk, T, 0, s>>>(g.N, S.bin_of, S.bin_start, tmp_grid, S.perm_grid, S.inv_grid, g.nbins_total);
     k_gather_near<Real><<<nblk, T, 0, s>>>(g, x, f, S.perm_near, S.cell_of, (Real *)S.src_near,
                                            (float4 *)S.xq, (unsigned short *)S.xp, S.cell_sorted);
     int64_t nt = (g.N + (g.P <= 16 ? 1 : 0)) / (g.P <= 16 ? 2 : 1) * 32;   // 16 or 32 lanes per particle

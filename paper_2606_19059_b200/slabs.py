@@ -157,9 +157,13 @@ class SlabEval:
         import torch
         lay = self.lay
         Ky = lay.M // lay.world
-        S = torch.fft.fft(torch.cat(list(blocks), dim=1), dim=1).contiguous()        # [3, M, Ky, M/2+1]
+        # the transform over x runs on a copy with x as the fastest index (cuFFT's strided 1-D transforms are several times
+        # slower than two transposes), K4 on the x-slowest layout it is written for
+        Bx = torch.cat(list(blocks), dim=1).permute(0, 2, 3, 1).contiguous()         # [3, Ky, M/2+1, M]
+        S = torch.fft.fft(Bx, dim=3).permute(0, 3, 1, 2).contiguous()                # [3, M, Ky, M/2+1]
         self._tables().scale_block(S, self.rank * Ky, Ky, stream=stream)
-        B = torch.fft.ifft(S, dim=1, norm="forward")                    # unnormalised inverse
+        Bx = torch.fft.ifft(S.permute(0, 2, 3, 1).contiguous(), dim=3, norm="forward")   # unnormalised inverse
+        B = Bx.permute(0, 3, 1, 2)
         return [B[:, d * lay.Ml:(d + 1) * lay.Ml].contiguous() for d in range(lay.world)]
 
     def planes_back(self, blocks):
