@@ -112,3 +112,23 @@ def test_scale_block_equals_the_scale_stage(prec):
     ref = oracle.scale_modes(idx, vals, c.L, c.xi, M, c.P)
     got = whole[:, idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy().T
     gate("scaled modes", got, ref, TOL[prec]["Hs"])
+
+
+def test_slabs_config3_full_size_against_the_one_gpu_plan():
+    """Config 3 at full size (N = 1,048,576, M = 360) cut into 4 slabs against se_eval on the whole problem (which
+    tests/test_gpu_fullsize.py compares with the oracle on all N): same kernels, so the two agree to rounding."""
+    import torch
+    import paper_2606_19059_b200 as se
+    from paper_2606_19059_b200 import slabs
+    c, x, f = W.make(3)
+    lay = slabs.SlabLayout(c.L, c.M, c.P, c.rc, 4)
+    own = lay.owner(x[:, 0])
+    idx = [np.nonzero(own == r)[0] for r in range(4)]
+    us = slabs.evaluate_emulated(lay, c.xi, [torch.as_tensor(x[i], device="cuda") for i in idx],
+                                 [torch.as_tensor(f[i], device="cuda") for i in idx])
+    u = np.empty_like(x)
+    for i, ur in zip(idx, us):
+        u[i] = ur.cpu().numpy()
+    with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P) as p:
+        ref = p.eval(torch.as_tensor(x, device="cuda"), torch.as_tensor(f, device="cuda")).cpu().numpy()
+    gate("u, config 3, 4 slabs vs one plan", u, ref, 1e-13)
