@@ -37,7 +37,7 @@ UNIT = "particles/s"
 # (se_measure_peak: register-only DFMA / DMMA / FFMA chains, run before the timed region) are unavailable.
 NOMINAL_TFLOPS = {"fp64": 148 * 64 * 2 * 1.965e9 / 1e12, "fp32": 148 * 128 * 2 * 1.965e9 / 1e12}
 # FP64 (FP32) arithmetic instructions K2 spends per in-range pair (DESIGN.md section 6 "K2"): the "alu" work of P2P.
-# fp64: 60 DFMA + 10.5 DMUL + 7 DADD + 3 DSETP per pair in the SASS of the evaluation round (profiles/r02q_final.md);
+# fp64: 60 DFMA + 10.5 DMUL + 7 DADD + 3 DSETP per pair in the SASS of the evaluation round (profiles/r02r_final.md);
 # fp32: the same algorithm with the degree-6 rational and expf, counted from the source
 P2P_INSTR_PER_PAIR = {"fp64": 80, "fp32": 50}
 # sub-results of the default run (world size 1): (key, config, steps, plan overrides)
