@@ -29,7 +29,7 @@
  *   - There is no CPU fallback: without a CUDA device se_plan_create returns SE_ECUDA.
  *   - Environment variables read at se_plan_create (experiments and tests only; results do not change beyond
  *     rounding order): SE_GRID_MODE = tile (force the generic gridding kernel; default: the FP64 tensor-core
- *     sweep for fp64 plans with P = 8, 12, 16, 24 and fp32 plans with P = 8, 12, else the generic tile kernel),
+ *     sweep for fp64 plans with even 4 <= P <= 24 and fp32 plans with even 4 <= P <= 16, else the generic tile kernel),
  *     SE_NCHUNK and SE_NCHUNK_G2P (x-chunks of K3 / K5), SE_OVERLAP = 1 (K2 on a side stream next to the FFT
  *     stages).
  */

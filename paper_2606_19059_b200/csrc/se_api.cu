@@ -191,6 +191,7 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
             (slab || (nbins_mma <= 64.0 * (double)std::max(N, Nt) + 4.0e6 && !want_tile))) {
             g.grid_mode = 2;
             g.ring = se_mma_ring(P);
+            g.ring_g = se_mma_ring_g(P);
             g.nbin = zb;
             g.nbins_total = Mx * zb * M;
             const int BY = 4 * SE_MMA_NWY, BZ = 4 * SE_MMA_NWZ;
@@ -276,7 +277,7 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
         A.get(&Q.anchor, n * sizeof(short4));
         if (g.grid_mode == 2) {
             if (spread) A.get(&Q.wtab, (size_t)n * SE_MMA_RECS(g.ring) * 8);
-            if (gather) A.get(&Q.recg, (size_t)n * SE_MMA_RECG(P) * 8);
+            if (gather) A.get(&Q.recg, (size_t)n * SE_MMA_RECG(g.ring_g) * 8);
         } else
             A.get(&Q.wtab, (size_t)n * 3 * P * rb);
         A.get(&Q.fs_grid, std::max((size_t)n * 3 * rb, (size_t)n * sizeof(int)));

@@ -24,9 +24,9 @@ constexpr int SE_PMAX = 32;                          // largest window support
 // FP64 tensor-core gridding kernels (se_mma.cu): particles sorted by (anchor plane, anchor_z / ZBIN, anchor_y);
 // a block of NWY x NWZ consumer warps (+ the producer warpgroup) owns 4 NWY x 4 NWZ (y, z) columns.  K1 writes two
 // 16-byte aligned records per particle in sorted order (always double, also for fp32 plans; anchors as two int32
-// in one double slot; R = P rounded up to a multiple of 8, rows zero beyond P):
+// in one double slot; R = P rounded up to a multiple of 8, Rg = P rounded up to a multiple of 4, rows zero beyond P):
 //   spread record, SE_MMA_RECS(R) doubles: c_w f_x Wx[R] | c_w f_y Wx[R] | c_w f_z Wx[R] | Wy[R] | Wz[R] | (a_y, a_z) | pad
-//   gather record, SE_MMA_RECG(P) doubles: Wx[P] | Wy[P] | Wz[P] | (a_y, a_z) | pad
+//   gather record, SE_MMA_RECG(Rg) doubles: Wx[Rg] | Wy[Rg] | Wz[Rg] | (a_y, a_z) | pad
 // (sizes = 24 mod 32 four-byte words, so that consecutive records start in different shared-memory bank octets)
 constexpr int SE_MMA_ZBIN = 8;
 constexpr int SE_MMA_NWY = 2, SE_MMA_NWZ = 6;
@@ -50,10 +50,10 @@ struct SeGeom {
     short window;       // se_window
     short nu;           // Kaiser-Bessel: polynomial degree per bin
     short grid_mode;    // 0: tile-stationary k_grid (any even P),
-                        // 2: FP64 tensor-core sweep (se_mma.cu; fp64 P = 8, 12, 16, 24; fp32 P = 8, 12)
+                        // 2: FP64 tensor-core sweep (se_mma.cu; fp64 any even P <= 24, fp32 any even P <= 16)
     short ring;         // mma mode: row stride of the spread records = P rounded up to a multiple of 8
     short rel_coords;   // 1: near-sorted positions are cell-relative (fp32 path)
-    short pad_;
+    short ring_g;       // mma mode: row stride of the gather records = P rounded up to a multiple of 4
     double L, xi, rc;
     double h;           // L / M
     double wcell;       // L / ncell
@@ -148,3 +148,4 @@ cudaError_t se_launch_mma_g2p(se_plan *p, cudaStream_t s);
 bool se_mma_supported(int P, int precision);
 int se_mma_slots(int P);
 int se_mma_ring(int P);
+int se_mma_ring_g(int P);

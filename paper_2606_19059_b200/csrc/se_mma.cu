@@ -1,6 +1,7 @@
 // K3 P2G (eq. (2.5)) and K5 G2P (eq. (2.7)) in FP64 as an x-SWEEP whose inner
-// product runs on the FP64 tensor-core instruction (mma.sync m8n8k4 f64 -> DMMA), for P = 16 and 24 in fp64
-// plans and P = 12 in fp32 plans (float grid, double records and accumulators; P2G on a ring of 16 planes).
+// product runs on the FP64 tensor-core instruction (mma.sync m8n8k4 f64 -> DMMA), for every even 4 <= P <= 24 in fp64
+// plans and 4 <= P <= 16 in fp32 plans (float grid, double records and accumulators); supports that are not a
+// multiple of 8 (P2G) / 4 (G2P) run on the next ring size with zero rows in the records.
 //
 // Why.  With a Gaussian window at P = 24 both gridding steps are FP64-arithmetic bound: 3 P^3 = 41,472
 // FMA per particle against ~1 KB of compulsory traffic.  On B200 DFMA and DMMA
@@ -171,7 +172,7 @@ __global__ void __launch_bounds__((NWY * NWZ + 4) * 32, 1)
 k_mma(MmaGeom g, const double *__restrict__ recs, const int *__restrict__ bin_start, GR *__restrict__ grid,
       double *__restrict__ uFpart)
 {
-    static_assert(W <= P && (SPREAD || W == P), "window / ring");
+    static_assert(W <= P && W > P - (SPREAD ? 8 : 4), "window / ring");
     typedef Cfg<P, SPREAD> C;
     constexpr int NCW = C::NCW, BY = C::BY, BZ = C::BZ, MT = C::MT, REC = C::REC, NST = C::NST, GRP = C::GRP;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -629,7 +630,7 @@ k_mma(MmaGeom g, const double *__restrict__ recs, const int *__restrict__ bin_st
 }
 
 // u^F (grid-sorted order) = fixed-order sum of the slots the particle's window actually meets
-template <int P, typename GR>
+template <int P, int W, typename GR>
 __global__ void k_reduce_slots(SeGeom g, const short4 *__restrict__ anchor, const double *__restrict__ part,
                                GR *__restrict__ uF)
 {
@@ -642,10 +643,10 @@ __global__ void k_reduce_slots(SeGeom g, const short4 *__restrict__ anchor, cons
     double s0 = 0.0, s1 = 0.0, s2 = 0.0;
     for (int rb = 0; rb < C::NSB && rb < ntY; ++rb) {
         const int ty = (a.y / C::BY + rb) % ntY, Y0 = ty * C::BY;
-        if (!meets(modM(Y0 - a.y, M), min(C::BY, M - Y0), M, P)) continue;
+        if (!meets(modM(Y0 - a.y, M), min(C::BY, M - Y0), M, W)) continue;
         for (int rc = 0; rc < C::NSC && rc < ntZ; ++rc) {
             const int tz = (a.z / C::BZ + rc) % ntZ, Z0 = tz * C::BZ;
-            if (!meets(modM(Z0 - a.z, M), min(C::BZ, M - Z0), M, P)) continue;
+            if (!meets(modM(Z0 - a.z, M), min(C::BZ, M - Z0), M, W)) continue;
             const double *q = part + ((size_t)(rb * C::NSC + rc) * g.N + i) * 3;
             s0 += q[0]; s1 += q[1]; s2 += q[2];
         }
@@ -673,7 +674,7 @@ cudaError_t launch_k(se_plan *p, cudaStream_t s, bool prepare)
                                                              (GR *)p->grid, (double *)p->uFpart);
     p->launches += 1;
     if (!SPREAD) {
-        k_reduce_slots<P, GR><<<(unsigned)((g.N + 255) / 256), 256, 0, s>>>(g, Q.anchor, (const double *)p->uFpart,
+        k_reduce_slots<P, W, GR><<<(unsigned)((g.N + 255) / 256), 256, 0, s>>>(g, Q.anchor, (const double *)p->uFpart,
                                                                             (GR *)p->uF);
         p->launches += 1;
     }
@@ -689,37 +690,43 @@ cudaError_t launch(se_plan *p, cudaStream_t s, bool prepare)
 template <bool SPREAD>
 cudaError_t dispatch(se_plan *p, cudaStream_t s, bool prepare = false)
 {
-    // ring (row stride of the records) P rounded up to 8 for P2G; fp32 plans: float grid, double records / accumulators
+    // ring (row stride of the records; the rows are zero beyond the window): P rounded up to a multiple of 8 for P2G
+    // (m-tiles of 8 planes), of 4 for G2P (k-steps of 4 planes); fp32 plans: float grid, double records / accumulators
+#define SE_MMA_CASE(W, GR) \
+    case W: return launch<SPREAD ? (W + 7) / 8 * 8 : (W + 3) / 4 * 4, SPREAD, W, GR>(p, s, prepare);
     if (p->precision == SE_FP64) {
         switch (p->g.P) {
-        case 24: return launch<24, SPREAD, 24, double>(p, s, prepare);
-        case 16: return launch<16, SPREAD, 16, double>(p, s, prepare);
-        case 12: return launch<SPREAD ? 16 : 12, SPREAD, 12, double>(p, s, prepare);
-        case 8: return launch<8, SPREAD, 8, double>(p, s, prepare);
+            SE_MMA_CASE(4, double) SE_MMA_CASE(6, double) SE_MMA_CASE(8, double) SE_MMA_CASE(10, double)
+            SE_MMA_CASE(12, double) SE_MMA_CASE(14, double) SE_MMA_CASE(16, double) SE_MMA_CASE(18, double)
+            SE_MMA_CASE(20, double) SE_MMA_CASE(22, double) SE_MMA_CASE(24, double)
         default: return cudaErrorInvalidValue;
         }
     }
     switch (p->g.P) {
-    case 12: return launch<SPREAD ? 16 : 12, SPREAD, 12, float>(p, s, prepare);
-    case 8: return launch<8, SPREAD, 8, float>(p, s, prepare);
+        SE_MMA_CASE(4, float) SE_MMA_CASE(6, float) SE_MMA_CASE(8, float) SE_MMA_CASE(10, float)
+        SE_MMA_CASE(12, float) SE_MMA_CASE(14, float) SE_MMA_CASE(16, float)
     default: return cudaErrorInvalidValue;
     }
+#undef SE_MMA_CASE
 }
 
 }  // namespace
 
 bool se_mma_supported(int P, int precision)
 {
-    return precision == SE_FP64 ? (P == 24 || P == 16 || P == 12 || P == 8) : (P == 12 || P == 8);
+    return P >= 4 && !(P & 1) && P <= (precision == SE_FP64 ? 24 : 16);
 }
 int se_mma_ring(int P) { return (P + 7) / 8 * 8; }     // row stride of the spread records
-int se_mma_slots(int P)
+int se_mma_ring_g(int P) { return (P + 3) / 4 * 4; }   // row stride of the gather records
+int se_mma_slots(int P)                                // slots of a particle in uFpart: block tiles its window can meet
 {
-    switch (P) {
+    switch (se_mma_ring_g(P)) {
     case 24: return Cfg<24, false>::NSB * Cfg<24, false>::NSC;
+    case 20: return Cfg<20, false>::NSB * Cfg<20, false>::NSC;
     case 16: return Cfg<16, false>::NSB * Cfg<16, false>::NSC;
     case 12: return Cfg<12, false>::NSB * Cfg<12, false>::NSC;
-    default: return Cfg<8, false>::NSB * Cfg<8, false>::NSC;
+    case 8: return Cfg<8, false>::NSB * Cfg<8, false>::NSC;
+    default: return Cfg<4, false>::NSB * Cfg<4, false>::NSC;
     }
 }
 cudaError_t se_launch_mma_p2g(se_plan *p, cudaStream_t s) { return dispatch<true>(p, s); }

@@ -24,12 +24,15 @@ __device__ __forceinline__ int near_cell1(double v, const SeGeom &g)
     return min(max(c, 0), g.ncell - 1);
 }
 
-// base grid index floor(x/h) and fractional offset in grid units
+// base grid index floor(x/h), in [0, M], and fractional offset in grid units.  M itself happens for the last few
+// representable points below L, where x/h rounds up to M: the window then starts at anchor M - (P/2 - 1) and wraps
+// like any other (the oracle's window_1d takes the same floor and wraps the indices), so the callers
+// wrap the index instead of clamping it to M - 1 (which would truncate the window one plane earlier)
 __device__ __forceinline__ int grid_base1(double v, const SeGeom &g, double &frac)
 {
     double q = v / g.h;
     int i0 = (int)floor(q);
-    i0 = min(max(i0, 0), g.M - 1);
+    i0 = min(max(i0, 0), g.M);
     frac = q - (double)i0;
     return i0;
 }
@@ -47,6 +50,7 @@ __global__ void k_bin(SeGeom g, const Real *__restrict__ x, int *__restrict__ ce
         c[d] = near_cell1(v, g);
         double fr;
         b[d] = grid_base1(v, g, fr);
+        if (b[d] == g.M) b[d] = 0;
     }
     int ci = (c[0] * g.ncell + c[1]) * g.ncell + c[2];
     int bi;
@@ -263,8 +267,8 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
         fd = f ? f[3 * (int64_t)i + l] : (Real)0;
     }
     const bool recs = g.grid_mode == 2;
-    const int R = recs ? g.ring : P;
-    Rec *rs = wtab + pc * SE_MMA_RECS(R), *rg = recg + pc * SE_MMA_RECG(P);
+    const int R = recs ? g.ring : P, Rg = recs ? g.ring_g : P;         // row strides (R >= Rg >= P)
+    Rec *rs = wtab + pc * SE_MMA_RECS(R), *rg = recg + pc * SE_MMA_RECG(Rg);
     Rec cf[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) cf[c] = (Rec)g.cw * (Rec)__shfl_sync(0xffffffffu, fd, gbase + c);   // c_w of eq. (2.5) folded in
@@ -289,7 +293,7 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
         }
         const Rec w = (Rec)wv;
         if (recs) {
-            if (recg && l < P) rg[d * P + l] = w;
+            if (recg && l < Rg) rg[d * Rg + l] = w;
             if (wtab) {
                 if (d == 0) {
 #pragma unroll
@@ -303,13 +307,14 @@ __global__ void k_gather_grid(SeGeom g, const Real *__restrict__ x, const Real *
     if (live && l < 3) {
         int a = i0 - (P / 2 - 1);
         if (a < 0) a += g.M;
+        if (a >= g.M) a -= g.M;
         short *ap = reinterpret_cast<short *>(&anchor[p]);
         ap[l] = (short)a;
         if (l == 0) ap[3] = 0;
         fs[3 * p + l] = fd;
         if (recs && l > 0) {
             if (wtab) reinterpret_cast<int *>(&rs[5 * R])[l - 1] = a;
-            if (recg) reinterpret_cast<int *>(&rg[P3])[l - 1] = a;
+            if (recg) reinterpret_cast<int *>(&rg[3 * Rg])[l - 1] = a;
         }
     }
 }

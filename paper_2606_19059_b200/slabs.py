@@ -41,11 +41,18 @@ class SlabLayout:
         """global index of local plane 0 of `rank`"""
         return (rank * self.Ml - self.nlo) % self.M
 
+    @staticmethod
+    def _quot(a, b):
+        """a / b rounded as the IEEE quotient K1 takes (torch's CUDA kernels turn a division by a Python scalar into a
+        multiplication by its reciprocal, which moves floor(x/h) by one for points within an ulp of a plane)"""
+        import torch
+        return torch.div(a, torch.full_like(a, b))
+
     def _wrap(self, x0):
         """x0 wrapped into [0, L) exactly as K1 does it (a result that is not in [0, L), e.g. L itself after rounding, is 0)"""
         if hasattr(x0, "floor"):                    # torch
             import torch
-            xw = x0 - self.L * (x0 / self.L).floor()
+            xw = x0 - self.L * self._quot(x0, self.L).floor()
             return torch.where((xw >= 0) & (xw < self.L), xw, torch.zeros_like(xw))
         xw = x0 - self.L * np.floor(x0 / self.L)
         return np.where((xw >= 0) & (xw < self.L), xw, 0.0)
@@ -54,8 +61,8 @@ class SlabLayout:
         """floor(x_w / h) of first coordinates (numpy or torch, double), as the library takes it"""
         xw = self._wrap(x0)
         if hasattr(xw, "floor"):
-            return (xw / self.h).floor().long().clamp(0, self.M - 1)
-        return np.clip(np.floor(xw / self.h).astype(np.int64), 0, self.M - 1)
+            return self._quot(xw, self.h).floor().long().clamp(0, self.M) % self.M      # x/h may round up to M: plane 0
+        return np.clip(np.floor(xw / self.h).astype(np.int64), 0, self.M) % self.M
 
     def owner(self, x0):
         """rank that owns each point (by the base grid plane of its first coordinate)"""
@@ -65,6 +72,11 @@ class SlabLayout:
         """(to_left, to_right): which of this rank's points lie within rc of its lower / upper face (periodic)"""
         lo, hi = rank * self.Ml * self.h, (rank + 1) * self.Ml * self.h
         xw = self._wrap(x0)
+        if hasattr(xw, "floor"):                    # a point whose x/h rounds up to M lives in plane 0 (rank 0): it sits at 0-
+            import torch
+            xw = torch.where(self._quot(xw, self.h).floor() >= self.M, xw - self.L, xw)
+        else:
+            xw = np.where(np.floor(xw / self.h) >= self.M, xw - self.L, xw)
         to_left, to_right = (xw - lo) < self.rc, (hi - xw) <= self.rc
         if self.world == 2:                         # both neighbours are the same rank: a point goes there once
             to_left = to_left & ~to_right

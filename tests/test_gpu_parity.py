@@ -42,7 +42,7 @@ def check_all(c, x, f, tol_override=None):
     pos_cell = np.searchsorted(cs, np.arange(N), side="right") - 1
     assert np.array_equal(lin[g["perm_near"]], pos_cell)
     nb = g["info"]["nbin"]
-    i0 = np.minimum(np.floor(xw / (c.L / c.M)).astype(np.int64), c.M - 1)
+    i0 = np.floor(xw / (c.L / c.M)).astype(np.int64) % c.M     # x/h may round up to M: the periodic image
     if g["info"]["grid_mode"] == 2:      # FP64 tensor-core sweep: key (anchor plane, anchor_z / 8, anchor_y)
         an = (i0 - (c.P // 2 - 1)) % c.M
         linb = (an[:, 0] * nb + an[:, 2] // 8) * c.M + an[:, 1]
@@ -300,13 +300,48 @@ def test_large_xi_rc_clamp_path_and_tiny_N():
 
 @pytest.mark.parametrize("P,M", [(16, 48), (32, 64), (8, 40), (2, 24)])
 def test_other_window_sizes_fp64(P, M):
-    """P = 16 is the second tensor-core instantiation; P = 32 (the largest support), 8 and 2 run the generic tile
+    """P = 16 and 8 are tensor-core instantiations; P = 32 (the largest support) and 2 run the generic tile
     kernel.  Small P make the method inaccurate, not the parity: the oracle uses the same discretisation."""
     from dataclasses import replace
     rng = np.random.default_rng(83 + P)
     c = replace(W.CONFIGS[1], N=900, rc=0.2, xi=12.0, M=M, P=P, label=f"P={P} M={M}")
     x = rng.random((900, 3)); f = rng.standard_normal((900, 3))
     check_all(c, x, f)
+
+
+@pytest.mark.parametrize("prec,P", [("fp64", 4), ("fp64", 6), ("fp64", 10), ("fp64", 14), ("fp64", 18), ("fp64", 20),
+                                    ("fp64", 22), ("fp32", 4), ("fp32", 6), ("fp32", 10), ("fp32", 14), ("fp32", 16)])
+def test_padded_ring_supports(prec, P):
+    """Supports that are not a multiple of 8 (P2G) / 4 (G2P) run the tensor-core sweep on a ring padded with zero
+    rows (records of stride ceil8(P) / ceil4(P)): grids from the smallest the ring fits (M = ceil8(P)) to several
+    block tiles with a ragged tail, points on the faces, and the evaluation is bit-repeatable (no atomics)."""
+    from dataclasses import replace
+    import torch
+    import paper_2606_19059_b200 as se
+    rng = np.random.default_rng(4100 + P)
+    dt = np.float32 if prec == "fp32" else np.float64
+    ring = (P + 7) // 8 * 8
+    base = W.CONFIGS[4] if prec == "fp32" else W.CONFIGS[1]
+    for M in (ring, ring + 2, 50, 74):
+        if M < P:
+            continue
+        N = 700
+        h = 1.0 / M
+        xi = 0.8 * 0.95 * np.sqrt(np.pi * P) / (P * h)
+        rc = min(0.3, 3.2 / xi) if prec == "fp32" else min(0.3, 4.5 / xi)
+        c = replace(base, N=N, L=1.0, rc=rc, xi=xi, M=M, P=P, label=f"{prec} P={P} M={M} (padded ring)")
+        x = rng.random((N, 3)).astype(dt)
+        x[0] = [0.0, 0.0, 0.0]
+        x[1] = [np.nextafter(dt(1.0), dt(0)), 0.5, 0.25]
+        f = rng.standard_normal((N, 3)).astype(dt)
+        check_all(c, x, f)
+        plan = se.Plan(N, 1.0, rc=rc, xi=xi, M=M, P=P, precision=prec)
+        assert plan.info().grid_mode == 2
+        xd, fd = torch.from_numpy(x).cuda(), torch.from_numpy(f).cuda()
+        u1 = plan.eval(xd, fd).clone()
+        u2 = plan.eval(xd, fd)
+        assert torch.equal(u1, u2)
+        plan.destroy()
 
 
 @pytest.mark.parametrize("seed", range(12))

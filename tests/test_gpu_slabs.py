@@ -72,6 +72,22 @@ def test_slabs_empty_slab_and_points_on_faces():
     gate("u, empty slabs", u, ref, TOL["fp64"]["u"])
 
 
+def test_slabs_padded_ring_and_the_last_point_below_L():
+    """P = 10 (ring of 16 / 12 planes, zero rows) on three slabs, M = 72: the largest double below L has x/h = M after
+    rounding, so its base plane is plane 0 of rank 0 and it is a ghost source of the last rank (PAPER.md:215 anchor,
+    periodic index wrap) -- at P = 10 the window's edge value (7e-7) makes a clamp to plane M - 1 visible."""
+    from dataclasses import replace
+    rng = np.random.default_rng(190590 + 7)
+    N, M, P = 5000, 72, 10
+    xi = 0.8 * 0.95 * np.sqrt(np.pi * P) * M / P
+    c = replace(W.CONFIGS[3], N=N, M=M, P=P, rc=4.5 / xi, xi=xi, label="P = 10 slabs")
+    x = rng.random((N, 3)); f = rng.standard_normal((N, 3))
+    x[:30, 0] = np.repeat([0.0, np.nextafter(1.0, 0), np.nextafter(1.0 / 3.0, 0)], 10)
+    assert np.floor(x[10, 0] / (1.0 / M)) == M
+    u, ref, counts = run_slabs(c, x, f, 3)
+    gate("u, 3 slabs, P = 10", u, ref, TOL["fp64"]["u"])
+
+
 def test_slab_plan_rejects_bad_arguments():
     import paper_2606_19059_b200 as se
     c, x, f = W.scaled(3, 20000)

@@ -33,7 +33,7 @@ def test_layout_planes_and_ownership():
     own = lay.owner(x0)
     xw = x0 - np.floor(x0)
     xw[xw >= 1.0] = 0.0
-    ref = np.minimum(np.floor(xw / (L / M)).astype(int), M - 1) // lay.Ml
+    ref = (np.floor(xw / (L / M)).astype(int) % M) // lay.Ml
     assert np.array_equal(own, ref)
 
 
