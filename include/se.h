@@ -77,6 +77,12 @@ enum {
     SE_STAGE_SUM = 7,    /* K6: u = u^N + u^F - (4 xi/sqrt(pi)) f, user order    */
     SE_NSTAGES = 8
 };
+/* se_eval_stage runs stages 3-5 as written above (3-D transforms, spectrum readable in between).  se_eval, se_eval_targets
+ * and se_eval_host run them FUSED when se_info.fft_fused is 1 (M has no prime factor above 7 and 3 x 4 (fp32: 3 x 8) columns
+ * of M modes fit in shared memory; SE_FFT_MODE=3d at plan creation switches it off): stage 3 = cuFFT 2-D R2C over (y, z) of
+ * every x-plane, stage 4 = ONE kernel that transforms over x, applies K4 and transforms back over x (a 3-D transform is the
+ * 2-D transforms followed by 1-D transforms over x, and K4 is diagonal in k), stage 5 = cuFFT 2-D C2R.  The result H~ is the
+ * same up to rounding; SE_BUF_SPEC then holds the 2-D spectra, and se_stage_ms reports the three parts under the same names. */
 
 /* Internal buffers visible to tests and the benchmark through se_buffer_read/write. */
 enum {
@@ -117,6 +123,8 @@ typedef struct {
     int nu;              /* Kaiser-Bessel: degree of the piecewise polynomial            */
     double kb_beta;      /* Kaiser-Bessel: beta = 2.5 P ; a_w = P h / 2                  */
     int Mx, px0;         /* planes of the plan's grid along x (M unless a slab plan) and global index of plane 0 */
+    int fft_fused;       /* 1: se_eval / se_eval_targets / se_eval_host run the transform over x, K4 and the inverse transform
+                            over x as one kernel between cuFFT 2-D transforms of the x-planes (see SE_STAGE_SCALE below) */
 } se_info;
 
 /* Everything se_plan_create takes, plus the window and an optional separate target count. */

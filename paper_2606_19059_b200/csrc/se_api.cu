@@ -37,10 +37,12 @@ void free_all(se_plan *p)
     };
     free_set(p->S);
     if (p->own_targets) free_set(p->T);
-    void *ptrs[] = {p->uN, p->uF, p->uFpart, p->grid, p->spec, p->ktab, p->mtab, p->wcoef, p->hx, p->hf, p->hu};
+    void *ptrs[] = {p->uN, p->uF, p->uFpart, p->grid, p->spec, p->ktab, p->mtab, p->wcoef, p->hx, p->hf, p->hu, p->xf_tw, p->xf_xk};
     for (void *q : ptrs) if (q) cudaFree(q);
     if (p->fft_ok & 1) cufftDestroy(p->fft_fwd);
     if (p->fft_ok & 2) cufftDestroy(p->fft_inv);
+    if (p->fft2_ok & 1) cufftDestroy(p->fft2_fwd);
+    if (p->fft2_ok & 2) cufftDestroy(p->fft2_inv);
     if (p->ev_ok) for (int i = 0; i <= SE_NSTAGES; ++i) cudaEventDestroy(p->ev[i]);
     if (p->side_ok) {
         cudaEventDestroy(p->ev_fork); cudaEventDestroy(p->ev_join);
@@ -50,9 +52,10 @@ void free_all(se_plan *p)
     delete p;
 }
 
-se_status run_fft(se_plan *p, bool forward, cudaStream_t s)
+// planes == false: the 3-D transforms; planes == true: the 2-D transforms over (y, z) of every x-plane (fused path, K4x)
+se_status run_fft(se_plan *p, bool forward, cudaStream_t s, bool planes = false)
 {
-    cufftHandle h = forward ? p->fft_fwd : p->fft_inv;
+    cufftHandle h = planes ? (forward ? p->fft2_fwd : p->fft2_inv) : (forward ? p->fft_fwd : p->fft_inv);
     if (cufftSetStream(h, s) != CUFFT_SUCCESS) return SE_ECUFFT;
     cufftResult r;
     if (p->precision == SE_FP64)
@@ -64,9 +67,17 @@ se_status run_fft(se_plan *p, bool forward, cudaStream_t s)
     return r == CUFFT_SUCCESS ? SE_OK : SE_ECUFFT;
 }
 
-se_status run_stage(se_plan *p, int stage, const void *x, const void *f, void *u, cudaStream_t s)
+// fused == true (se_eval and its siblings on plans with xf_ok): FFT = 2-D transforms of the x-planes, SCALE = K4x (transform
+// over x, K4, inverse transform over x in one kernel), IFFT = 2-D transforms back.  The staged interface keeps the 3-D
+// transforms and the stand-alone K4, so that the spectrum can be read between the stages.
+se_status run_stage(se_plan *p, int stage, const void *x, const void *f, void *u, cudaStream_t s, bool fused = false)
 {
     cudaError_t e = cudaSuccess;
+    if (fused && !p->slab) {
+        if (stage == SE_STAGE_FFT) return run_fft(p, true, s, true);
+        if (stage == SE_STAGE_IFFT) return run_fft(p, false, s, true);
+        if (stage == SE_STAGE_SCALE) return se_launch_xfft_scale(p, s) == cudaSuccess ? SE_OK : SE_ECUDA;
+    }
     switch (stage) {
     case SE_STAGE_SORT:
         if (!x || !f || (p->own_targets && !p->xt_stage)) return SE_EINVAL;
@@ -318,10 +329,33 @@ se_status se_plan_create_ex(se_plan **out, const se_plan_desc *d)
         free_all(p);
         return st;
     }
+    if (se_build_xfft(p) != cudaSuccess) {
+        cudaGetLastError();
+        free_all(p);
+        return SE_ECUDA;
+    }
+    if (p->xf_ok) {
+        // fused path: batch of 3 M out-of-place 2-D transforms over (y, z), one per x-plane and component
+        int n2[2] = {M, M};
+        r = cufftPlanMany(&p->fft2_fwd, 2, n2, nullptr, 1, (int)0, nullptr, 1, (int)0, tf, 3 * M);
+        if (r == CUFFT_SUCCESS) {
+            p->fft2_ok |= 1;
+            if (cufftGetSize(p->fft2_fwd, &wsz) == CUFFT_SUCCESS) p->fft_work_bytes += wsz;
+            r = cufftPlanMany(&p->fft2_inv, 2, n2, nullptr, 1, (int)0, nullptr, 1, (int)0, ti, 3 * M);
+        }
+        if (r == CUFFT_SUCCESS) {
+            p->fft2_ok |= 2;
+            if (cufftGetSize(p->fft2_inv, &wsz) == CUFFT_SUCCESS) p->fft_work_bytes += wsz;
+        } else {
+            se_status st = (r == CUFFT_ALLOC_FAILED) ? SE_ENOMEM : SE_ECUFFT;
+            free_all(p);
+            return st;
+        }
+    }
     p->workspace_bytes += p->fft_work_bytes;
 
     if (se_build_ktab(p) != cudaSuccess || se_build_wcoef(p) != cudaSuccess || se_build_mtab(p) != cudaSuccess ||
-        se_prepare_grid(p) != cudaSuccess) {
+        se_prepare_grid(p) != cudaSuccess || se_tune_xfft(p) != cudaSuccess) {
         cudaGetLastError();
         free_all(p);
         return SE_ECUDA;
@@ -383,6 +417,7 @@ se_status se_plan_info(const se_plan *p, se_info *o)
     o->grid_mode = g.grid_mode; o->nbins_total = g.nbins_total; o->nchunk = g.nchunk;
     o->nmodes = (int64_t)g.M * g.M * (g.M / 2 + 1);
     o->Mx = g.Mx; o->px0 = g.px0;
+    o->fft_fused = p->xf_ok;
     o->workspace_bytes = p->workspace_bytes;
     return SE_OK;
 }
@@ -394,16 +429,17 @@ static se_status run_all(se_plan *p, const void *x, const void *f, void *u, void
     p->ev_recorded = 0;
     const bool prof = p->profiling != 0;
     const bool fork = p->overlap != 0;
+    const bool fused = p->xf_ok != 0;
     if (prof && cudaEventRecord(p->ev[0], s) != cudaSuccess) return SE_ECUDA;
     for (int st = 0; st < SE_NSTAGES; ++st) {
         if (fork && st == SE_STAGE_P2P) {
             // deferred: launched on the side stream once K3 has been queued (below)
         } else if (fork && st == SE_STAGE_SUM) {
             if (cudaStreamWaitEvent(s, p->ev_join, 0) != cudaSuccess) return SE_ECUDA;
-            se_status r = run_stage(p, st, x, f, u, s);
+            se_status r = run_stage(p, st, x, f, u, s, fused);
             if (r != SE_OK) return r;
         } else {
-            se_status r = run_stage(p, st, x, f, u, s);
+            se_status r = run_stage(p, st, x, f, u, s, fused);
             if (r != SE_OK) return r;
         }
         if (fork && st == SE_STAGE_P2G) {

@@ -114,6 +114,13 @@ struct se_plan {
     double *mtab;                  // K2 function tables (se_p2p.cu): erfcx pieces + exp polynomial, always double
     cufftHandle fft_fwd, fft_inv;
     int fft_ok;
+    // fused x-transform + K4 (se_scale.cu, K4x): se_eval runs cuFFT 2-D over (y, z) per x-plane, k_xfft_scale, cuFFT 2-D back
+    cufftHandle fft2_fwd, fft2_inv;
+    int fft2_ok;
+    int xf_ok, xf_tz, xf_nst, xf_radix[12], xf_threads, xf_r16;
+    unsigned xf_magic[12];
+    void *xf_tw;                   // [M] complex Real: w_M^t
+    int *xf_xk;                    // [M] x-index of the mode at position p after the forward stages
     size_t fft_work_bytes;
     // host-buffer entry point staging
     void *hx, *hf, *hu;            // device staging [N][3] Real each
@@ -132,6 +139,9 @@ cudaError_t se_launch_sort(se_plan *p, const void *x, const void *f, const void 
 cudaError_t se_launch_p2p(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_p2g(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_scale(se_plan *p, cudaStream_t s);
+cudaError_t se_build_xfft(se_plan *p);       // se_scale.cu: decides p->xf_ok, builds the tables of the fused x-transform
+cudaError_t se_launch_xfft_scale(se_plan *p, cudaStream_t s);
+cudaError_t se_tune_xfft(se_plan *p);        // se_scale.cu: times the block shapes of K4x once (end of plan creation)
 cudaError_t se_launch_g2p(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_sum(se_plan *p, const void *f, void *u, cudaStream_t s);
 cudaError_t se_build_ktab(se_plan *p);      // se_window.cu: k values and the deconvolution factor per 1-D index

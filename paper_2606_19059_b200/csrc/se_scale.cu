@@ -8,6 +8,11 @@
 // mode of the R2C half-spectrum (conjugate symmetry).  The exponential factors
 // as a product of three 1-D tables built once per plan, so the kernel is pure HBM streaming:
 // 3 complex in, 3 complex out per mode.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
 #include "se_common.cuh"
 
 namespace {
@@ -15,6 +20,24 @@ namespace {
 template <typename Real> struct Cplx;
 template <> struct Cplx<double> { typedef double2 type; };
 template <> struct Cplx<float> { typedef float2 type; };
+
+// one mode of eq. (2.6): (h0, h1, h2) <- s(k) [k^2 h - k (k . h)]; e = e(k1) e(k2) e(k3) from the table
+template <typename Real, typename C>
+__device__ __forceinline__ void scale_mode(int M, int ix, int iy, int iz, Real kx, Real ky, Real kz, Real e, Real pref,
+                                           Real inv4xi2, C &h0, C &h1, C &h2)
+{
+    const Real k2 = kx * kx + ky * ky + kz * kz;
+    const bool nyq = (2 * ix == M) || (2 * iy == M) || (2 * iz == M);
+    Real s = 0;
+    if (!nyq && k2 > (Real)0) s = pref * ((Real)1 + k2 * inv4xi2) * e / (k2 * k2);
+    const Real kr = kx * h0.x + ky * h1.x + kz * h2.x;
+    const Real ki = kx * h0.y + ky * h1.y + kz * h2.y;
+    C o0, o1, o2;
+    o0.x = s * (k2 * h0.x - kx * kr); o0.y = s * (k2 * h0.y - kx * ki);
+    o1.x = s * (k2 * h1.x - ky * kr); o1.y = s * (k2 * h1.y - ky * ki);
+    o2.x = s * (k2 * h2.x - kz * kr); o2.y = s * (k2 * h2.y - kz * ki);
+    h0 = o0; h1 = o1; h2 = o2;
+}
 
 // ktab layout: [0..M) k value of index i, [M..2M) e(k_i)
 template <typename Real>
@@ -29,22 +52,397 @@ k_scale(int M, int Mh, int y0, int ny, Real pref, Real inv4xi2, const Real *__re
     if (iz >= Mh) return;
     const size_t nm = (size_t)M * ny * Mh;
     const size_t idx = ((size_t)ix * ny + blockIdx.y) * Mh + iz;
-    const Real kx = ktab[ix], ky = ktab[iy], kz = ktab[iz];
-    const Real k2 = kx * kx + ky * ky + kz * kz;
-    const bool nyq = (2 * ix == M) || (2 * iy == M) || (2 * iz == M);
-    Real s = 0;
-    if (!nyq && k2 > (Real)0) {
-        const Real e = ktab[M + ix] * ktab[M + iy] * ktab[M + iz];
-        s = pref * ((Real)1 + k2 * inv4xi2) * e / (k2 * k2);
-    }
     C h0 = spec[idx], h1 = spec[nm + idx], h2 = spec[2 * nm + idx];
-    const Real kr = kx * h0.x + ky * h1.x + kz * h2.x;
-    const Real ki = kx * h0.y + ky * h1.y + kz * h2.y;
-    C o0, o1, o2;
-    o0.x = s * (k2 * h0.x - kx * kr); o0.y = s * (k2 * h0.y - kx * ki);
-    o1.x = s * (k2 * h1.x - ky * kr); o1.y = s * (k2 * h1.y - ky * ki);
-    o2.x = s * (k2 * h2.x - kz * kr); o2.y = s * (k2 * h2.y - kz * ki);
-    spec[idx] = o0; spec[nm + idx] = o1; spec[2 * nm + idx] = o2;
+    scale_mode<Real>(M, ix, iy, iz, ktab[ix], ktab[iy], ktab[iz], ktab[M + ix] * ktab[M + iy] * ktab[M + iz], pref, inv4xi2, h0, h1, h2);
+    spec[idx] = h0; spec[nm + idx] = h1; spec[2 * nm + idx] = h2;
+}
+
+
+// ================================================================================================================
+// K4x: the transform over x, K4 and the inverse transform over x in ONE kernel (se_eval's path when the plan's
+// `xf_ok` is set).  A 3-D transform is a 2-D transform over (y, z) of every x-plane followed by 1-D transforms
+// over x; K4 is diagonal in k, and the 1-D transforms over x of different (ky, kz) are independent.  So
+//   H --cuFFT 2-D R2C, batch 3 M--> [this kernel] --cuFFT 2-D C2R, batch 3 M--> H~
+// where a block of this kernel owns TZ consecutive kz of one ky for all three components (K4 mixes the
+// components, eq. (2.6)): it loads the 3 TZ x-columns (length M, stride M (M/2+1)) into shared memory
+// with 16-byte asynchronous copies, runs them through an in-place mixed-radix decimation-in-frequency transform
+// (radices 16, 9, 8, 7, 5, 4, 3, 2 in registers, twiddles from a shared table), applies K4 in the digit-reversed
+// order the transform leaves (index table per plan), runs the mirror-image decimation-in-time inverse (which
+// takes that order and returns the natural one, unnormalised like cuFFT's) and writes the columns back in place.
+// Against cuFFT's third pass + k_scale + cuFFT's first inverse pass that is one read and one write of the
+// half-spectrum instead of three of each; the arithmetic is the same.  HBM-bound: 2 x 16 (8) bytes per mode.
+// Layout in shared memory: element x of column f (= component * TZ + tz) at [x][f], so that the threads of a
+// quarter-warp touch 128 contiguous bytes whatever the stride of the stage.
+__constant__ double c_cs[17][16][2];      // (cos, sin)(2 pi j / R) for R <= 16, j < R
+__constant__ float c_csf[17][16][2];
+
+template <typename Real> struct XfT;
+template <> struct XfT<double> {
+    typedef double2 C;
+    static __device__ __forceinline__ double cs(int R, int j, int k) { return c_cs[R][j][k]; }
+};
+template <> struct XfT<float> {
+    typedef float2 C;
+    static __device__ __forceinline__ float cs(int R, int j, int k) { return c_csf[R][j][k]; }
+};
+
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { C r; r.x = a.x + b.x; r.y = a.y + b.y; return r; }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { C r; r.x = a.x - b.x; r.y = a.y - b.y; return r; }
+// a * (wr + i wi)
+template <typename C, typename Real> __device__ __forceinline__ C cmulw(C a, Real wr, Real wi)
+{
+    C r;
+    r.x = fma(-a.y, wi, a.x * wr);
+    r.y = fma(a.y, wr, a.x * wi);
+    return r;
+}
+
+template <typename Real, int R, bool INV> struct Dft;
+
+template <typename Real, bool INV> struct Dft<Real, 2, INV> {
+    typedef typename XfT<Real>::C C;
+    static __device__ __forceinline__ void run(C (&v)[2])
+    {
+        const C a = cadd(v[0], v[1]), b = csub(v[0], v[1]);
+        v[0] = a; v[1] = b;
+    }
+};
+template <typename Real, bool INV> struct Dft<Real, 4, INV> {
+    typedef typename XfT<Real>::C C;
+    static __device__ __forceinline__ void run(C (&v)[4])
+    {
+        const C a = cadd(v[0], v[2]), b = csub(v[0], v[2]), c = cadd(v[1], v[3]), d = csub(v[1], v[3]);
+        C md;                                   // -i d (forward), +i d (inverse)
+        md.x = INV ? -d.y : d.y; md.y = INV ? d.x : -d.x;
+        v[0] = cadd(a, c); v[1] = cadd(b, md); v[2] = csub(a, c); v[3] = csub(b, md);
+    }
+};
+// odd prime R: X_p = v0 + sum_q cos(2 pi p q / R) (v_q + v_{R-q}) -/+ i sum_q sin(2 pi p q / R) (v_q - v_{R-q})
+template <typename Real, int R, bool INV> struct DftPrime {
+    typedef typename XfT<Real>::C C;
+    static __device__ __forceinline__ void run(C (&v)[R])
+    {
+        constexpr int H = (R - 1) / 2;
+        C s[H + 1], d[H + 1];
+#pragma unroll
+        for (int q = 1; q <= H; ++q) { s[q] = cadd(v[q], v[R - q]); d[q] = csub(v[q], v[R - q]); }
+        const C x0 = v[0];
+        C sum = x0;
+#pragma unroll
+        for (int q = 1; q <= H; ++q) sum = cadd(sum, s[q]);
+#pragma unroll
+        for (int p = 1; p <= H; ++p) {
+            Real ar = x0.x, ai = x0.y, br = (Real)0, bi = (Real)0;
+#pragma unroll
+            for (int q = 1; q <= H; ++q) {
+                const Real cj = XfT<Real>::cs(R, (p * q) % R, 0), sj = XfT<Real>::cs(R, (p * q) % R, 1);
+                ar = fma(cj, s[q].x, ar); ai = fma(cj, s[q].y, ai);
+                br = fma(sj, d[q].x, br); bi = fma(sj, d[q].y, bi);
+            }
+            C lo, hi;                           // a - i b, a + i b
+            lo.x = ar + bi; lo.y = ai - br; hi.x = ar - bi; hi.y = ai + br;
+            v[p] = INV ? hi : lo; v[R - p] = INV ? lo : hi;
+        }
+        v[0] = sum;
+    }
+};
+template <typename Real, bool INV> struct Dft<Real, 3, INV> : DftPrime<Real, 3, INV> {};
+template <typename Real, bool INV> struct Dft<Real, 5, INV> : DftPrime<Real, 5, INV> {};
+template <typename Real, bool INV> struct Dft<Real, 7, INV> : DftPrime<Real, 7, INV> {};
+// R = A B in registers: n = n1 + A n2, k = B k1 + k2:  X[B k1 + k2] = sum_n1 w_A^{n1 k1} w_R^{n1 k2} sum_n2 x[n1 + A n2] w_B^{n2 k2}
+template <typename Real, int A, int B, bool INV> struct DftCT {
+    typedef typename XfT<Real>::C C;
+    static __device__ __forceinline__ void run(C (&v)[A * B])
+    {
+        constexpr int R = A * B;
+        C t[A][B];
+#pragma unroll
+        for (int n1 = 0; n1 < A; ++n1) {
+            C u[B];
+#pragma unroll
+            for (int n2 = 0; n2 < B; ++n2) u[n2] = v[n1 + A * n2];
+            Dft<Real, B, INV>::run(u);
+#pragma unroll
+            for (int k2 = 0; k2 < B; ++k2) {
+                const int j = n1 * k2;
+                if (j == 0) t[n1][k2] = u[k2];
+                else t[n1][k2] = cmulw(u[k2], XfT<Real>::cs(R, j, 0), INV ? XfT<Real>::cs(R, j, 1) : -XfT<Real>::cs(R, j, 1));
+            }
+        }
+#pragma unroll
+        for (int k2 = 0; k2 < B; ++k2) {
+            C u[A];
+#pragma unroll
+            for (int n1 = 0; n1 < A; ++n1) u[n1] = t[n1][k2];
+            Dft<Real, A, INV>::run(u);
+#pragma unroll
+            for (int k1 = 0; k1 < A; ++k1) v[B * k1 + k2] = u[k1];
+        }
+    }
+};
+template <typename Real, bool INV> struct Dft<Real, 8, INV> : DftCT<Real, 2, 4, INV> {};
+template <typename Real, bool INV> struct Dft<Real, 9, INV> : DftCT<Real, 3, 3, INV> {};
+template <typename Real, bool INV> struct Dft<Real, 16, INV> : DftCT<Real, 4, 4, INV> {};
+
+constexpr int XF_MAXST = 12;
+struct XfStages {
+    int nst;
+    int radix[XF_MAXST];
+    unsigned magic[XF_MAXST];      // ceil(2^32 / m), m = sub-transform length / radix of the stage (unused when m == 1)
+};
+
+// One in-place stage on this thread's column f: sub-transforms of length L = R m.  Forward (decimation in frequency):
+// R-point transform of x[b L + j + q m], q < R, times w_L^{j p}, written to the same places; inverse (decimation in
+// time): the same backwards.  GLOBAL: the forward stage reads its inputs from the spectrum in global memory instead
+// of shared memory, the inverse stage writes its outputs there (first / last stage of the kernel: no staging pass).
+template <typename Real, int R, bool INV, int NF, bool GLOBAL>
+__device__ __forceinline__ void xf_stage(typename XfT<Real>::C *sm, typename XfT<Real>::C *gcol, size_t gstride, bool gvalid,
+                                         const typename XfT<Real>::C *__restrict__ tw, int M, int L, unsigned magic, int w, int BW, int f)
+{
+    typedef typename XfT<Real>::C C;
+    const int m = L / R, tstep = M / L, nb = M / R;
+    for (int bf = w; bf < nb; bf += BW) {
+        const int b = m == 1 ? bf : (int)__umulhi((unsigned)bf, magic), j = bf - b * m;
+        const int e0 = b * L + j;
+        C v[R];
+        if (!INV && GLOBAL) {
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+                if (gvalid) v[q] = __ldcs(gcol + (size_t)(e0 + q * m) * gstride);
+                else { v[q].x = (Real)0; v[q].y = (Real)0; }
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < R; ++q) v[q] = sm[(e0 + q * m) * NF + f];
+        }
+        if (!INV) Dft<Real, R, false>::run(v);
+        if (j != 0) {
+#pragma unroll
+            for (int p = 1; p < R; ++p) {
+                const C t = __ldg(tw + tstep * j * p);            // w_L^{j p}, forward sign
+                v[p] = cmulw(v[p], t.x, INV ? -t.y : t.y);
+            }
+        }
+        if (INV) Dft<Real, R, true>::run(v);
+        if (INV && GLOBAL) {
+            if (gvalid) {
+#pragma unroll
+                for (int q = 0; q < R; ++q) __stcs(gcol + (size_t)(e0 + q * m) * gstride, v[q]);
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < R; ++q) sm[(e0 + q * m) * NF + f] = v[q];
+        }
+    }
+}
+
+template <typename Real, bool INV, int NF, bool GLOBAL, bool R16>
+__device__ __forceinline__ void xf_stage_any(int R, typename XfT<Real>::C *sm, typename XfT<Real>::C *gcol, size_t gstride, bool gvalid,
+                                             const typename XfT<Real>::C *__restrict__ tw, int M, int L, unsigned magic, int w, int BW, int f)
+{
+#define XF_CASE(RR) case RR: xf_stage<Real, RR, INV, NF, GLOBAL>(sm, gcol, gstride, gvalid, tw, M, L, magic, w, BW, f); break;
+    switch (R) {
+    case 16: if constexpr (R16) xf_stage<Real, 16, INV, NF, GLOBAL>(sm, gcol, gstride, gvalid, tw, M, L, magic, w, BW, f); break;
+        XF_CASE(9) XF_CASE(8) XF_CASE(7) XF_CASE(5) XF_CASE(4) XF_CASE(3)
+    default: xf_stage<Real, 2, INV, NF, GLOBAL>(sm, gcol, gstride, gvalid, tw, M, L, magic, w, BW, f); break;
+    }
+#undef XF_CASE
+}
+
+// The innermost stage (L = R: contiguous groups of R positions), K4 and the same stage of the inverse in registers, for
+// the three components of one kz at a time (K4 mixes the components): saves two passes over shared memory and the K4 pass.
+template <typename Real, int R, int TZ>
+__device__ __forceinline__ void xf_centre(typename XfT<Real>::C *sm, int M, int iy, int iz, bool valid, const Real *__restrict__ ktab,
+                                          const int *__restrict__ xk, Real pref, Real inv4xi2, int w, int BW, int tz)
+{
+    typedef typename XfT<Real>::C C;
+    constexpr int NF = 3 * TZ;
+    if (!valid) return;                                          // a kz beyond the half-spectrum (ragged last tile): zeros stay zeros
+    const Real ky = __ldg(ktab + iy), kz = __ldg(ktab + iz), ey = __ldg(ktab + M + iy), ez = __ldg(ktab + M + iz);
+    for (int bf = w; bf < M / R; bf += BW) {
+        C v[3][R];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+#pragma unroll
+            for (int q = 0; q < R; ++q) v[c][q] = sm[(bf * R + q) * NF + c * TZ + tz];
+            Dft<Real, R, false>::run(v[c]);
+        }
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            const int ix = __ldg(xk + bf * R + q);
+            scale_mode<Real>(M, ix, iy, iz, __ldg(ktab + ix), ky, kz, __ldg(ktab + M + ix) * ey * ez, pref, inv4xi2,     // (e_x e_y) e_z as in k_scale
+                             v[0][q], v[1][q], v[2][q]);
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            Dft<Real, R, true>::run(v[c]);
+#pragma unroll
+            for (int q = 0; q < R; ++q) sm[(bf * R + q) * NF + c * TZ + tz] = v[c][q];
+        }
+    }
+}
+
+// blockDim.x = NF * BW: thread (w, f) works on column f = component * TZ + tz, butterflies w, w + BW, ...
+template <int BYTES> __device__ __forceinline__ void cp_async(void *dst, const void *src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
+    if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src) : "memory");
+}
+
+#ifndef XF_MINB
+#define XF_MINB 2
+#endif
+template <typename Real, int TZ, bool R16>
+__global__ void __launch_bounds__(256, R16 ? 1 : XF_MINB)
+k_xfft_scale(int M, int Mh, XfStages xs, Real pref, Real inv4xi2, const Real *__restrict__ ktab, const int *__restrict__ xk,
+             const typename XfT<Real>::C *__restrict__ tw, typename XfT<Real>::C *__restrict__ spec)
+{
+    typedef typename XfT<Real>::C C;
+    constexpr int NF = 3 * TZ;
+    extern __shared__ __align__(16) unsigned char xf_raw[];
+    C *sm = reinterpret_cast<C *>(xf_raw);                 // [M][NF]
+    const int tid = threadIdx.x, NT = blockDim.x;
+    const int iy = blockIdx.y, iz0 = blockIdx.x * TZ;
+    const size_t plane = (size_t)M * Mh;
+    const int f = tid % NF, w = tid / NF, BW = NT / NF;
+    const int fc = f / TZ, ftz = f - fc * TZ;
+    const bool gvalid = iz0 + ftz < Mh;
+    C *gcol = spec + (size_t)fc * M * plane + (size_t)iy * Mh + iz0 + ftz;      // element x of this thread's column at + x * plane
+    const int nst = xs.nst;
+    const bool gfirst = nst >= 2;                          // the outermost inverse stage writes global memory directly
+
+    // all columns of the block by asynchronous 16-byte (fp32: 8-byte) copies: every load of the block is in flight at once,
+    // and the other blocks of the SM compute meanwhile
+    for (int ix = w; ix < M; ix += BW) {
+        if (gvalid) cp_async<sizeof(C)>(&sm[ix * NF + f], gcol + (size_t)ix * plane);
+        else { sm[ix * NF + f].x = (Real)0; sm[ix * NF + f].y = (Real)0; }
+    }
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();
+    int L = M;
+    for (int st = 0; st < nst - 1; ++st) {
+        xf_stage_any<Real, false, NF, false, R16>(xs.radix[st], sm, gcol, plane, gvalid, tw, M, L, xs.magic[st], w, BW, f);
+        L /= xs.radix[st];
+        __syncthreads();
+    }
+    {
+        // innermost stage (L == its radix), K4, and back
+        const int R = xs.radix[nst - 1];
+        const int tz = tid % TZ, w3 = tid / TZ, BW3 = NT / TZ;
+        const bool valid = iz0 + tz < Mh;
+        const int iz = min(iz0 + tz, Mh - 1);
+        if (R <= 5) {
+            switch (R) {
+            case 5: xf_centre<Real, 5, TZ>(sm, M, iy, iz, valid, ktab, xk, pref, inv4xi2, w3, BW3, tz); break;
+            case 4: xf_centre<Real, 4, TZ>(sm, M, iy, iz, valid, ktab, xk, pref, inv4xi2, w3, BW3, tz); break;
+            case 3: xf_centre<Real, 3, TZ>(sm, M, iy, iz, valid, ktab, xk, pref, inv4xi2, w3, BW3, tz); break;
+            default: xf_centre<Real, 2, TZ>(sm, M, iy, iz, valid, ktab, xk, pref, inv4xi2, w3, BW3, tz); break;
+            }
+        } else {
+            xf_stage_any<Real, false, NF, false, R16>(R, sm, gcol, plane, gvalid, tw, M, L, xs.magic[nst - 1], w, BW, f);
+            __syncthreads();
+            if (valid) {
+                const Real ky = __ldg(ktab + iy), kz = __ldg(ktab + iz);
+                for (int pos = w3; pos < M; pos += BW3) {
+                    const int ix = __ldg(xk + pos);
+                    C *q = sm + pos * NF + tz;
+                    scale_mode<Real>(M, ix, iy, iz, __ldg(ktab + ix), ky, kz, __ldg(ktab + M + ix) * __ldg(ktab + M + iy) * __ldg(ktab + M + iz),
+                                     pref, inv4xi2, q[0], q[TZ], q[2 * TZ]);
+                }
+            }
+            __syncthreads();
+            xf_stage_any<Real, true, NF, false, R16>(R, sm, gcol, plane, gvalid, tw, M, L, xs.magic[nst - 1], w, BW, f);
+        }
+        __syncthreads();
+    }
+    for (int st = nst - 2; st >= 0; --st) {
+        L *= xs.radix[st];
+        if (st == 0 && gfirst) xf_stage_any<Real, true, NF, true, R16>(xs.radix[st], sm, gcol, plane, gvalid, tw, M, L, xs.magic[st], w, BW, f);
+        else xf_stage_any<Real, true, NF, false, R16>(xs.radix[st], sm, gcol, plane, gvalid, tw, M, L, xs.magic[st], w, BW, f);
+        if (st > 0) __syncthreads();
+    }
+    if (!gfirst) {
+        __syncthreads();
+        for (int ix = w; ix < M; ix += BW)
+            if (gvalid) gcol[(size_t)ix * plane] = sm[ix * NF + f];
+    }
+}
+
+// radices of the x-transform; false if M has a prime factor > 7.  Large radices first (fewest passes over shared memory; the
+// first stage's loads come straight from global memory), the smallest last: a last radix <= 5 is merged with K4.
+bool xf_factor(int M, bool allow16, XfStages &xs)
+{
+    static const int pref[] = {16, 9, 8, 7, 5, 4, 3, 2};
+    xs.nst = 0;
+    int rem = M;
+    for (int r : pref) {
+        if (r == 16 && !allow16) continue;
+        while (rem % r == 0 && rem > 1) {
+            if (xs.nst == XF_MAXST) return false;
+            xs.radix[xs.nst++] = r;
+            rem /= r;
+        }
+    }
+    if (rem != 1 || M < 2) return false;
+    // a lone trailing 8 or 9 (e.g. 576 = 9 8 8, 64 = 8 8): split off a small last radix when that costs no extra pass over
+    // what the unmerged K4 would, i.e. 8 -> 4 2
+    if (xs.nst >= 1 && xs.radix[xs.nst - 1] == 8 && xs.nst < XF_MAXST) { xs.radix[xs.nst - 1] = 4; xs.radix[xs.nst++] = 2; }
+    int L = M;
+    for (int st = 0; st < xs.nst; ++st) {
+        const int m = L / xs.radix[st];
+        xs.magic[st] = m > 1 ? (unsigned)((0x100000000ull + (unsigned)m - 1) / (unsigned)m) : 0u;
+        L = m;
+    }
+    return true;
+}
+
+template <typename Real, int TZ> size_t xf_smem(int M) { return (size_t)M * (3 * TZ) * sizeof(typename XfT<Real>::C); }
+
+// threads: NF columns x BW butterfly lanes, BW chosen so that the stages' butterfly counts M / R split evenly
+template <int NF> int xf_threads(int M, const XfStages &xs)
+{
+    int best = 1;
+    double bc = 1e30;
+    for (int bw = 256 / NF; bw >= 4; --bw) {
+        double cost = 0;
+        for (int st = 0; st < xs.nst; ++st) {
+            const int nb = M / xs.radix[st];
+            cost += (double)((nb + bw - 1) / bw) * xs.radix[st];           // iterations x work per butterfly
+        }
+        cost *= 1.0 + 2.0 / bw;                                             // fewer threads: less latency hiding
+        if (cost < bc) { bc = cost; best = bw; }
+    }
+    return best * NF;
+}
+
+template <typename Real, int TZ, bool R16>
+cudaError_t xf_launch(se_plan *p, cudaStream_t s, bool prepare)
+{
+    typedef typename XfT<Real>::C C;
+    const SeGeom &g = p->g;
+    const int M = g.M, Mh = M / 2 + 1;
+    auto kern = k_xfft_scale<Real, TZ, R16>;
+    const size_t smem = xf_smem<Real, TZ>(M);
+    if (prepare) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    XfStages xs;
+    xs.nst = p->xf_nst;
+    for (int i = 0; i < XF_MAXST; ++i) { xs.radix[i] = i < p->xf_nst ? p->xf_radix[i] : 1; xs.magic[i] = i < p->xf_nst ? p->xf_magic[i] : 0u; }
+    const double M3 = (double)M * M * M;
+    dim3 grid((Mh + TZ - 1) / TZ, M);
+    kern<<<grid, p->xf_threads, smem, s>>>(M, Mh, xs, (Real)(8.0 * SE_PI / M3), (Real)(1.0 / (4.0 * g.xi * g.xi)), (const Real *)p->ktab,
+                                           p->xf_xk, (const C *)p->xf_tw, (C *)p->spec);
+    p->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t xf_dispatch(se_plan *p, cudaStream_t s, bool prepare)
+{
+    if (p->precision == SE_FP64) {
+        if (p->xf_r16) return p->xf_tz == 4 ? xf_launch<double, 4, true>(p, s, prepare) : xf_launch<double, 2, true>(p, s, prepare);
+        return p->xf_tz == 4 ? xf_launch<double, 4, false>(p, s, prepare) : xf_launch<double, 2, false>(p, s, prepare);
+    }
+    return p->xf_tz == 8 ? xf_launch<float, 8, true>(p, s, prepare) : xf_launch<float, 4, true>(p, s, prepare);
 }
 
 template <typename Real>
@@ -81,4 +479,121 @@ extern "C" se_status se_scale_block(se_plan *p, void *spec, int ky0, int nky, vo
     cudaError_t e = p->precision == SE_FP64 ? scale_impl<double>(p, spec, ky0, nky, (cudaStream_t)stream)
                                             : scale_impl<float>(p, spec, ky0, nky, (cudaStream_t)stream);
     return e == cudaSuccess ? SE_OK : SE_ECUDA;
+}
+
+// Decides whether the plan's se_eval takes the fused x-transform (M 7-smooth, the columns of a block fit in shared
+// memory, not switched off by SE_FFT_MODE=3d) and builds its tables: twiddles w_M^t in long double, the x-index of
+// every position after the forward stages (mixed-radix digit reversal), the small-transform constants.
+cudaError_t se_build_xfft(se_plan *p)
+{
+    p->xf_ok = 0;
+    if (p->slab) return cudaSuccess;
+    const char *mode = std::getenv("SE_FFT_MODE");
+    if (mode && std::strcmp(mode, "3d") == 0) return cudaSuccess;
+    const int M = p->g.M;
+    XfStages xs;
+    if (!xf_factor(M, false, xs)) return cudaSuccess;
+    // passes over shared memory (32 bytes per mode each): the outermost stage half a pass each way, the inner ones a
+    // whole pass each way, the innermost one pass merged with K4 or three (stage, K4, stage) unmerged
+    auto passes = [](const XfStages &x) { return 1 + 2 * (x.nst >= 2 ? x.nst - 2 : 0) + (x.radix[x.nst - 1] <= 5 ? 1 : 3); };
+    p->xf_r16 = p->precision == SE_FP32;
+    {
+        XfStages x16;
+        if (xf_factor(M, true, x16) && (p->precision == SE_FP32 ? passes(x16) <= passes(xs) : passes(x16) < passes(xs))) { xs = x16; p->xf_r16 = 1; }
+    }
+    const size_t lim = 227 * 1024;
+    if (p->precision == SE_FP64) {
+        if (xf_smem<double, 4>(M) <= lim) p->xf_tz = 4;
+        else if (xf_smem<double, 2>(M) <= lim) p->xf_tz = 2;
+        else return cudaSuccess;
+        p->xf_threads = p->xf_tz == 4 ? xf_threads<12>(M, xs) : xf_threads<6>(M, xs);
+    } else {
+        if (xf_smem<float, 8>(M) <= lim) p->xf_tz = 8;
+        else if (xf_smem<float, 4>(M) <= lim) p->xf_tz = 4;
+        else return cudaSuccess;
+        p->xf_threads = p->xf_tz == 8 ? xf_threads<24>(M, xs) : xf_threads<12>(M, xs);
+    }
+    if (const char *e = std::getenv("SE_XF_BW")) {                  // experiments: butterfly lanes per column
+        const int nf = 3 * p->xf_tz, bw = std::atoi(e);
+        if (bw >= 1 && bw * nf <= 256) p->xf_threads = bw * nf;
+    }
+    p->xf_nst = xs.nst;
+    for (int i = 0; i < xs.nst; ++i) { p->xf_radix[i] = xs.radix[i]; p->xf_magic[i] = xs.magic[i]; }
+    const long double PI = 3.14159265358979323846264338327950288L;
+    static double hcs[17][16][2];
+    static float hcsf[17][16][2];
+    for (int R = 1; R <= 16; ++R)
+        for (int j = 0; j < 16; ++j) {
+            const long double a = 2.0L * PI * (long double)(j % R) / (long double)R;
+            hcs[R][j][0] = (double)cosl(a); hcs[R][j][1] = (double)sinl(a);
+            hcsf[R][j][0] = (float)cosl(a); hcsf[R][j][1] = (float)sinl(a);
+        }
+    cudaError_t e = cudaMemcpyToSymbol(c_cs, hcs, sizeof(hcs));
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_csf, hcsf, sizeof(hcsf));
+    if (e != cudaSuccess) return e;
+    std::vector<int> xk(M);
+    for (int pos = 0; pos < M; ++pos) {
+        int rem = pos, L = M, k = 0, mult = 1;
+        for (int st = 0; st < xs.nst; ++st) {
+            const int r = xs.radix[st], m = L / r;
+            k += (rem / m) * mult;
+            rem %= m; mult *= r; L = m;
+        }
+        xk[pos] = k;
+    }
+    const size_t cb = p->precision == SE_FP64 ? sizeof(double2) : sizeof(float2);
+    if ((e = cudaMalloc(&p->xf_tw, (size_t)M * cb)) != cudaSuccess) return e;
+    if ((e = cudaMalloc((void **)&p->xf_xk, (size_t)M * sizeof(int))) != cudaSuccess) return e;
+    p->workspace_bytes += (size_t)M * (cb + sizeof(int));
+    if (p->precision == SE_FP64) {
+        std::vector<double2> tw(M);
+        for (int t = 0; t < M; ++t) { const long double a = 2.0L * PI * t / M; tw[t] = make_double2((double)cosl(a), (double)-sinl(a)); }
+        e = cudaMemcpy(p->xf_tw, tw.data(), (size_t)M * cb, cudaMemcpyHostToDevice);
+    } else {
+        std::vector<float2> tw(M);
+        for (int t = 0; t < M; ++t) { const long double a = 2.0L * PI * t / M; tw[t] = make_float2((float)cosl(a), (float)-sinl(a)); }
+        e = cudaMemcpy(p->xf_tw, tw.data(), (size_t)M * cb, cudaMemcpyHostToDevice);
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(p->xf_xk, xk.data(), (size_t)M * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = xf_dispatch(p, nullptr, true);
+    if (e == cudaSuccess) p->xf_ok = 1;
+    return e;
+}
+
+cudaError_t se_launch_xfft_scale(se_plan *p, cudaStream_t s) { return xf_dispatch(p, s, false); }
+
+// Block shape of K4x: NF columns x BW butterfly lanes.  How evenly the stages' butterfly counts M / R split over BW, how many
+// blocks fit an SM and how well they hide one another's loads depends on M in a way a formula did not capture (config 3:
+// 0.94 ms at BW = 12, 1.03-1.11 ms at BW = 14...21; config 5: 4.8 ms at BW = 10, 5.7-6.8 ms above), so the plan times the
+// candidates once on its own (still unused) spectrum buffer.  The result of the kernel does not depend on BW.
+cudaError_t se_tune_xfft(se_plan *p)
+{
+    if (!p->xf_ok || std::getenv("SE_XF_BW")) return cudaSuccess;
+    const int nf = 3 * p->xf_tz, M = p->g.M;
+    const size_t bytes = (size_t)3 * M * M * (M / 2 + 1) * 2 * p->real_bytes;
+    cudaError_t e = cudaMemset(p->spec, 0, bytes);
+    if (e != cudaSuccess) return e;
+    cudaEvent_t e0, e1;
+    if ((e = cudaEventCreate(&e0)) != cudaSuccess) return e;
+    if ((e = cudaEventCreate(&e1)) != cudaSuccess) { cudaEventDestroy(e0); return e; }
+    const int saved = p->launches;
+    int best = p->xf_threads;
+    float bt = 1e30f;
+    for (int bw = 256 / nf; bw >= 4 && e == cudaSuccess; --bw) {
+        p->xf_threads = bw * nf;
+        float ms = 1e30f;
+        for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {              // first launch of a shape: warm-up
+            cudaEventRecord(e0, nullptr);
+            e = xf_dispatch(p, nullptr, false);
+            cudaEventRecord(e1, nullptr);
+            if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+            float t = 0.f;
+            if (e == cudaSuccess && rep > 0 && cudaEventElapsedTime(&t, e0, e1) == cudaSuccess) ms = t < ms ? t : ms;
+        }
+        if (ms < bt) { bt = ms; best = bw * nf; }
+    }
+    p->xf_threads = best;
+    p->launches = saved;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    return e;
 }

@@ -112,8 +112,10 @@ def _targets_case(prec, window, P, M, N=4000, Nt=1777, seed=0):
         u2 = torch.empty_like(td)
         plan.stage("sum", u=u2)
         torch.cuda.synchronize()
-        if info.grid_mode == 2:                               # the tensor-core sweep is bit-reproducible
-            assert torch.equal(u2, ut)
+        if info.grid_mode == 2 and not info.fft_fused:        # the tensor-core sweep is bit-reproducible
+            assert torch.equal(u2, ut)                        # (fused plans: se_eval_targets and the stages transform in different orders)
+        elif info.fft_fused:                                  # two transform orders in the plan's precision
+            assert rel(u2.cpu().numpy(), ut.cpu().numpy()) < 0.1 * tol["u"]
         else:                                                 # generic G2P adds with atomics: same to rounding
             assert rel(u2.cpu().numpy(), ut.cpu().numpy()) < 1e-3 * tol["u"]
     return o
