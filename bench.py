@@ -4,7 +4,8 @@
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl b200|reference]
 
 A step = one pass of the whole hot path (K1 sort, K2 P2P, K3 P2G, cuFFT R2C, K4 scale, cuFFT C2R,
-K5 G2P, K6 sum: SURVEY.md §8(a)) over one synthetic batch.  Default workload: BASELINE.json
+K5 G2P, K6 sum: SURVEY.md §8(a)) over one synthetic batch; on plans with fft_fused (se.h) the transforms over x
+run inside the K4 kernel and cuFFT does the 2-D transforms of the x-planes.  Default workload: BASELINE.json
 configs[2] (N = 1,048,576 uniform, fp64, 9 digits), the configuration SURVEY.md §8(d) names as the
 fp64 headline that fits one GPU comfortably; `--config` selects another (1..5).
 Multi-GPU (`--gpus N` under torchrun): N independent replicas, no data-path collective
@@ -324,7 +325,7 @@ def bench_plan(ctx, cfg, steps, warmup, over, headline):
     dom = max(own, key=lambda s_: stage_ms[s_])
     roof = dict(per_stage[dom])
     roof["kernel"] = {"p2p": "k_p2p (K2)", "p2g": "k_mma<spread> (K3)", "g2p": "k_mma<gather> (K5)",
-                      "scale": "k_scale (K4)", "sort": "K1", "sum": "K6"}[dom]
+                      "scale": "k_xfft_scale (K4x)" if info.fft_fused else "k_scale (K4)", "sort": "K1", "sum": "K6"}[dom]
     total_stage = sum(stage_ms.values())
     res = {
         "workload": c.label + ("" if not over else f" [{window} window, P={P}]"),
@@ -346,6 +347,9 @@ def bench_plan(ctx, cfg, steps, warmup, over, headline):
             "gridding": ("FP64 tensor-core sweep (double records and accumulators%s)" %
                          (", float grid" if c.precision == "fp32" else "")) if info.grid_mode == 2
             else "generic tile kernel in the plan's precision",
+            "transforms": ("fft / ifft = cuFFT 2-D over (y, z) of every x-plane, scale = k_xfft_scale: transform over x + K4 + "
+                           "inverse transform over x in one kernel (se.h, fft_fused)") if info.fft_fused
+            else "fft / ifft = cuFFT 3-D, scale = k_scale (K4)",
             "parallelism": "replicas x%d" % world,
             "l2": "no explicit flush: every step streams the %.2f GB plan workspace (grid %.2f GB + spectrum %.2f GB), "
                   "far larger than the 126 MB L2" % (info.workspace_bytes / 1e9, 3 * B * c.M ** 3 / 1e9,

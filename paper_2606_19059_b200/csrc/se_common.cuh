@@ -120,7 +120,7 @@ struct se_plan {
     int xf_ok, xf_tz, xf_nst, xf_radix[12], xf_threads, xf_r16;
     unsigned xf_magic[12];
     void *xf_tw;                   // [M] complex Real: w_M^t
-    int *xf_xk;                    // [M] x-index of the mode at position p after the forward stages
+    void *xf_xk;                   // [M] complex Real: (k_x, e_x) of the mode at position p after the forward stages
     size_t fft_work_bytes;
     // host-buffer entry point staging
     void *hx, *hf, *hu;            // device staging [N][3] Real each
@@ -141,7 +141,7 @@ cudaError_t se_launch_p2g(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_scale(se_plan *p, cudaStream_t s);
 cudaError_t se_build_xfft(se_plan *p);       // se_scale.cu: decides p->xf_ok, builds the tables of the fused x-transform
 cudaError_t se_launch_xfft_scale(se_plan *p, cudaStream_t s);
-cudaError_t se_tune_xfft(se_plan *p);        // se_scale.cu: times the block shapes of K4x once (end of plan creation)
+cudaError_t se_tune_xfft(se_plan *p);        // se_scale.cu: K4x's mode table (after se_build_ktab) and its block shape, timed once
 cudaError_t se_launch_g2p(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_sum(se_plan *p, const void *f, void *u, cudaStream_t s);
 cudaError_t se_build_ktab(se_plan *p);      // se_window.cu: k values and the deconvolution factor per 1-D index

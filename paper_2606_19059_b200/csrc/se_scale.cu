@@ -39,6 +39,32 @@ __device__ __forceinline__ void scale_mode(int M, int ix, int iy, int iz, Real k
     h0 = o0; h1 = o1; h2 = o2;
 }
 
+// 1 / x for x > 0 finite, to rounding: hardware seed and two Newton steps (no IEEE division sequence)
+__device__ __forceinline__ double fast_rcp(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    y = fma(y, fma(-x, y, 1.0), y);
+    return fma(y, fma(-x, y, 1.0), y);
+}
+__device__ __forceinline__ float fast_rcp(float x) { return __frcp_rn(x); }
+
+// the same for K4x: the Nyquist planes are zeros of the table factor e (set by the caller), 1 / k^4 by fast_rcp
+template <typename Real, typename C>
+__device__ __forceinline__ void scale_mode_x(Real kx, Real ky, Real kz, Real e, Real pref, Real inv4xi2, C &h0, C &h1, C &h2)
+{
+    const Real k2 = kx * kx + ky * ky + kz * kz;
+    Real s = 0;
+    if (k2 > (Real)0) s = pref * ((Real)1 + k2 * inv4xi2) * e * fast_rcp(k2 * k2);
+    const Real kr = kx * h0.x + ky * h1.x + kz * h2.x;
+    const Real ki = kx * h0.y + ky * h1.y + kz * h2.y;
+    C o0, o1, o2;
+    o0.x = s * (k2 * h0.x - kx * kr); o0.y = s * (k2 * h0.y - kx * ki);
+    o1.x = s * (k2 * h1.x - ky * kr); o1.y = s * (k2 * h1.y - ky * ki);
+    o2.x = s * (k2 * h2.x - kz * kr); o2.y = s * (k2 * h2.y - kz * ki);
+    h0 = o0; h1 = o1; h2 = o2;
+}
+
 // ktab layout: [0..M) k value of index i, [M..2M) e(k_i)
 template <typename Real>
 __global__ void __launch_bounds__(256)
@@ -252,14 +278,16 @@ __device__ __forceinline__ void xf_stage_any(int R, typename XfT<Real>::C *sm, t
 // The innermost stage (L = R: contiguous groups of R positions), K4 and the same stage of the inverse in registers, for
 // the three components of one kz at a time (K4 mixes the components): saves two passes over shared memory and the K4 pass.
 template <typename Real, int R, int TZ>
-__device__ __forceinline__ void xf_centre(typename XfT<Real>::C *sm, int M, int iy, int iz, bool valid, const Real *__restrict__ ktab,
-                                          const int *__restrict__ xk, Real pref, Real inv4xi2, int w, int BW, int tz)
+__device__ __forceinline__ void xf_centre(typename XfT<Real>::C *sm, int M, Real ky, Real kz, Real eyz, bool valid,
+                                          const typename XfT<Real>::C *__restrict__ xkk, Real pref, Real inv4xi2, int w, int BW, int tz)
 {
     typedef typename XfT<Real>::C C;
     constexpr int NF = 3 * TZ;
     if (!valid) return;                                          // a kz beyond the half-spectrum (ragged last tile): zeros stay zeros
-    const Real ky = __ldg(ktab + iy), kz = __ldg(ktab + iz), ey = __ldg(ktab + M + iy), ez = __ldg(ktab + M + iz);
     for (int bf = w; bf < M / R; bf += BW) {
+        C kk[R];                                                 // (k_x, e_x) of the R positions: loads in flight during the transforms
+#pragma unroll
+        for (int q = 0; q < R; ++q) kk[q] = __ldg(xkk + bf * R + q);
         C v[3][R];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -268,11 +296,7 @@ __device__ __forceinline__ void xf_centre(typename XfT<Real>::C *sm, int M, int 
             Dft<Real, R, false>::run(v[c]);
         }
 #pragma unroll
-        for (int q = 0; q < R; ++q) {
-            const int ix = __ldg(xk + bf * R + q);
-            scale_mode<Real>(M, ix, iy, iz, __ldg(ktab + ix), ky, kz, __ldg(ktab + M + ix) * ey * ez, pref, inv4xi2,     // (e_x e_y) e_z as in k_scale
-                             v[0][q], v[1][q], v[2][q]);
-        }
+        for (int q = 0; q < R; ++q) scale_mode_x<Real>(kk[q].x, ky, kz, kk[q].y * eyz, pref, inv4xi2, v[0][q], v[1][q], v[2][q]);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             Dft<Real, R, true>::run(v[c]);
@@ -295,8 +319,9 @@ template <int BYTES> __device__ __forceinline__ void cp_async(void *dst, const v
 #endif
 template <typename Real, int TZ, bool R16>
 __global__ void __launch_bounds__(256, R16 ? 1 : XF_MINB)
-k_xfft_scale(int M, int Mh, XfStages xs, Real pref, Real inv4xi2, const Real *__restrict__ ktab, const int *__restrict__ xk,
-             const typename XfT<Real>::C *__restrict__ tw, typename XfT<Real>::C *__restrict__ spec)
+k_xfft_scale(int M, int Mh, XfStages xs, Real pref, Real inv4xi2, const Real *__restrict__ ktab,
+             const typename XfT<Real>::C *__restrict__ xkk, const typename XfT<Real>::C *__restrict__ tw,
+             typename XfT<Real>::C *__restrict__ spec)
 {
     typedef typename XfT<Real>::C C;
     constexpr int NF = 3 * TZ;
@@ -332,23 +357,24 @@ k_xfft_scale(int M, int Mh, XfStages xs, Real pref, Real inv4xi2, const Real *__
         const int tz = tid % TZ, w3 = tid / TZ, BW3 = NT / TZ;
         const bool valid = iz0 + tz < Mh;
         const int iz = min(iz0 + tz, Mh - 1);
+        // k_y, k_z and e_y e_z of this thread's modes; zero on the Nyquist planes (reading S8), like e_x in the table
+        const Real ky = __ldg(ktab + iy), kz = __ldg(ktab + iz);
+        const Real eyz = (2 * iy == M || 2 * iz == M) ? (Real)0 : __ldg(ktab + M + iy) * __ldg(ktab + M + iz);
         if (R <= 5) {
             switch (R) {
-            case 5: xf_centre<Real, 5, TZ>(sm, M, iy, iz, valid, ktab, xk, pref, inv4xi2, w3, BW3, tz); break;
-            case 4: xf_centre<Real, 4, TZ>(sm, M, iy, iz, valid, ktab, xk, pref, inv4xi2, w3, BW3, tz); break;
-            case 3: xf_centre<Real, 3, TZ>(sm, M, iy, iz, valid, ktab, xk, pref, inv4xi2, w3, BW3, tz); break;
-            default: xf_centre<Real, 2, TZ>(sm, M, iy, iz, valid, ktab, xk, pref, inv4xi2, w3, BW3, tz); break;
+            case 5: xf_centre<Real, 5, TZ>(sm, M, ky, kz, eyz, valid, xkk, pref, inv4xi2, w3, BW3, tz); break;
+            case 4: xf_centre<Real, 4, TZ>(sm, M, ky, kz, eyz, valid, xkk, pref, inv4xi2, w3, BW3, tz); break;
+            case 3: xf_centre<Real, 3, TZ>(sm, M, ky, kz, eyz, valid, xkk, pref, inv4xi2, w3, BW3, tz); break;
+            default: xf_centre<Real, 2, TZ>(sm, M, ky, kz, eyz, valid, xkk, pref, inv4xi2, w3, BW3, tz); break;
             }
         } else {
             xf_stage_any<Real, false, NF, false, R16>(R, sm, gcol, plane, gvalid, tw, M, L, xs.magic[nst - 1], w, BW, f);
             __syncthreads();
             if (valid) {
-                const Real ky = __ldg(ktab + iy), kz = __ldg(ktab + iz);
                 for (int pos = w3; pos < M; pos += BW3) {
-                    const int ix = __ldg(xk + pos);
+                    const C kk = __ldg(xkk + pos);
                     C *q = sm + pos * NF + tz;
-                    scale_mode<Real>(M, ix, iy, iz, __ldg(ktab + ix), ky, kz, __ldg(ktab + M + ix) * __ldg(ktab + M + iy) * __ldg(ktab + M + iz),
-                                     pref, inv4xi2, q[0], q[TZ], q[2 * TZ]);
+                    scale_mode_x<Real>(kk.x, ky, kz, kk.y * eyz, pref, inv4xi2, q[0], q[TZ], q[2 * TZ]);
                 }
             }
             __syncthreads();
@@ -431,7 +457,7 @@ cudaError_t xf_launch(se_plan *p, cudaStream_t s, bool prepare)
     const double M3 = (double)M * M * M;
     dim3 grid((Mh + TZ - 1) / TZ, M);
     kern<<<grid, p->xf_threads, smem, s>>>(M, Mh, xs, (Real)(8.0 * SE_PI / M3), (Real)(1.0 / (4.0 * g.xi * g.xi)), (const Real *)p->ktab,
-                                           p->xf_xk, (const C *)p->xf_tw, (C *)p->spec);
+                                           (const C *)p->xf_xk, (const C *)p->xf_tw, (C *)p->spec);
     p->launches += 1;
     return cudaGetLastError();
 }
@@ -531,20 +557,10 @@ cudaError_t se_build_xfft(se_plan *p)
     cudaError_t e = cudaMemcpyToSymbol(c_cs, hcs, sizeof(hcs));
     if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_csf, hcsf, sizeof(hcsf));
     if (e != cudaSuccess) return e;
-    std::vector<int> xk(M);
-    for (int pos = 0; pos < M; ++pos) {
-        int rem = pos, L = M, k = 0, mult = 1;
-        for (int st = 0; st < xs.nst; ++st) {
-            const int r = xs.radix[st], m = L / r;
-            k += (rem / m) * mult;
-            rem %= m; mult *= r; L = m;
-        }
-        xk[pos] = k;
-    }
     const size_t cb = p->precision == SE_FP64 ? sizeof(double2) : sizeof(float2);
     if ((e = cudaMalloc(&p->xf_tw, (size_t)M * cb)) != cudaSuccess) return e;
-    if ((e = cudaMalloc((void **)&p->xf_xk, (size_t)M * sizeof(int))) != cudaSuccess) return e;
-    p->workspace_bytes += (size_t)M * (cb + sizeof(int));
+    if ((e = cudaMalloc(&p->xf_xk, (size_t)M * cb)) != cudaSuccess) return e;
+    p->workspace_bytes += (size_t)M * 2 * cb;
     if (p->precision == SE_FP64) {
         std::vector<double2> tw(M);
         for (int t = 0; t < M; ++t) { const long double a = 2.0L * PI * t / M; tw[t] = make_double2((double)cosl(a), (double)-sinl(a)); }
@@ -554,7 +570,6 @@ cudaError_t se_build_xfft(se_plan *p)
         for (int t = 0; t < M; ++t) { const long double a = 2.0L * PI * t / M; tw[t] = make_float2((float)cosl(a), (float)-sinl(a)); }
         e = cudaMemcpy(p->xf_tw, tw.data(), (size_t)M * cb, cudaMemcpyHostToDevice);
     }
-    if (e == cudaSuccess) e = cudaMemcpy(p->xf_xk, xk.data(), (size_t)M * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = xf_dispatch(p, nullptr, true);
     if (e == cudaSuccess) p->xf_ok = 1;
     return e;
@@ -566,12 +581,37 @@ cudaError_t se_launch_xfft_scale(se_plan *p, cudaStream_t s) { return xf_dispatc
 // blocks fit an SM and how well they hide one another's loads depends on M in a way a formula did not capture (config 3:
 // 0.94 ms at BW = 12, 1.03-1.11 ms at BW = 14...21; config 5: 4.8 ms at BW = 10, 5.7-6.8 ms above), so the plan times the
 // candidates once on its own (still unused) spectrum buffer.  The result of the kernel does not depend on BW.
+template <typename Real, typename C>
+cudaError_t xf_build_xkk(se_plan *p)
+{
+    // (k_x, e_x) of the mode at every position after the forward stages (mixed-radix digit reversal of the x-index), from the
+    // plan's K4 table; e_x = 0 on the Nyquist plane (reading S8)
+    const int M = p->g.M;
+    std::vector<Real> kt(2 * (size_t)M);
+    cudaError_t e = cudaMemcpy(kt.data(), p->ktab, kt.size() * sizeof(Real), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return e;
+    std::vector<C> tab(M);
+    for (int pos = 0; pos < M; ++pos) {
+        int rem = pos, L = M, k = 0, mult = 1;
+        for (int st = 0; st < p->xf_nst; ++st) {
+            const int r = p->xf_radix[st], m = L / r;
+            k += (rem / m) * mult;
+            rem %= m; mult *= r; L = m;
+        }
+        tab[pos].x = kt[k];
+        tab[pos].y = 2 * k == M ? (Real)0 : kt[M + k];
+    }
+    return cudaMemcpy(p->xf_xk, tab.data(), (size_t)M * sizeof(C), cudaMemcpyHostToDevice);
+}
+
 cudaError_t se_tune_xfft(se_plan *p)
 {
-    if (!p->xf_ok || std::getenv("SE_XF_BW")) return cudaSuccess;
+    if (!p->xf_ok) return cudaSuccess;
+    cudaError_t e = p->precision == SE_FP64 ? xf_build_xkk<double, double2>(p) : xf_build_xkk<float, float2>(p);
+    if (e != cudaSuccess || std::getenv("SE_XF_BW")) return e;
     const int nf = 3 * p->xf_tz, M = p->g.M;
     const size_t bytes = (size_t)3 * M * M * (M / 2 + 1) * 2 * p->real_bytes;
-    cudaError_t e = cudaMemset(p->spec, 0, bytes);
+    e = cudaMemset(p->spec, 0, bytes);
     if (e != cudaSuccess) return e;
     cudaEvent_t e0, e1;
     if ((e = cudaEventCreate(&e0)) != cudaSuccess) return e;
