@@ -31,7 +31,9 @@
  *     rounding order): SE_GRID_MODE = tile (force the generic gridding kernel; default: the FP64 tensor-core
  *     sweep for fp64 plans with even 4 <= P <= 24 and fp32 plans with even 4 <= P <= 16, else the generic tile kernel),
  *     SE_NCHUNK and SE_NCHUNK_G2P (x-chunks of K3 / K5), SE_OVERLAP = 1 (K2 on a side stream next to the FFT
- *     stages).
+ *     stages), SE_FFT_MODE = 3d (se_eval with the 3-D transforms and the stand-alone K4 instead of the fused path, see
+ *     the stages below), SE_XF_BW = n (block shape of the fused kernel: n lanes per column, instead of timing the
+ *     candidates at plan creation).
  */
 #ifndef SE_B200_H
 #define SE_B200_H
@@ -125,6 +127,8 @@ typedef struct {
     int Mx, px0;         /* planes of the plan's grid along x (M unless a slab plan) and global index of plane 0 */
     int fft_fused;       /* 1: se_eval / se_eval_targets / se_eval_host run the transform over x, K4 and the inverse transform
                             over x as one kernel between cuFFT 2-D transforms of the x-planes (see SE_STAGE_SCALE below) */
+    int fft_threads;     /* fused plans: threads per block of that kernel (timed once at plan creation; SE_XF_BW = lanes per
+                            column fixes it instead); 0 otherwise */
 } se_info;
 
 /* Everything se_plan_create takes, plus the window and an optional separate target count. */

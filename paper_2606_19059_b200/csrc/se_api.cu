@@ -418,6 +418,7 @@ se_status se_plan_info(const se_plan *p, se_info *o)
     o->nmodes = (int64_t)g.M * g.M * (g.M / 2 + 1);
     o->Mx = g.Mx; o->px0 = g.px0;
     o->fft_fused = p->xf_ok;
+    o->fft_threads = p->xf_ok ? p->xf_threads : 0;
     o->workspace_bytes = p->workspace_bytes;
     return SE_OK;
 }
