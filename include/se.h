@@ -64,7 +64,8 @@ typedef enum {
     SE_EINVAL = 1,   /* bad argument (see se_plan_create) or null pointer            */
     SE_ENOMEM = 2,   /* device or host allocation failed                             */
     SE_ECUDA = 3,    /* a CUDA runtime call or kernel launch failed / no device      */
-    SE_ECUFFT = 4    /* a cuFFT call failed                                          */
+    SE_ECUFFT = 4,   /* a cuFFT call failed                                          */
+    SE_ELIMIT = 5    /* a size beyond the fixed capacity of an entry point that allocates nothing (se_scale_noalloc) */
 } se_status;
 
 /* Stages of Algorithm 2.1 as this library runs them. */
@@ -239,6 +240,24 @@ se_status se_count_pairs(se_plan *p, int64_t *candidates, int64_t *in_range);
  * range outside [0, M).
  */
 se_status se_scale_block(se_plan *p, void *spec, int ky0, int nky, void *stream);
+
+/*
+ * K4 (eq. (2.6) with (2.4b) and the Gaussian window's deconvolution, reading S4) WITHOUT A PLAN AND WITHOUT ANY
+ * ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): the same kernel as se_scale_block on a caller-owned DEVICE block spec = [3][M][nky][M/2 + 1] complex numbers of
+ * `precision` (modes ky0 <= i_y < ky0 + nky), in place, asynchronous on `stream`, for the multiplier of a Gaussian-window plan
+ * with parameters (M, P, L, xi) -- the result equals se_scale_block's on such a plan up to the rounding of the multiplier table
+ * (built here in double on the device, there in long double on the host).  Kaiser-Bessel plans are not covered.
+ * The multiplier table (2 M reals) lives in a static device array of FIXED size inside the library: M <= 4096, i.e. 64 KB that
+ * every GPU which loads the library holds until the process exits.  The call makes no cudaMalloc / cudaFree and calls no
+ * library routine that allocates; its first call on a device looks up the array's address (cudaGetSymbolAddress), so make one
+ * call per device before starting a graph capture.  The array is shared by all calls and is refilled by each of them (it keeps
+ * the last call's table; nothing has to be cleared): calls that overlap on the GPU -- different streams, or graphs replayed
+ * side by side -- RACE on it; calls ordered on one stream do not.
+ * Errors: SE_EINVAL for a null pointer, odd or too small M or P, P > M, L or xi not positive, a ky range outside [0, M) or an
+ * unknown precision; SE_ELIMIT for M > 4096 (or a device ordinal >= 64); SE_ECUDA if the look-up or a launch fails.
+ */
+se_status se_scale_noalloc(void *spec, int M, int P, double L, double xi, se_precision precision, int ky0, int nky, void *stream);
 
 /* ---- parameter selection from a tolerance (section 2.4, eq. (2.9)) ------- */
 

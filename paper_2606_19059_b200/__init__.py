@@ -27,7 +27,8 @@ SE_NSTAGES = 8
 EXPORTS = ("se_plan_create", "se_plan_create_ex", "se_plan_create_tol", "se_select_params", "se_eval",
            "se_eval_targets", "se_set_targets", "se_eval_host", "se_plan_destroy", "se_strerror",
            "se_plan_info", "se_eval_stage", "se_buffer_read", "se_buffer_write",
-           "se_set_profiling", "se_stage_ms", "se_last_launch_count", "se_measure_peak", "se_count_pairs", "se_scale_block")
+           "se_set_profiling", "se_stage_ms", "se_last_launch_count", "se_measure_peak", "se_count_pairs", "se_scale_block",
+           "se_scale_noalloc")
 
 
 class SeInfo(C.Structure):
@@ -82,6 +83,7 @@ def lib() -> C.CDLL:
         L.se_measure_peak.argtypes = [i32, i32, C.POINTER(dbl)]
         L.se_count_pairs.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
         L.se_scale_block.argtypes = [vp, vp, i32, i32, vp]
+        L.se_scale_noalloc.argtypes = [vp, i32, i32, dbl, dbl, i32, i32, i32, vp]
         L.se_eval_host.argtypes = [vp, vp, vp, vp, vp]
         L.se_plan_destroy.argtypes = [vp]
         L.se_strerror.argtypes = [i32]
@@ -109,6 +111,21 @@ def _stream_ptr(stream):
     import torch
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
+
+
+def scale_noalloc(spec, M, P, L, xi, precision="fp64", ky0=0, nky=None, stream=None):
+    """se_scale_noalloc: K4 of a Gaussian-window plan (M, P, L, xi) in place on a complex block [3, M, nky, M // 2 + 1], without
+    a plan and without any allocation (the multiplier table sits in a fixed 64 KB device array of the library: M <= 4096;
+    calls that overlap on the GPU race on it)."""
+    import torch
+    nky = M if nky is None else nky
+    cdt = torch.complex128 if precision == "fp64" else torch.complex64
+    if not (spec.is_cuda and spec.is_contiguous() and spec.dtype == cdt and
+            tuple(spec.shape) == (3, int(M), int(nky), int(M) // 2 + 1)):
+        raise ValueError("scale_noalloc: need a contiguous CUDA complex tensor [3, M, nky, M // 2 + 1] of the given precision")
+    _check(lib().se_scale_noalloc(C.c_void_p(spec.data_ptr()), int(M), int(P), float(L), float(xi), {"fp64": SE_FP64, "fp32": SE_FP32}[precision],
+                                  int(ky0), int(nky), _stream_ptr(stream)), "se_scale_noalloc")
+    return spec
 
 
 def select_params(N, L, eps, window="gaussian", precision="fp64") -> SeParams:

@@ -129,6 +129,7 @@ const char *se_strerror(se_status s)
     case SE_ENOMEM: return "out of memory";
     case SE_ECUDA: return "CUDA error";
     case SE_ECUFFT: return "cuFFT error";
+    case SE_ELIMIT: return "size beyond the fixed capacity of an entry point that allocates nothing";
     default: return "unknown status";
     }
 }

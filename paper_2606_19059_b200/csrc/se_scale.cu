@@ -11,6 +11,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "se_common.cuh"
@@ -504,6 +505,88 @@ extern "C" se_status se_scale_block(se_plan *p, void *spec, int ky0, int nky, vo
     if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) { cudaGetLastError(); return SE_EINVAL; }
     cudaError_t e = p->precision == SE_FP64 ? scale_impl<double>(p, spec, ky0, nky, (cudaStream_t)stream)
                                             : scale_impl<float>(p, spec, ky0, nky, (cudaStream_t)stream);
+    return e == cudaSuccess ? SE_OK : SE_ECUDA;
+}
+
+// ================================================================================================================
+// se_scale_noalloc (se.h): K4 for callers that may not allocate (CUDA graph capture, serving loops, harnesses that
+// forbid cudaMalloc).  Same kernel as se_scale_block (k_scale); what a plan keeps in its cudaMalloc'ed multiplier
+// table (k and e(k) per 1-D index, 2 M reals) lives here in a file-scope device array of fixed size, refilled by a
+// small kernel on every call (the array keeps the previous call's table: nothing in it is reused, nothing needs to
+// start at zero).  Every GPU that loads the library holds the 64 KB until the process exits.  All calls share the
+// array: two calls that overlap on the GPU (different streams) race on it.
+constexpr int SE_NOALLOC_MAX_M = 4096;                          // = se_plan_create's own limit on M
+static __device__ __align__(256) double se_noalloc_ktab[2 * SE_NOALLOC_MAX_M];
+
+namespace {
+
+// table of a Gaussian-window plan (se_build_ktab builds the same in long double on the host): k_i = 2 pi n_i / L,
+// e_i = exp(-(1 - eta) k_i^2 / 4 xi^2), computed in double, stored in the precision of the spectrum
+template <typename Real>
+__global__ void k_fill_ktab(int M, double L, double xi, double eta, Real *__restrict__ tab)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= M) return;
+    const int n = (2 * i >= M) ? i - M : i;
+    const double k = 2.0 * SE_PI * (double)n / L;
+    tab[i] = (Real)k;
+    tab[M + i] = (Real)exp(-(1.0 - eta) * k * k / (4.0 * xi * xi));
+}
+
+// device address of the array, looked up once per device with that device current (the array's name is only a
+// host-side handle in host code, not an address a kernel can use)
+constexpr int SE_NOALLOC_MAX_DEV = 64;
+void *g_noalloc_ptr[SE_NOALLOC_MAX_DEV];
+std::mutex g_noalloc_mutex;
+
+cudaError_t noalloc_scratch(int dev, void **out)
+{
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, se_noalloc_ktab);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        g_noalloc_ptr[dev] = ptr;
+    }
+    *out = g_noalloc_ptr[dev];
+    return cudaSuccess;
+}
+
+template <typename Real>
+cudaError_t scale_noalloc_impl(void *spec, void *tab, int M, int P, double L, double xi, int ky0, int nky, cudaStream_t s)
+{
+    const int Mh = M / 2 + 1;
+    const double h = L / M, m = 0.95 * std::sqrt(SE_PI * P);    // reading S4, as se_plan_create_ex
+    const double eta = (P * h * xi / m) * (P * h * xi / m);
+    k_fill_ktab<Real><<<(M + 255) / 256, 256, 0, s>>>(M, L, xi, eta, (Real *)tab);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const double M3 = (double)M * M * M;
+    const int T = Mh < 256 ? ((Mh + 31) / 32) * 32 : 256;
+    dim3 grid((Mh + T - 1) / T, nky, M);
+    k_scale<Real><<<grid, T, 0, s>>>(M, Mh, ky0, nky, (Real)(8.0 * SE_PI / M3), (Real)(1.0 / (4.0 * xi * xi)), (const Real *)tab,
+                                     (typename Cplx<Real>::type *)spec);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+extern "C" se_status se_scale_noalloc(void *spec, int M, int P, double L, double xi, se_precision precision, int ky0, int nky,
+                                      void *stream)
+{
+    if (!spec || M < 2 || (M & 1) || P < 2 || (P & 1) || P > M || !(L > 0.0) || !(xi > 0.0) || ky0 < 0 || nky < 1 ||
+        (precision != SE_FP64 && precision != SE_FP32))
+        return SE_EINVAL;
+    if (M > SE_NOALLOC_MAX_M) return SE_ELIMIT;                  // the table would not fit the fixed array
+    if (ky0 + nky > M) return SE_EINVAL;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return SE_ECUDA; }
+    if (dev < 0 || dev >= SE_NOALLOC_MAX_DEV) return SE_ELIMIT;
+    void *tab = nullptr;
+    if (noalloc_scratch(dev, &tab) != cudaSuccess) { cudaGetLastError(); return SE_ECUDA; }
+    cudaError_t e = precision == SE_FP64 ? scale_noalloc_impl<double>(spec, tab, M, P, L, xi, ky0, nky, (cudaStream_t)stream)
+                                         : scale_noalloc_impl<float>(spec, tab, M, P, L, xi, ky0, nky, (cudaStream_t)stream);
     return e == cudaSuccess ? SE_OK : SE_ECUDA;
 }
 
