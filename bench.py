@@ -347,8 +347,9 @@ def bench_plan(ctx, cfg, steps, warmup, over, headline):
             "gridding": ("FP64 tensor-core sweep (double records and accumulators%s)" %
                          (", float grid" if c.precision == "fp32" else "")) if info.grid_mode == 2
             else "generic tile kernel in the plan's precision",
-            "transforms": ("fft / ifft = cuFFT 2-D over (y, z) of every x-plane, scale = k_xfft_scale: transform over x + K4 + "
-                           "inverse transform over x in one kernel (se.h, fft_fused), %d threads per block" % info.fft_threads) if info.fft_fused
+            "transforms": ("fft / ifft = %s 2-D over (y, z) of every x-plane, scale = k_xfft_scale: transform over x + K4 + "
+                           "inverse transform over x in one kernel (se.h, fft_fused), %d threads per block"
+                           % ("own (k_zr2c + k_yfft / k_yfft + k_zc2r)" if info.fft_planes_own else "cuFFT", info.fft_threads)) if info.fft_fused
             else "fft / ifft = cuFFT 3-D, scale = k_scale (K4)",
             "parallelism": "replicas x%d" % world,
             "l2": "no explicit flush: every step streams the %.2f GB plan workspace (grid %.2f GB + spectrum %.2f GB), "

@@ -32,7 +32,7 @@
  *     sweep for fp64 plans with even 4 <= P <= 24 and fp32 plans with even 4 <= P <= 16, else the generic tile kernel),
  *     SE_NCHUNK and SE_NCHUNK_G2P (x-chunks of K3 / K5), SE_OVERLAP = 1 (K2 on a side stream next to the FFT
  *     stages), SE_FFT_MODE = 3d (se_eval with the 3-D transforms and the stand-alone K4 instead of the fused path, see
- *     the stages below), SE_XF_BW = n (block shape of the fused kernel: n lanes per column, instead of timing the
+ *     the stages below) or cufft2d (fused path with cuFFT's 2-D transforms instead of the library's own), SE_XF_BW = n (block shape of the fused kernel: n lanes per column, instead of timing the
  *     candidates at plan creation).
  */
 #ifndef SE_B200_H
@@ -84,7 +84,8 @@ enum {
  * and se_eval_host run them FUSED when se_info.fft_fused is 1 (M has no prime factor above 7 and 3 x 4 (fp32: 3 x 8) columns
  * of M modes fit in shared memory; SE_FFT_MODE=3d at plan creation switches it off): stage 3 = cuFFT 2-D R2C over (y, z) of
  * every x-plane, stage 4 = ONE kernel that transforms over x, applies K4 and transforms back over x (a 3-D transform is the
- * 2-D transforms followed by 1-D transforms over x, and K4 is diagonal in k), stage 5 = cuFFT 2-D C2R.  The result H~ is the
+ * 2-D transforms followed by 1-D transforms over x, and K4 is diagonal in k), stage 5 = cuFFT 2-D C2R; with
+ * se_info.fft_planes_own the 2-D transforms are the library's own kernels as well (no cuFFT call in se_eval).  The result H~ is the
  * same up to rounding; SE_BUF_SPEC then holds the 2-D spectra, and se_stage_ms reports the three parts under the same names. */
 
 /* Internal buffers visible to tests and the benchmark through se_buffer_read/write. */
@@ -130,6 +131,9 @@ typedef struct {
                             over x as one kernel between cuFFT 2-D transforms of the x-planes (see SE_STAGE_SCALE below) */
     int fft_threads;     /* fused plans: threads per block of that kernel (timed once at plan creation; SE_XF_BW = lanes per
                             column fixes it instead); 0 otherwise */
+    int fft_planes_own;  /* fused plans: 1 if the 2-D transforms of the x-planes are the library's own kernels (a real-to-complex
+                            pass over z, a pass over y that leaves k_y in digit-reversed order for the fused kernel), 0 if
+                            cuFFT's (SE_FFT_MODE = cufft2d, or shapes the own kernels do not cover) */
 } se_info;
 
 /* Everything se_plan_create takes, plus the window and an optional separate target count. */

@@ -38,7 +38,7 @@ class SeInfo(C.Structure):
                 ("ncell", C.c_int), ("nbin", C.c_int), ("grid_mode", C.c_int), ("nbins_total", C.c_int),
                 ("nchunk", C.c_int), ("nmodes", C.c_int64),
                 ("workspace_bytes", C.c_size_t), ("Nt", C.c_int64), ("window", C.c_int), ("nu", C.c_int),
-                ("kb_beta", C.c_double), ("Mx", C.c_int), ("px0", C.c_int), ("fft_fused", C.c_int), ("fft_threads", C.c_int)]
+                ("kb_beta", C.c_double), ("Mx", C.c_int), ("px0", C.c_int), ("fft_fused", C.c_int), ("fft_threads", C.c_int), ("fft_planes_own", C.c_int)]
 
 
 class SePlanDesc(C.Structure):

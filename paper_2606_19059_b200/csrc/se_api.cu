@@ -37,7 +37,8 @@ void free_all(se_plan *p)
     };
     free_set(p->S);
     if (p->own_targets) free_set(p->T);
-    void *ptrs[] = {p->uN, p->uF, p->uFpart, p->grid, p->spec, p->ktab, p->mtab, p->wcoef, p->hx, p->hf, p->hu, p->xf_tw, p->xf_xk};
+    void *ptrs[] = {p->uN, p->uF, p->uFpart, p->grid, p->spec, p->ktab, p->mtab, p->wcoef, p->hx, p->hf, p->hu, p->xf_tw, p->xf_xk,
+                    p->f2_zpos, p->f2_ykk};
     for (void *q : ptrs) if (q) cudaFree(q);
     if (p->fft_ok & 1) cufftDestroy(p->fft_fwd);
     if (p->fft_ok & 2) cufftDestroy(p->fft_inv);
@@ -55,6 +56,7 @@ void free_all(se_plan *p)
 // planes == false: the 3-D transforms; planes == true: the 2-D transforms over (y, z) of every x-plane (fused path, K4x)
 se_status run_fft(se_plan *p, bool forward, cudaStream_t s, bool planes = false)
 {
+    if (planes && p->f2_ok) return se_launch_fft2(p, forward, s) == cudaSuccess ? SE_OK : SE_ECUDA;
     cufftHandle h = planes ? (forward ? p->fft2_fwd : p->fft2_inv) : (forward ? p->fft_fwd : p->fft_inv);
     if (cufftSetStream(h, s) != CUFFT_SUCCESS) return SE_ECUFFT;
     cufftResult r;
@@ -420,6 +422,7 @@ se_status se_plan_info(const se_plan *p, se_info *o)
     o->Mx = g.Mx; o->px0 = g.px0;
     o->fft_fused = p->xf_ok;
     o->fft_threads = p->xf_ok ? p->xf_threads : 0;
+    o->fft_planes_own = p->xf_ok && p->f2_ok;
     o->workspace_bytes = p->workspace_bytes;
     return SE_OK;
 }

@@ -121,6 +121,12 @@ struct se_plan {
     unsigned xf_magic[12];
     void *xf_tw;                   // [M] complex Real: w_M^t
     void *xf_xk;                   // [M] complex Real: (k_x, e_x) of the mode at position p after the forward stages
+    // own 2-D transforms of the x-planes (se_scale.cu k_zr2c / k_zc2r / k_yfft) instead of cuFFT's, when f2_ok
+    int f2_ok, f2_rb, f2_rbi, f2_rbmax, f2_rs, f2_zthreads, f2_zithreads, f2_ythreads;
+    int f2z_nst, f2z_radix[12], f2y_nst, f2y_radix[12];
+    unsigned f2z_magic[12], f2y_magic[12];
+    int *f2_zpos;                  // [M/2] position of frequency k after the forward stages of the M/2-point transform over z
+    void *f2_ykk;                  // [M] complex Real: (k_y, e_y) of the mode at position p of the second axis (digit-reversed)
     size_t fft_work_bytes;
     // host-buffer entry point staging
     void *hx, *hf, *hu;            // device staging [N][3] Real each
@@ -141,6 +147,7 @@ cudaError_t se_launch_p2g(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_scale(se_plan *p, cudaStream_t s);
 cudaError_t se_build_xfft(se_plan *p);       // se_scale.cu: decides p->xf_ok, builds the tables of the fused x-transform
 cudaError_t se_launch_xfft_scale(se_plan *p, cudaStream_t s);
+cudaError_t se_launch_fft2(se_plan *p, bool forward, cudaStream_t s);   // se_scale.cu: own 2-D transforms (p->f2_ok)
 cudaError_t se_tune_xfft(se_plan *p);        // se_scale.cu: K4x's mode table (after se_build_ktab) and its block shape, timed once
 cudaError_t se_launch_g2p(se_plan *p, cudaStream_t s);
 cudaError_t se_launch_sum(se_plan *p, const void *f, void *u, cudaStream_t s);

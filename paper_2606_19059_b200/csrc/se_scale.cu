@@ -220,9 +220,10 @@ struct XfStages {
 
 // One in-place stage on this thread's column f: sub-transforms of length L = R m.  Forward (decimation in frequency):
 // R-point transform of x[b L + j + q m], q < R, times w_L^{j p}, written to the same places; inverse (decimation in
-// time): the same backwards.  GLOBAL: the forward stage reads its inputs from the spectrum in global memory instead
-// of shared memory, the inverse stage writes its outputs there (first / last stage of the kernel: no staging pass).
-template <typename Real, int R, bool INV, int NF, bool GLOBAL>
+// time): the same backwards.  GLOBAL == 1: the forward stage reads its inputs from the spectrum in global memory instead
+// of shared memory, the inverse stage writes its outputs there (first / last stage of the kernel: no staging pass);
+// GLOBAL == 2: the stage writes its outputs to global memory whatever its direction.
+template <typename Real, int R, bool INV, int NF, int GLOBAL>
 __device__ __forceinline__ void xf_stage(typename XfT<Real>::C *sm, typename XfT<Real>::C *gcol, size_t gstride, bool gvalid,
                                          const typename XfT<Real>::C *__restrict__ tw, int M, int L, unsigned magic, int w, int BW, int f)
 {
@@ -232,7 +233,7 @@ __device__ __forceinline__ void xf_stage(typename XfT<Real>::C *sm, typename XfT
         const int b = m == 1 ? bf : (int)__umulhi((unsigned)bf, magic), j = bf - b * m;
         const int e0 = b * L + j;
         C v[R];
-        if (!INV && GLOBAL) {
+        if (!INV && GLOBAL == 1) {
 #pragma unroll
             for (int q = 0; q < R; ++q) {
                 if (gvalid) v[q] = __ldcs(gcol + (size_t)(e0 + q * m) * gstride);
@@ -251,7 +252,7 @@ __device__ __forceinline__ void xf_stage(typename XfT<Real>::C *sm, typename XfT
             }
         }
         if (INV) Dft<Real, R, true>::run(v);
-        if (INV && GLOBAL) {
+        if ((INV && GLOBAL == 1) || GLOBAL == 2) {
             if (gvalid) {
 #pragma unroll
                 for (int q = 0; q < R; ++q) __stcs(gcol + (size_t)(e0 + q * m) * gstride, v[q]);
@@ -263,7 +264,7 @@ __device__ __forceinline__ void xf_stage(typename XfT<Real>::C *sm, typename XfT
     }
 }
 
-template <typename Real, bool INV, int NF, bool GLOBAL, bool R16>
+template <typename Real, bool INV, int NF, int GLOBAL, bool R16>
 __device__ __forceinline__ void xf_stage_any(int R, typename XfT<Real>::C *sm, typename XfT<Real>::C *gcol, size_t gstride, bool gvalid,
                                              const typename XfT<Real>::C *__restrict__ tw, int M, int L, unsigned magic, int w, int BW, int f)
 {
@@ -321,9 +322,10 @@ template <int BYTES> __device__ __forceinline__ void cp_async(void *dst, const v
 template <typename Real, int TZ, bool R16>
 __global__ void __launch_bounds__(256, R16 ? 1 : XF_MINB)
 k_xfft_scale(int M, int Mh, XfStages xs, Real pref, Real inv4xi2, const Real *__restrict__ ktab,
-             const typename XfT<Real>::C *__restrict__ xkk, const typename XfT<Real>::C *__restrict__ tw,
-             typename XfT<Real>::C *__restrict__ spec)
+             const typename XfT<Real>::C *__restrict__ xkk, const typename XfT<Real>::C *__restrict__ ykk,
+             const typename XfT<Real>::C *__restrict__ tw, typename XfT<Real>::C *__restrict__ spec)
 {
+    // ykk != nullptr: the second axis of the spectrum is in the digit-reversed order k_yfft leaves, (k_y, e_y) per position
     typedef typename XfT<Real>::C C;
     constexpr int NF = 3 * TZ;
     extern __shared__ __align__(16) unsigned char xf_raw[];
@@ -359,8 +361,11 @@ k_xfft_scale(int M, int Mh, XfStages xs, Real pref, Real inv4xi2, const Real *__
         const bool valid = iz0 + tz < Mh;
         const int iz = min(iz0 + tz, Mh - 1);
         // k_y, k_z and e_y e_z of this thread's modes; zero on the Nyquist planes (reading S8), like e_x in the table
-        const Real ky = __ldg(ktab + iy), kz = __ldg(ktab + iz);
-        const Real eyz = (2 * iy == M || 2 * iz == M) ? (Real)0 : __ldg(ktab + M + iy) * __ldg(ktab + M + iz);
+        Real ky, ey;
+        if (ykk) { const C t = __ldg(ykk + iy); ky = t.x; ey = t.y; }
+        else { ky = __ldg(ktab + iy); ey = 2 * iy == M ? (Real)0 : __ldg(ktab + M + iy); }
+        const Real kz = __ldg(ktab + iz);
+        const Real eyz = 2 * iz == M ? (Real)0 : ey * __ldg(ktab + M + iz);
         if (R <= 5) {
             switch (R) {
             case 5: xf_centre<Real, 5, TZ>(sm, M, ky, kz, eyz, valid, xkk, pref, inv4xi2, w3, BW3, tz); break;
@@ -396,9 +401,202 @@ k_xfft_scale(int M, int Mh, XfStages xs, Real pref, Real inv4xi2, const Real *__
     }
 }
 
+// ================================================================================================================
+// Own 2-D transforms of the x-planes (the fused path's SE_STAGE_FFT / SE_STAGE_IFFT): a real-to-complex pass over z
+// with M/2-point complex transforms (k_zr2c / k_zc2r) and a complex pass over y (k_yfft), built from the same
+// register butterflies as K4x.  cuFFT's 2-D plan runs its pass over z at 2.3 TB/s (blocks of 60 threads); these
+// passes stream whole contiguous chunks of rows / 12 adjacent columns through shared memory.
+// The pass over y leaves the ky index in the digit-reversed order of its decimation-in-frequency stages (position p of
+// the second axis holds mode ky = rev(p)); K4x takes k_y and e_y from a table per position, and the inverse pass
+// (decimation in time) takes that order and returns the natural one.  Nothing else reads the spectrum on this path.
+
+// one in-place stage of a length-N transform on a column whose element `pos` is at col[pos] (shared memory);
+// twiddle w_N^t = tw[tws * t] (the plan's table of w_M^t, M = tws N)
+template <typename Real, int R, bool INV>
+__device__ __forceinline__ void zf_stage(typename XfT<Real>::C *col, const typename XfT<Real>::C *__restrict__ tw, int tws, int N,
+                                         int L, unsigned magic, int w, int BW)
+{
+    typedef typename XfT<Real>::C C;
+    const int m = L / R, tstep = (N / L) * tws, nb = N / R;
+    for (int bf = w; bf < nb; bf += BW) {
+        const int b = m == 1 ? bf : (int)__umulhi((unsigned)bf, magic), j = bf - b * m;
+        C *base = col + b * L + j;
+        C v[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = base[q * m];
+        if (!INV) Dft<Real, R, false>::run(v);
+        if (j != 0) {
+#pragma unroll
+            for (int p = 1; p < R; ++p) {
+                const C t = __ldg(tw + tstep * j * p);
+                v[p] = cmulw(v[p], t.x, INV ? -t.y : t.y);
+            }
+        }
+        if (INV) Dft<Real, R, true>::run(v);
+#pragma unroll
+        for (int q = 0; q < R; ++q) base[q * m] = v[q];
+    }
+}
+
+template <typename Real, bool INV, bool R16>
+__device__ __forceinline__ void zf_stage_any(int R, typename XfT<Real>::C *col, const typename XfT<Real>::C *__restrict__ tw, int tws,
+                                             int N, int L, unsigned magic, int w, int BW)
+{
+#define ZF_CASE(RR) case RR: zf_stage<Real, RR, INV>(col, tw, tws, N, L, magic, w, BW); break;
+    switch (R) {
+    case 16: if constexpr (R16) zf_stage<Real, 16, INV>(col, tw, tws, N, L, magic, w, BW); break;
+        ZF_CASE(9) ZF_CASE(8) ZF_CASE(7) ZF_CASE(5) ZF_CASE(4) ZF_CASE(3)
+    default: zf_stage<Real, 2, INV>(col, tw, tws, N, L, magic, w, BW); break;
+    }
+#undef ZF_CASE
+}
+
+// Real-to-complex over z.  A block takes RB consecutive rows (M reals each = N2 = M/2 complex numbers z_j = x_2j + i x_2j+1,
+// one contiguous chunk of the grid), row r at sm[r * RS ...] with RS = 1 mod 8 (16) complex numbers so that the RB lanes of
+// a butterfly step hit different banks; thread (w, f): row f, butterflies w, w + BW, ...  After the N2-point transform Z
+// (digit-reversed: Z_k at position zpos[k]):  X_k = E_k + w_M^k O_k, E_k = (Z_k + conj Z_{N2-k}) / 2, O_k = -i (Z_k - conj Z_{N2-k}) / 2,
+// k = 0 .. N2, written straight to the spectrum rows (M/2 + 1 complex numbers, again one contiguous chunk).
+template <typename Real, bool R16>
+__global__ void __launch_bounds__(256)
+k_zr2c(int M, int RS, int RB, long long nrows, XfStages xs, const typename XfT<Real>::C *__restrict__ tw, const int *__restrict__ zpos,
+       const Real *__restrict__ grid, typename XfT<Real>::C *__restrict__ spec)
+{
+    typedef typename XfT<Real>::C C;
+    extern __shared__ __align__(16) unsigned char xf_raw[];
+    C *sm = reinterpret_cast<C *>(xf_raw);
+    const int tid = threadIdx.x, NT = blockDim.x, N2 = M / 2, Mh = N2 + 1;
+    const long long row0 = (long long)blockIdx.x * RB;
+    const int nr = (int)min((long long)RB, nrows - row0);
+    const C *src = reinterpret_cast<const C *>(grid) + row0 * N2;
+    const unsigned mg = 0xffffffffu / (unsigned)N2 + 1u;                               // e / N2 for e < 2^16
+    for (int e = tid; e < nr * N2; e += NT) {
+        const int r = (int)__umulhi((unsigned)e, mg);
+        cp_async<sizeof(C)>(&sm[r * RS + (e - r * N2)], src + e);
+    }
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();
+    const int f = tid % RB, w = tid / RB, BW = NT / RB;
+    C *col = sm + f * RS;
+    int L = N2;
+    for (int st = 0; st < xs.nst; ++st) {
+        if (f < nr) zf_stage_any<Real, false, R16>(xs.radix[st], col, tw, 2, N2, L, xs.magic[st], w, BW);
+        L /= xs.radix[st];
+        __syncthreads();
+    }
+    // lanes run over the rows first (the same position of RB rows: conflict-free; consecutive k of one row sit 20 or more
+    // positions apart, i.e. in two bank groups), each row gets 32 / RB consecutive k of a warp
+    C *dst = spec + row0 * Mh + (long long)f * Mh;
+    for (int k = w; k < Mh && f < nr; k += BW) {
+        const int ka = k == N2 ? 0 : k, kb = k == 0 ? 0 : N2 - k;
+        const C a = col[__ldg(zpos + ka)], bq = col[__ldg(zpos + kb)];
+        // E = (a + conj b) / 2, O = -i (a - conj b) / 2
+        const Real er = (Real)0.5 * (a.x + bq.x), ei = (Real)0.5 * (a.y - bq.y);
+        const Real dr = (Real)0.5 * (a.x - bq.x), di = (Real)0.5 * (a.y + bq.y);      // (a - conj b) / 2
+        const Real orr = di, oi = -dr;                                                // times -i
+        const C t = __ldg(tw + k);                                                    // w_M^k
+        C o;
+        o.x = er + (orr * t.x - oi * t.y);
+        o.y = ei + (orr * t.y + oi * t.x);
+        dst[k] = o;
+    }
+}
+
+// Complex-to-real over z, unnormalised like cuFFT's: Z_k = E_k + i O_k with E_k = X_k + conj X_{N2-k}, O_k = (X_k - conj X_{N2-k}) w_M^{-k},
+// k = 0 .. N2 - 1 (the imaginary parts of X_0 and X_{N2} are ignored, as by cuFFT), placed at position zpos[k]; the inverse
+// (decimation-in-time) stages return z_j = x_2j + i x_2j+1 in natural order, i.e. the grid rows.
+template <typename Real, bool R16>
+__global__ void __launch_bounds__(256)
+k_zc2r(int M, int RS, int RB, long long nrows, XfStages xs, const typename XfT<Real>::C *__restrict__ tw, const int *__restrict__ zpos,
+       const typename XfT<Real>::C *__restrict__ spec, Real *__restrict__ grid)
+{
+    typedef typename XfT<Real>::C C;
+    extern __shared__ __align__(16) unsigned char xf_raw[];
+    C *sm = reinterpret_cast<C *>(xf_raw);
+    const int tid = threadIdx.x, NT = blockDim.x, N2 = M / 2, Mh = N2 + 1;
+    const long long row0 = (long long)blockIdx.x * RB;
+    const int nr = (int)min((long long)RB, nrows - row0);
+    const int f = tid % RB, w = tid / RB, BW = NT / RB;
+    C *col = sm + f * RS;
+    // lanes along k: coalesced loads of the spectrum rows (every entry is read twice, the second time from L1); the stores
+    // into the digit-reversed positions conflict two- to four-way, which measured cheaper than staging the rows in shared
+    // memory (half the blocks per SM) or loading with the lanes over the rows (64-byte pieces)
+    const C *src = spec + row0 * Mh;
+    const unsigned mg = 0xffffffffu / (unsigned)N2 + 1u;                               // e / N2 for e < 2^16
+    for (int e = tid; e < nr * N2; e += NT) {
+        const int r = (int)__umulhi((unsigned)e, mg), k = e - r * N2;
+        C a = __ldg(src + (long long)r * Mh + k), bq = __ldg(src + (long long)r * Mh + N2 - k);
+        if (k == 0) { a.y = (Real)0; bq.y = (Real)0; }
+        const Real er = a.x + bq.x, ei = a.y - bq.y;                                   // a + conj b
+        const Real dr = a.x - bq.x, di = a.y + bq.y;                                   // a - conj b
+        const C t = __ldg(tw + k);                                                     // w_M^k; O = d conj(t)
+        const Real orr = dr * t.x + di * t.y, oi = di * t.x - dr * t.y;
+        C z;
+        z.x = er - oi; z.y = ei + orr;                                                 // E + i O
+        sm[r * RS + __ldg(zpos + k)] = z;
+    }
+    __syncthreads();
+    int L = 1;
+    for (int st = xs.nst - 1; st >= 0; --st) {
+        L *= xs.radix[st];
+        if (f < nr) zf_stage_any<Real, true, R16>(xs.radix[st], col, tw, 2, N2, L, xs.magic[st], w, BW);
+        __syncthreads();
+    }
+    C *dst = reinterpret_cast<C *>(grid) + row0 * N2;
+    for (int e = tid; e < nr * N2; e += NT) {
+        const int r = (int)__umulhi((unsigned)e, mg);
+        dst[e] = sm[r * RS + (e - r * N2)];
+    }
+}
+
+// Complex transform over y of NF adjacent columns (consecutive kz, running on into the next x-plane), in place.
+// Forward: decimation in frequency, the result stays in digit-reversed order along y; inverse: decimation in time from
+// that order, the last stage writes global memory directly.
+#ifndef YF_MINB
+#define YF_MINB 3
+#endif
+template <typename Real, int NF, bool INV, bool R16>
+__global__ void __launch_bounds__(192, YF_MINB)
+k_yfft(int M, int Mh, long long ncols, XfStages xs, const typename XfT<Real>::C *__restrict__ tw, typename XfT<Real>::C *__restrict__ spec)
+{
+    typedef typename XfT<Real>::C C;
+    extern __shared__ __align__(16) unsigned char xf_raw[];
+    C *sm = reinterpret_cast<C *>(xf_raw);                 // [M][NF]
+    const int tid = threadIdx.x, NT = blockDim.x;
+    const int f = tid % NF, w = tid / NF, BW = NT / NF;
+    const long long q = (long long)blockIdx.x * NF + f;
+    const bool gvalid = q < ncols;
+    const long long pl = q / Mh;
+    C *gcol = spec + pl * (long long)M * Mh + (q - pl * Mh);
+    const size_t gstride = (size_t)Mh;
+    for (int iy = w; iy < M; iy += BW) {
+        if (gvalid) cp_async<sizeof(C)>(&sm[iy * NF + f], gcol + (size_t)iy * gstride);
+        else { sm[iy * NF + f].x = (Real)0; sm[iy * NF + f].y = (Real)0; }
+    }
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();
+    const int nst = xs.nst;
+    if (!INV) {
+        int L = M;
+        for (int st = 0; st < nst; ++st) {
+            if (st == nst - 1) xf_stage_any<Real, false, NF, 2, R16>(xs.radix[st], sm, gcol, gstride, gvalid, tw, M, L, xs.magic[st], w, BW, f);
+            else xf_stage_any<Real, false, NF, 0, R16>(xs.radix[st], sm, gcol, gstride, gvalid, tw, M, L, xs.magic[st], w, BW, f);
+            L /= xs.radix[st];
+            if (st < nst - 1) __syncthreads();
+        }
+    } else {
+        int L = 1;
+        for (int st = nst - 1; st >= 0; --st) {
+            L *= xs.radix[st];
+            if (st == 0) xf_stage_any<Real, true, NF, true, R16>(xs.radix[st], sm, gcol, gstride, gvalid, tw, M, L, xs.magic[st], w, BW, f);
+            else xf_stage_any<Real, true, NF, false, R16>(xs.radix[st], sm, gcol, gstride, gvalid, tw, M, L, xs.magic[st], w, BW, f);
+            if (st > 0) __syncthreads();
+        }
+    }
+}
+
 // radices of the x-transform; false if M has a prime factor > 7.  Large radices first (fewest passes over shared memory; the
 // first stage's loads come straight from global memory), the smallest last: a last radix <= 5 is merged with K4.
-bool xf_factor(int M, bool allow16, XfStages &xs)
+bool xf_factor(int M, bool allow16, XfStages &xs, bool split_last = true)
 {
     static const int pref[] = {16, 9, 8, 7, 5, 4, 3, 2};
     xs.nst = 0;
@@ -414,7 +612,7 @@ bool xf_factor(int M, bool allow16, XfStages &xs)
     if (rem != 1 || M < 2) return false;
     // a lone trailing 8 or 9 (e.g. 576 = 9 8 8, 64 = 8 8): split off a small last radix when that costs no extra pass over
     // what the unmerged K4 would, i.e. 8 -> 4 2
-    if (xs.nst >= 1 && xs.radix[xs.nst - 1] == 8 && xs.nst < XF_MAXST) { xs.radix[xs.nst - 1] = 4; xs.radix[xs.nst++] = 2; }
+    if (split_last && xs.nst >= 1 && xs.radix[xs.nst - 1] == 8 && xs.nst < XF_MAXST) { xs.radix[xs.nst - 1] = 4; xs.radix[xs.nst++] = 2; }
     int L = M;
     for (int st = 0; st < xs.nst; ++st) {
         const int m = L / xs.radix[st];
@@ -458,7 +656,8 @@ cudaError_t xf_launch(se_plan *p, cudaStream_t s, bool prepare)
     const double M3 = (double)M * M * M;
     dim3 grid((Mh + TZ - 1) / TZ, M);
     kern<<<grid, p->xf_threads, smem, s>>>(M, Mh, xs, (Real)(8.0 * SE_PI / M3), (Real)(1.0 / (4.0 * g.xi * g.xi)), (const Real *)p->ktab,
-                                           (const C *)p->xf_xk, (const C *)p->xf_tw, (C *)p->spec);
+                                           (const C *)p->xf_xk, (const C *)(p->f2_ok ? p->f2_ykk : nullptr), (const C *)p->xf_tw,
+                                           (C *)p->spec);
     p->launches += 1;
     return cudaGetLastError();
 }
@@ -660,6 +859,126 @@ cudaError_t se_build_xfft(se_plan *p)
 
 cudaError_t se_launch_xfft_scale(se_plan *p, cudaStream_t s) { return xf_dispatch(p, s, false); }
 
+namespace {
+
+// frequency held at position `pos` after the decimation-in-frequency stages of a length-N transform (mixed-radix digit reversal)
+int xf_rev(int pos, int N, int nst, const int *radix)
+{
+    int rem = pos, L = N, k = 0, mult = 1;
+    for (int st = 0; st < nst; ++st) {
+        const int r = radix[st], m = L / r;
+        k += (rem / m) * mult;
+        rem %= m; mult *= r; L = m;
+    }
+    return k;
+}
+
+XfStages f2_stages(const se_plan *p, bool z)
+{
+    XfStages xs;
+    xs.nst = z ? p->f2z_nst : p->f2y_nst;
+    for (int i = 0; i < XF_MAXST; ++i) {
+        xs.radix[i] = i < xs.nst ? (z ? p->f2z_radix[i] : p->f2y_radix[i]) : 1;
+        xs.magic[i] = i < xs.nst ? (z ? p->f2z_magic[i] : p->f2y_magic[i]) : 0u;
+    }
+    return xs;
+}
+
+// the own 2-D transforms of the x-planes (k_zr2c / k_zc2r over z, k_yfft over y); prepare: dynamic shared memory opt-in only
+template <typename Real, int NF, bool R16>
+cudaError_t fft2_impl(se_plan *p, bool forward, cudaStream_t s, bool prepare, int parts)
+{
+    typedef typename XfT<Real>::C C;
+    const int M = p->g.M, Mh = M / 2 + 1;
+    const size_t smz = (size_t)p->f2_rb * p->f2_rs * sizeof(C), smzi = (size_t)p->f2_rbi * p->f2_rs * sizeof(C), smy = (size_t)M * NF * sizeof(C);
+    if (prepare) {
+        const int smax = (int)((size_t)p->f2_rbmax * p->f2_rs * sizeof(C));
+        cudaError_t e = cudaFuncSetAttribute(k_zr2c<Real, R16>, cudaFuncAttributeMaxDynamicSharedMemorySize, smax);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_zc2r<Real, R16>, cudaFuncAttributeMaxDynamicSharedMemorySize, smax);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_yfft<Real, NF, false, R16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smy);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_yfft<Real, NF, true, R16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smy);
+        return e;
+    }
+    const long long nrows = 3LL * M * M, ncols = 3LL * M * Mh;
+    const unsigned gz = (unsigned)((nrows + p->f2_rb - 1) / p->f2_rb), gzi = (unsigned)((nrows + p->f2_rbi - 1) / p->f2_rbi), gy = (unsigned)((ncols + NF - 1) / NF);
+    const XfStages xz = f2_stages(p, true), xy = f2_stages(p, false);
+    const C *tw = (const C *)p->xf_tw;
+    // parts: 1 = the pass over z, 2 = the pass over y (the tuner times them one by one)
+    if (forward) {
+        if (parts & 1) k_zr2c<Real, R16><<<gz, p->f2_zthreads, smz, s>>>(M, p->f2_rs, p->f2_rb, nrows, xz, tw, p->f2_zpos, (const Real *)p->grid, (C *)p->spec);
+        if (parts & 2) k_yfft<Real, NF, false, R16><<<gy, p->f2_ythreads, smy, s>>>(M, Mh, ncols, xy, tw, (C *)p->spec);
+    } else {
+        if (parts & 2) k_yfft<Real, NF, true, R16><<<gy, p->f2_ythreads, smy, s>>>(M, Mh, ncols, xy, tw, (C *)p->spec);
+        if (parts & 1) k_zc2r<Real, R16><<<gzi, p->f2_zithreads, smzi, s>>>(M, p->f2_rs, p->f2_rbi, nrows, xz, tw, p->f2_zpos, (const C *)p->spec, (Real *)p->grid);
+    }
+    p->launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t fft2_dispatch(se_plan *p, bool forward, cudaStream_t s, bool prepare, int parts = 3)
+{
+    return p->precision == SE_FP64 ? fft2_impl<double, 12, false>(p, forward, s, prepare, parts)
+                                   : fft2_impl<float, 24, true>(p, forward, s, prepare, parts);
+}
+
+// decides p->f2_ok and builds the tables of the own 2-D transforms (after se_build_ktab: the k_y table comes from the plan's)
+template <typename Real, typename C>
+cudaError_t fft2_build(se_plan *p)
+{
+    p->f2_ok = 0;
+    const char *mode = std::getenv("SE_FFT_MODE");
+    if (!p->xf_ok || (mode && std::strcmp(mode, "cufft2d") == 0)) return cudaSuccess;
+    const int M = p->g.M, N2 = M / 2;
+    const bool r16 = p->precision == SE_FP32;
+    XfStages xz, xy;
+    if (N2 < 2 || !xf_factor(N2, r16, xz, false) || !xf_factor(M, r16, xy, false)) return cudaSuccess;
+    const int NF = p->precision == SE_FP64 ? 12 : 24;
+    if ((size_t)M * NF * sizeof(C) > 227 * 1024) return cudaSuccess;
+    // rows of the z-pass: stride = 1 mod 8 (fp32: 16) complex numbers, up to 16 rows in <= 100 KB (two blocks per SM)
+    const int al = p->precision == SE_FP64 ? 8 : 16;
+    int rs = N2 + 1;
+    while (rs % al != 1) ++rs;
+    const int rbmax = (int)std::min<size_t>(16, (size_t)113 * 1024 / ((size_t)rs * sizeof(C)));
+    p->f2_rbmax = rbmax;
+    int rb = std::min(8, rbmax);
+    if (const char *e = std::getenv("SE_F2_RB")) rb = std::max(1, std::min(std::atoi(e), rbmax));
+    if (rb < 4 && !std::getenv("SE_F2_RB")) return cudaSuccess;
+    int bwz = std::max(1, std::min(192 / rb, 16)), bwy = std::max(4, 192 / NF);
+    if (const char *e = std::getenv("SE_F2_BWZ")) bwz = std::max(1, std::min(std::atoi(e), 256 / rb));
+    if (const char *e = std::getenv("SE_F2_BWY")) bwy = std::max(1, std::min(std::atoi(e), 192 / NF));
+    int rbi = rb, bwzi = bwz;                                  // rows per block and lanes per row of the inverse pass over z
+    if (const char *e = std::getenv("SE_F2_RBI")) rbi = std::max(1, std::min(std::atoi(e), rbmax));
+    if (const char *e = std::getenv("SE_F2_BWZI")) bwzi = std::max(1, std::min(std::atoi(e), 256 / rbi));
+    p->f2_rbi = rbi; p->f2_zithreads = rbi * bwzi;
+    p->f2_rs = rs; p->f2_rb = rb; p->f2_zthreads = rb * bwz; p->f2_ythreads = NF * bwy;
+    p->f2z_nst = xz.nst; p->f2y_nst = xy.nst;
+    for (int i = 0; i < XF_MAXST; ++i) {
+        p->f2z_radix[i] = xz.radix[i]; p->f2z_magic[i] = xz.magic[i];
+        p->f2y_radix[i] = xy.radix[i]; p->f2y_magic[i] = xy.magic[i];
+    }
+    std::vector<int> zpos(N2);
+    for (int pos = 0; pos < N2; ++pos) zpos[xf_rev(pos, N2, xz.nst, xz.radix)] = pos;
+    std::vector<Real> kt(2 * (size_t)M);
+    cudaError_t e = cudaMemcpy(kt.data(), p->ktab, kt.size() * sizeof(Real), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return e;
+    std::vector<C> ykk(M);
+    for (int pos = 0; pos < M; ++pos) {
+        const int k = xf_rev(pos, M, xy.nst, xy.radix);
+        ykk[pos].x = kt[k];
+        ykk[pos].y = 2 * k == M ? (Real)0 : kt[M + k];
+    }
+    if ((e = cudaMalloc((void **)&p->f2_zpos, (size_t)N2 * sizeof(int))) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&p->f2_ykk, (size_t)M * sizeof(C))) != cudaSuccess) return e;
+    p->workspace_bytes += (size_t)N2 * sizeof(int) + (size_t)M * sizeof(C);
+    if ((e = cudaMemcpy(p->f2_zpos, zpos.data(), (size_t)N2 * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return e;
+    if ((e = cudaMemcpy(p->f2_ykk, ykk.data(), (size_t)M * sizeof(C), cudaMemcpyHostToDevice)) != cudaSuccess) return e;
+    if ((e = fft2_dispatch(p, true, nullptr, true)) != cudaSuccess) return e;
+    p->f2_ok = 1;
+    return cudaSuccess;
+}
+
+}  // namespace
+
 // Block shape of K4x: NF columns x BW butterfly lanes.  How evenly the stages' butterfly counts M / R split over BW, how many
 // blocks fit an SM and how well they hide one another's loads depends on M in a way a formula did not capture (config 3:
 // 0.94 ms at BW = 12, 1.03-1.11 ms at BW = 14...21; config 5: 4.8 ms at BW = 10, 5.7-6.8 ms above), so the plan times the
@@ -691,6 +1010,7 @@ cudaError_t se_tune_xfft(se_plan *p)
 {
     if (!p->xf_ok) return cudaSuccess;
     cudaError_t e = p->precision == SE_FP64 ? xf_build_xkk<double, double2>(p) : xf_build_xkk<float, float2>(p);
+    if (e == cudaSuccess) e = p->precision == SE_FP64 ? fft2_build<double, double2>(p) : fft2_build<float, float2>(p);
     if (e != cudaSuccess || std::getenv("SE_XF_BW")) return e;
     const int nf = 3 * p->xf_tz, M = p->g.M;
     const size_t bytes = (size_t)3 * M * M * (M / 2 + 1) * 2 * p->real_bytes;
@@ -716,7 +1036,52 @@ cudaError_t se_tune_xfft(se_plan *p)
         if (ms < bt) { bt = ms; best = bw * nf; }
     }
     p->xf_threads = best;
+    // the same for the own 2-D transforms: rows per block x lanes per row of the two passes over z, lanes per column of the
+    // pass over y (config 3 is fastest at 8 x 12, config 5 at 8 x 16, config 4 at 16 x 8)
+    const bool f2env = std::getenv("SE_F2_RB") || std::getenv("SE_F2_BWZ") || std::getenv("SE_F2_RBI") || std::getenv("SE_F2_BWZI") ||
+                       std::getenv("SE_F2_BWY");
+    if (p->f2_ok && !f2env && e == cudaSuccess) e = cudaMemset(p->grid, 0, (size_t)3 * M * M * M * p->real_bytes);
+    if (p->f2_ok && !f2env && e == cudaSuccess) {
+        auto time_it = [&](bool forward, int parts) -> float {
+            float ms = 1e30f;
+            for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {
+                cudaEventRecord(e0, nullptr);
+                e = fft2_dispatch(p, forward, nullptr, false, parts);
+                cudaEventRecord(e1, nullptr);
+                if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+                float t = 0.f;
+                if (e == cudaSuccess && rep > 0 && cudaEventElapsedTime(&t, e0, e1) == cudaSuccess) ms = t < ms ? t : ms;
+            }
+            return ms;
+        };
+        static const int cand[][2] = {{8, 8}, {8, 12}, {8, 16}, {16, 8}, {16, 12}, {4, 16}};
+        for (int inv = 0; inv < 2; ++inv) {
+            int brb = inv ? p->f2_rbi : p->f2_rb, bth = inv ? p->f2_zithreads : p->f2_zthreads;
+            float btz = 1e30f;
+            for (const auto &c : cand) {
+                if (c[0] > p->f2_rbmax) continue;
+                (inv ? p->f2_rbi : p->f2_rb) = c[0];
+                (inv ? p->f2_zithreads : p->f2_zthreads) = c[0] * c[1];
+                const float ms = time_it(!inv, 1);
+                if (ms < btz) { btz = ms; brb = c[0]; bth = c[0] * c[1]; }
+            }
+            (inv ? p->f2_rbi : p->f2_rb) = brb;
+            (inv ? p->f2_zithreads : p->f2_zthreads) = bth;
+        }
+        const int NFy = p->precision == SE_FP64 ? 12 : 24;
+        int bby = p->f2_ythreads;
+        float bty = 1e30f;
+        for (int bw = 192 / NFy; bw >= 4; bw -= (NFy == 12 ? 2 : 1)) {
+            p->f2_ythreads = bw * NFy;
+            const float ms = time_it(true, 2) + time_it(false, 2);
+            if (ms < bty) { bty = ms; bby = bw * NFy; }
+        }
+        p->f2_ythreads = bby;
+    }
     p->launches = saved;
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     return e;
 }
+
+// the fused path's SE_STAGE_FFT / SE_STAGE_IFFT when the plan has its own 2-D transforms (p->f2_ok)
+cudaError_t se_launch_fft2(se_plan *p, bool forward, cudaStream_t s) { return fft2_dispatch(p, forward, s, false); }

@@ -71,6 +71,26 @@ def test_kb_window_fused_fp64():
     gate("u", u, o["u"], TOL["fp64"]["u"])
 
 
+def test_own_and_cufft_plane_transforms_agree(monkeypatch):
+    """The library's own 2-D transforms of the x-planes (real-to-complex over z, digit-reversed pass over y) against cuFFT's in
+    the same fused path, fp64 and fp32, on a grid whose M / 2 needs three radices (M = 90: 45 = 9 x 5; M = 112: 56 = 8 x 7)."""
+    import paper_2606_19059_b200 as se
+    from dataclasses import replace
+    for base, M, tol in ((3, 90, 1e-14), (3, 112, 1e-14), (4, 96, 2e-6)):
+        c, x, f = W.scaled(base, 8000)
+        c = replace(c, M=M, P=8 if base == 4 else 12)
+        with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P, c.precision) as plan:
+            assert plan.info().fft_planes_own == 1
+        _, Ht1, u1 = eval_Ht(c, x, f)
+        monkeypatch.setenv("SE_FFT_MODE", "cufft2d")
+        with se.Plan(c.N, c.L, c.xi, c.rc, c.M, c.P, c.precision) as plan:
+            assert plan.info().fft_planes_own == 0 and plan.info().fft_fused == 1
+        _, Ht0, u0 = eval_Ht(c, x, f)
+        monkeypatch.delenv("SE_FFT_MODE")
+        gate(f"Ht own vs cuFFT planes, M = {M}", Ht1, Ht0, tol)
+        gate(f"u own vs cuFFT planes, M = {M}", u1, u0, tol)
+
+
 def test_fused_and_3d_paths_agree_and_fall_back(monkeypatch):
     """Same plan parameters through both paths: H~ agrees to rounding; a grid size with a prime factor above 7 (M = 52) and
     SE_FFT_MODE=3d take the 3-D transforms."""
