@@ -5,7 +5,7 @@
 
 A step = one pass of the whole hot path (K1 sort, K2 P2P, K3 P2G, cuFFT R2C, K4 scale, cuFFT C2R,
 K5 G2P, K6 sum: SURVEY.md §8(a)) over one synthetic batch; on plans with fft_fused (se.h) the transforms over x
-run inside the K4 kernel and cuFFT does the 2-D transforms of the x-planes.  Default workload: BASELINE.json
+run inside the K4 kernel and the 2-D transforms of the x-planes are the library's own kernels (fft_planes_own) or cuFFT's.  Default workload: BASELINE.json
 configs[2] (N = 1,048,576 uniform, fp64, 9 digits), the configuration SURVEY.md §8(d) names as the
 fp64 headline that fits one GPU comfortably; `--config` selects another (1..5).
 Multi-GPU (`--gpus N` under torchrun): N independent replicas, no data-path collective
