@@ -932,6 +932,20 @@ cudaError_t fft2_build(se_plan *p)
     const bool r16 = p->precision == SE_FP32;
     XfStages xz, xy;
     if (N2 < 2 || !xf_factor(N2, r16, xz, false) || !xf_factor(M, r16, xy, false)) return cudaSuccess;
+    {
+        // pass over z: the radix with the most factors of two first, so that consecutive k sit an odd (or less even) number of
+        // positions apart and k_zc2r's stores into the digit-reversed positions spread over the banks (config 5: ifft 5.05 -> 4.87 ms)
+        int best = 0;
+        auto twos = [](int r) { int c = 0; while (!(r & 1)) { r >>= 1; ++c; } return c; };
+        for (int i = 1; i < xz.nst; ++i) if (twos(xz.radix[i]) > twos(xz.radix[best])) best = i;
+        std::swap(xz.radix[0], xz.radix[best]);
+        int L = N2;
+        for (int st = 0; st < xz.nst; ++st) {
+            const int m = L / xz.radix[st];
+            xz.magic[st] = m > 1 ? (unsigned)((0x100000000ull + (unsigned)m - 1) / (unsigned)m) : 0u;
+            L = m;
+        }
+    }
     const int NF = p->precision == SE_FP64 ? 12 : 24;
     if ((size_t)M * NF * sizeof(C) > 227 * 1024) return cudaSuccess;
     // rows of the z-pass: stride = 1 mod 8 (fp32: 16) complex numbers, up to 16 rows in <= 100 KB (two blocks per SM)
