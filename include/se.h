@@ -86,7 +86,9 @@ enum {
  * every x-plane, stage 4 = ONE kernel that transforms over x, applies K4 and transforms back over x (a 3-D transform is the
  * 2-D transforms followed by 1-D transforms over x, and K4 is diagonal in k), stage 5 = cuFFT 2-D C2R; with
  * se_info.fft_planes_own the 2-D transforms are the library's own kernels as well (no cuFFT call in se_eval).  The result H~ is the
- * same up to rounding; SE_BUF_SPEC then holds the 2-D spectra, and se_stage_ms reports the three parts under the same names. */
+ * same up to rounding; SE_BUF_SPEC then holds the 2-D spectra of the planes (with fft_planes_own: their second axis in the
+ * digit-reversed order of the library's transform over y -- an internal order, read the spectrum through the staged interface
+ * instead), and se_stage_ms reports the three parts under the same names. */
 
 /* Internal buffers visible to tests and the benchmark through se_buffer_read/write. */
 enum {
