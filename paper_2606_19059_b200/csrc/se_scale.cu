@@ -8,6 +8,9 @@
 // mode of the R2C half-spectrum (conjugate symmetry).  The exponential factors
 // as a product of three 1-D tables built once per plan, so the kernel is pure HBM streaming:
 // 3 complex in, 3 complex out per mode.
+// Also in this file, for se_eval's fused path ("Own 2-D transforms"): k_xfft_scale (transform over x + K4 +
+// inverse transform over x in one kernel), k_zr2c / k_zc2r / k_yfft (the 2-D transforms of the x-planes), and
+// se_scale_noalloc (K4 without a plan or an allocation, table in a static device array).
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -89,7 +92,7 @@ k_scale(int M, int Mh, int y0, int ny, Real pref, Real inv4xi2, const Real *__re
 // K4x: the transform over x, K4 and the inverse transform over x in ONE kernel (se_eval's path when the plan's
 // `xf_ok` is set).  A 3-D transform is a 2-D transform over (y, z) of every x-plane followed by 1-D transforms
 // over x; K4 is diagonal in k, and the 1-D transforms over x of different (ky, kz) are independent.  So
-//   H --cuFFT 2-D R2C, batch 3 M--> [this kernel] --cuFFT 2-D C2R, batch 3 M--> H~
+//   H --2-D R2C of every x-plane--> [this kernel] --2-D C2R of every x-plane--> H~      (own kernels below, or cuFFT batch 3 M)
 // where a block of this kernel owns TZ consecutive kz of one ky for all three components (K4 mixes the
 // components, eq. (2.6)): it loads the 3 TZ x-columns (length M, stride M (M/2+1)) into shared memory
 // with 16-byte asynchronous copies, runs them through an in-place mixed-radix decimation-in-frequency transform
