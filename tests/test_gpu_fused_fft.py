@@ -91,6 +91,42 @@ def test_own_and_cufft_plane_transforms_agree(monkeypatch):
         gate(f"u own vs cuFFT planes, M = {M}", u1, u0, tol)
 
 
+@pytest.mark.parametrize("prec,tol", [("fp64", 2e-14), ("fp32", 3e-6)])
+def test_fused_path_every_smooth_grid_size_up_to_130(prec, tol, monkeypatch):
+    """Every even grid size without a prime factor above 7 from 8 to 130 (all radix orders of the transforms over x, y and the
+    half-length transform over z, ragged last blocks of rows and columns): u of se_eval on the fused path with the library's own
+    plane transforms against the same library on cuFFT's 3-D transforms.  (Against the oracle: the tests above.)"""
+    import torch
+    import paper_2606_19059_b200 as se
+
+    def smooth7(n):
+        for q in (2, 3, 5, 7):
+            while n % q == 0:
+                n //= q
+        return n == 1
+
+    rng = np.random.default_rng(5)
+    N, P = 1500, 8
+    dt = torch.float64 if prec == "fp64" else torch.float32
+    xd = torch.as_tensor(rng.random((N, 3)), dtype=dt).cuda()
+    fd = torch.as_tensor(rng.standard_normal((N, 3)), dtype=dt).cuda()
+    sizes = [m for m in range(8, 131, 2) if smooth7(m)]
+    assert len(sizes) > 30
+    for M in sizes:
+        xi = 0.8 * 0.95 * np.sqrt(np.pi * P) * M / P
+        rc = min(0.3, 3.2 / xi)
+        u = {}
+        for mode in ("own", "3d"):
+            if mode == "3d":
+                monkeypatch.setenv("SE_FFT_MODE", "3d")
+            with se.Plan(N, 1.0, xi, rc, M, P, prec) as plan:
+                i = plan.info()
+                assert (i.fft_fused, i.fft_planes_own) == ((1, 1) if mode == "own" else (0, 0)), (M, mode)
+                u[mode] = plan.eval(xd, fd).double().cpu().numpy()
+            monkeypatch.delenv("SE_FFT_MODE", raising=False)
+        gate(f"u fused vs 3-D, M = {M}", u["own"], u["3d"], tol)
+
+
 def test_fused_and_3d_paths_agree_and_fall_back(monkeypatch):
     """Same plan parameters through both paths: H~ agrees to rounding; a grid size with a prime factor above 7 (M = 52) and
     SE_FFT_MODE=3d take the 3-D transforms."""
