@@ -408,7 +408,7 @@ k_xfft_scale(int M, int Mh, XfStages xs, Real pref, Real inv4xi2, const Real *__
 // Own 2-D transforms of the x-planes (the fused path's SE_STAGE_FFT / SE_STAGE_IFFT): a real-to-complex pass over z
 // with M/2-point complex transforms (k_zr2c / k_zc2r) and a complex pass over y (k_yfft), built from the same
 // register butterflies as K4x.  cuFFT's 2-D plan runs its pass over z at 2.3 TB/s (blocks of 60 threads); these
-// passes stream whole contiguous chunks of rows / 8 (fp32: 24) adjacent columns through shared memory.
+// passes stream whole contiguous chunks of rows / 8 (fp32: 16) adjacent columns through shared memory.
 // The pass over y leaves the ky index in the digit-reversed order of its decimation-in-frequency stages (position p of
 // the second axis holds mode ky = rev(p)); K4x takes k_y and e_y from a table per position, and the inverse pass
 // (decimation in time) takes that order and returns the natural one.  Nothing else reads the spectrum on this path.
@@ -556,6 +556,9 @@ k_zc2r(int M, int RS, int RB, long long nrows, XfStages xs, const typename XfT<R
 // that order, the last stage writes global memory directly.
 #ifndef YF_MINB
 #define YF_MINB 3
+#endif
+#ifndef SE_YF_NF32
+#define SE_YF_NF32 16      /* columns per block of k_yfft in fp32 plans */
 #endif
 #ifndef SE_YF_NF64
 #define SE_YF_NF64 8      /* columns per block of k_yfft in fp64 plans */
@@ -924,7 +927,7 @@ cudaError_t fft2_impl(se_plan *p, bool forward, cudaStream_t s, bool prepare, in
 cudaError_t fft2_dispatch(se_plan *p, bool forward, cudaStream_t s, bool prepare, int parts = 3)
 {
     return p->precision == SE_FP64 ? fft2_impl<double, SE_YF_NF64, false>(p, forward, s, prepare, parts)
-                                   : fft2_impl<float, 24, true>(p, forward, s, prepare, parts);
+                                   : fft2_impl<float, SE_YF_NF32, true>(p, forward, s, prepare, parts);
 }
 
 // decides p->f2_ok and builds the tables of the own 2-D transforms (after se_build_ktab: the k_y table comes from the plan's)
@@ -952,7 +955,7 @@ cudaError_t fft2_build(se_plan *p)
             L = m;
         }
     }
-    const int NF = p->precision == SE_FP64 ? SE_YF_NF64 : 24;
+    const int NF = p->precision == SE_FP64 ? SE_YF_NF64 : SE_YF_NF32;
     if ((size_t)M * NF * sizeof(C) > 227 * 1024) return cudaSuccess;
     // rows of the z-pass: stride = 1 mod 8 (fp32: 16) complex numbers, up to 16 rows in <= 100 KB (two blocks per SM)
     const int al = p->precision == SE_FP64 ? 8 : 16;
@@ -1088,7 +1091,7 @@ cudaError_t se_tune_xfft(se_plan *p)
             (inv ? p->f2_rbi : p->f2_rb) = brb;
             (inv ? p->f2_zithreads : p->f2_zthreads) = bth;
         }
-        const int NFy = p->precision == SE_FP64 ? SE_YF_NF64 : 24;
+        const int NFy = p->precision == SE_FP64 ? SE_YF_NF64 : SE_YF_NF32;
         int bby = p->f2_ythreads;
         float bty = 1e30f;
         for (int bw = 192 / NFy; bw >= 4; bw -= (NFy <= 12 ? 2 : 1)) {
